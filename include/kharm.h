@@ -1,0 +1,133 @@
+/* kharm.h -- C ABI of libkharm.so: the B200 (sm_100a) hot path of the KHARMA/HARM method.
+ *
+ * One explicit second-order (predictor-corrector) ideal-GRMHD update of a uniform logically
+ * Cartesian 3-D mesh block in a stationary metric, fp64, entirely in hand-written CUDA kernels.
+ * There is NO CPU fallback: every call that computes needs a CUDA device and fails with KH_ECUDA
+ * otherwise.
+ *
+ * Citations: "P:n" = PAPER.md line n.  The paper gives the scheme by citation (P:243 HARM, the
+ * modified 3-velocity, the 1D_W inversion, Flux-CT; P:253 MC / WENO5; P:255 predictor-corrector;
+ * P:111 FMKS; P:257-261 floors; P:317 the sub-step's task list) and prints eq. 1.1; the
+ * exact formulas adopted are the readings S1..S23 listed in DESIGN.md.
+ *
+ * Conventions
+ *   - primitives, 8 per zone: rho, u, ut^1, ut^2, ut^3, B^1, B^2, B^3  (ut = the velocity of P:243)
+ *   - arrays are fp64, SoA [var][k][j][i], x1 (i) fastest, C order, densely packed
+ *       with_ghosts = 0 : [8][n3][n2][n1]            interior only
+ *       with_ghosts = 1 : [8][n3+6][n2+6][n1+6]      KH_NG = 3 ghost layers per side in all directions
+ *   - `mem` says where a caller buffer lives: KH_MEM_DEVICE (a device pointer valid on the grid's
+ *     device; copies are enqueued on the grid's stream) or KH_MEM_HOST (a host pointer; the call
+ *     copies through the stream and returns after the copy completed)
+ *   - ownership: the library owns the grid and all internal buffers; callers own every buffer they pass
+ *   - errors: every call returns KH_OK (0) or a negative code; no exceptions or aborts cross the ABI;
+ *     out-parameters are untouched on error.  U->P failures are DATA (pflag), not errors.
+ *   - threading: calls on one grid must be serialised by the caller; all work is enqueued on the
+ *     stream given at creation (0 = the legacy default stream)
+ */
+#ifndef KHARM_H
+#define KHARM_H
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define KH_NG 3
+#define KH_NPRIM 8
+
+enum { KH_OK = 0, KH_EINVAL = -1, KH_ENOMEM = -2, KH_ECUDA = -3, KH_ENAN = -4 };
+enum { KH_MINKOWSKI = 0, KH_KS = 1, KH_FMKS = 2 };                            /* coords          */
+enum { KH_BC_PERIODIC = 0, KH_BC_OUTFLOW = 1, KH_BC_POLAR = 2, KH_BC_FIXED = 3 };
+enum { KH_RECON_MC = 0, KH_RECON_WENO5 = 1 };
+enum { KH_MEM_DEVICE = 0, KH_MEM_HOST = 1 };
+enum { KH_LOC_CENT = 0, KH_LOC_FACE1 = 1, KH_LOC_FACE2 = 2, KH_LOC_FACE3 = 3 };
+
+typedef struct {
+  int coords;                 /* KH_MINKOWSKI (Cartesian) | KH_KS (native = r,theta,phi) | KH_FMKS */
+  double a;                   /* black-hole spin (KS / FMKS)                                               */
+  double hslope, poly_xt, poly_alpha, mks_smooth;   /* FMKS map parameters (poly_alpha: even integer value) */
+  int n1, n2, n3;             /* interior zones; n3 == 1 runs a 2-D problem as a one-zone-thick block      */
+  double xmin[3], xmax[3];    /* native-coordinate bounds of the interior                                  */
+  int bc[6];                  /* x1lo x1hi x2lo x2hi x3lo x3hi; periodic must be set on both sides;
+                                 KH_BC_POLAR only in x2 (needs n2 >= 3)                                     */
+  double gamma, cfl;          /* adiabatic index; Courant factor                                           */
+  int recon;                  /* KH_RECON_MC | KH_RECON_WENO5                                              */
+  double rho_min, u_min, r_char, bsq_over_rho_max, bsq_over_u_max, u_over_rho_max, gamma_max; /* floors */
+  double dt_growth_max;       /* dt_next <= dt_growth_max * dt                                              */
+} kh_params;
+
+typedef struct kh_grid kh_grid;   /* opaque */
+
+/* Create a grid on the current CUDA device and run the one-time geometry precompute (kernel K1:
+ * gcov, gcon, sqrt(-g), lapse at zone centres and the three face centres, connection coefficients
+ * and floor profiles at centres; the "caches of expensive-to-calculate quantities" of P:285).
+ * cuda_stream: a cudaStream_t (as void*), or NULL for the default stream. */
+int kh_grid_create(const kh_params* params, void* cuda_stream, kh_grid** out);
+int kh_grid_destroy(kh_grid* g);
+
+/* Load primitives and fill the ghost zones (periodic / outflow / polar as configured; KH_BC_FIXED
+ * ghosts keep what a with_ghosts = 1 array supplies).  Kernel K7. */
+int kh_set_prims(kh_grid* g, const double* p, int with_ghosts, int mem);
+int kh_get_prims(kh_grid* g, double* p, int with_ghosts, int mem);
+
+/* Conserved variables U(P) = sqrt(-g)(rho u^t, T^t_t + rho u^t, T^t_i, B^i) at zone centres,
+ * interior [8][n3][n2][n1] (T from eq. 1.1). */
+int kh_get_cons(kh_grid* g, double* u, int mem);
+
+/* Flags of the LAST sub-step, interior [n3][n2][n1], as int32.  pflag: 0 ok, 1 bad input,
+ * 2 no convergence, 3 v^2 out of range, 4 rho <= 0, 5 u < 0, 6 both, 7 non-finite (1D_W inversion,
+ * P:243).  fflag: bits 1 rho geometric floor, 2 rho b^2 floor, 4 u geometric floor, 8 u b^2 floor,
+ * 16 u/rho ceiling, 32 Lorentz-factor ceiling.  Either pointer may be NULL. */
+int kh_get_flags(kh_grid* g, int* pflag, int* fflag, int mem);
+
+/* CFL time step from zone-centred fast-magnetosonic speeds (for the first step).  *dt is a HOST double. */
+int kh_estimate_dt(kh_grid* g, double* dt);
+
+/* One full predictor-corrector step:
+ *     P* = substep(P^n, P^n, dt/2);   P^{n+1} = substep(P^n, P*, dt)
+ * each sub-step = reconstruction + LLF fluxes per direction (K2), Flux-CT (K3), geometric source +
+ * conserved update + 1D_W inversion + floors (K4/K5), ghost fill (K7), fix-up of failed zones (K5b),
+ * ghost fill; the corrector's face speeds give the next CFL step (K6).
+ *   dt > 0   : use this step
+ *   dt <= 0  : use the device-resident dt_next of the previous step (no host round trip)
+ *   dt_next  : HOST pointer receiving min(cfl * min_zones dt_zone, dt_growth_max * dt), or NULL to
+ *              return without synchronising (the value stays on the device for the next dt <= 0 call) */
+int kh_step(kh_grid* g, double dt, double* dt_next);
+
+/* max |div B| of the corner-centred divergence that Flux-CT preserves.  HOST double. */
+int kh_divB(kh_grid* g, double* max_abs);
+
+/* Number of zones with pflag != 0 and with fflag != 0 in the last sub-step (HOST ints; may be NULL). */
+int kh_count_flags(kh_grid* g, long long* n_pflag, long long* n_fflag);
+
+/* ---- stage access (tests / debugging) ---- */
+/* Geometry tables over (j,i) with ghosts, [(n2+6)*(n1+6)] points: gcov/gcon as 16 doubles per point
+ * (row-major 4x4), gdet and alpha one per point.  Any pointer may be NULL. */
+int kh_get_geom(kh_grid* g, int loc, double* gcov16, double* gcon16, double* gdet, double* alpha, int mem);
+/* Connection Gamma^lam_{mu nu} at centres: 64 doubles per (j,i) point, [lam][mu][nu]. */
+int kh_get_conn(kh_grid* g, double* conn64, int mem);
+/* LLF face fluxes of direction dir (1..3) of the last sub-step, with ghosts [8][nt], index = lower
+ * face of the zone; hydro components as used by the update, B components replaced by their Flux-CT
+ * values (computed from the edge EMFs); ctop [nt].  Entries outside the computed face range are 0. */
+int kh_get_flux(kh_grid* g, int dir, double* F, double* ctop, int mem);
+/* Edge EMFs of the last sub-step, with ghosts [nt], index = lower edge of the zone. */
+int kh_get_emf(kh_grid* g, int dir, double* emf, int mem);
+/* Run the fix-up (K5b) + floors on the current primitives for a caller-supplied flag array
+ * (int32, with ghosts [nt]); test hook for hand-built neighbourhoods. */
+int kh_debug_fixup(kh_grid* g, const int* pflag_with_ghosts, int mem);
+/* Run only the predictor sub-step P* = substep(P^n, P^n, dt/2) and make P* the current state (test hook:
+ * exposes the intermediate state and the predictor's fluxes / flags to the stage getters). */
+int kh_debug_predictor(kh_grid* g, double dt);
+/* Number of kernel launches enqueued by this grid since creation. */
+long long kh_launch_count(const kh_grid* g);
+/* Enable/disable CUDA-graph replay of kh_step (default on); the first step after a change captures. */
+int kh_set_graph(kh_grid* g, int enable);
+/* Stand-alone DFMA-chain micro-benchmark: returns achieved fp64 TFLOP/s on the current device
+ * (HOST double) -- the measured fp64 peak used as an ALU roofline denominator by bench.py. */
+int kh_measure_fp64_peak(double* tflops, double* sm_mhz_est);
+
+const char* kh_strerror(int code);
+const char* kh_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -155,11 +155,41 @@ double invert4(const double g[4][4], double inv[4][4]) {
 
 struct Geom { double gcov[4][4], gcon[4][4], gdet, alpha; };
 
+// S6a: g^{mu nu} is the inverse of g_{mu nu} and sqrt(-g) the root of its determinant.  For KS / FMKS both
+// are evaluated from their CLOSED FORMS -- the Kerr-Schild inverse metric
+//   g^tt = -(1+2r/Sig), g^tr = 2r/Sig, g^rr = Delta/Sig, g^rphi = a/Sig, g^thth = 1/Sig, g^phph = 1/(Sig sin^2 th)
+// pushed through the inverse Jacobian of the coordinate map, and sqrt(-g) = Sig |sin th| r |dth/dx2| --
+// because the generic cofactor inverse loses ~(condition number) x eps near the polar axis (measured 1e-11
+// between two inversion algorithms).  The generic invert4() stays as the definition the closed form is
+// pinned against (tests: g * g^-1 = 1, det).
 void geom_at(const kho_params& p, double x1, double x2, Geom& G) {
   gcov_native<double>(p, x1, x2, G.gcov);
-  double det = invert4(G.gcov, G.gcon);
-  G.gdet = std::sqrt(-det);
-  G.alpha = 1.0 / std::sqrt(-G.gcon[0][0]);   // S6a
+  if (p.coords == KHO_MINKOWSKI) {
+    for (int m = 0; m < 4; m++) for (int n = 0; n < 4; n++) G.gcon[m][n] = G.gcov[m][n];
+    G.gdet = 1.0; G.alpha = 1.0;
+    return;
+  }
+  double r, th, t1 = 0.0, t2 = 1.0, jr = 1.0;     // jr = dr/dx1, t1 = dth/dx1, t2 = dth/dx2
+  if (p.coords == KHO_KS) { r = x1; th = x2; }
+  else { fmks_map<double>(p, x1, x2, r, th, t1, t2); jr = r; }
+  double s = std::sin(th), c = std::cos(th);
+  double Sig = r * r + p.a * p.a * c * c, f = 2.0 * r / Sig;
+  double ks[4][4] = {{0}};
+  ks[0][0] = -(1.0 + f);
+  ks[0][1] = ks[1][0] = f;
+  ks[1][1] = (r * r - 2.0 * r + p.a * p.a) / Sig;
+  ks[1][3] = ks[3][1] = p.a / Sig;
+  ks[2][2] = 1.0 / Sig;
+  ks[3][3] = 1.0 / (Sig * s * s);
+  double M[4][4] = {{0}};                          // M[native][emb] = d X_native / d X_emb
+  M[0][0] = 1.0; M[1][1] = 1.0 / jr; M[2][1] = -t1 / (jr * t2); M[2][2] = 1.0 / t2; M[3][3] = 1.0;
+  for (int m = 0; m < 4; m++) for (int n = 0; n < 4; n++) {
+    double acc = 0.0;
+    for (int al = 0; al < 4; al++) for (int be = 0; be < 4; be++) acc += M[m][al] * ks[al][be] * M[n][be];
+    G.gcon[m][n] = acc;
+  }
+  G.gdet = std::fabs(Sig * s * jr * t2);
+  G.alpha = 1.0 / std::sqrt(-G.gcon[0][0]);
 }
 void geom_zero(Geom& G) { std::memset(&G, 0, sizeof(G)); }
 
@@ -174,13 +204,13 @@ void conn_from_dg(const double gcon[4][4], const double dg[4][4][4] /* dg[k][m][
 void conn_exact(const kho_params& p, double x1, double x2, double conn[64]) {
   Dual g[4][4];
   gcov_native<Dual>(p, Dual(x1, 1.0, 0.0), Dual(x2, 0.0, 1.0), g);
-  double gc[4][4], gi[4][4], dg[4][4][4];
+  double dg[4][4][4];
   for (int m = 0; m < 4; m++) for (int n = 0; n < 4; n++) {
-    gc[m][n] = g[m][n].v;
     dg[0][m][n] = 0.0; dg[1][m][n] = g[m][n].d1; dg[2][m][n] = g[m][n].d2; dg[3][m][n] = 0.0;
   }
-  invert4(gc, gi);
-  conn_from_dg(gi, dg, conn);
+  Geom G;
+  geom_at(p, x1, x2, G);
+  conn_from_dg(G.gcon, dg, conn);
 }
 void conn_fd(const kho_params& p, double x1, double x2, double h, double conn[64]) {
   double gc[4][4], gi[4][4], dg[4][4][4], gp[4][4], gm[4][4];
@@ -270,7 +300,11 @@ void vchar(const Geom& G, const double P[NP], const FourVec& D, double gam, int 
   double A = ut * ut - (G.gcon[0][0] + ut * ut) * cms2;
   double B = 2.0 * (ud * ut - (G.gcon[0][dir] + ud * ut) * cms2);
   double C = ud * ud - (G.gcon[dir][dir] + ud * ud) * cms2;
-  double disc = B * B - 4.0 * A * C;
+  // Discriminant B^2 - 4AC in its algebraically reduced form: the O(1) terms (u^d u^t)^2 - (u^t)^2 (u^d)^2
+  // cancel identically, leaving  4 c_m^2 [ (1-c_m^2)(u^t^2 g^dd - 2 u^t u^d g^td + u^d^2 g^tt) + c_m^2 (g^td^2 - g^tt g^dd) ].
+  // Same number; the naive form loses eps/c_m^2 in cold zones (measured 1e-8 relative on ctop).
+  double disc = 4.0 * cms2 * ((1.0 - cms2) * (ut * ut * G.gcon[dir][dir] - 2.0 * ut * ud * G.gcon[0][dir] + ud * ud * G.gcon[0][0]) +
+                              cms2 * (G.gcon[0][dir] * G.gcon[0][dir] - G.gcon[0][0] * G.gcon[dir][dir]));
   if (!(disc >= 0.0)) disc = 0.0;
   double sq = std::sqrt(disc);
   // roots of A v^2 - B v + C = 0 (dispersion relation of a wave (-omega, k e_dir) with v = omega/k)
@@ -397,14 +431,16 @@ int u2p(const Geom& G, const double U[NP], const double Pg[NP], double gam, doub
   c.QdotB = Qcov[1] * Bc[1] + Qcov[2] * Bc[2] + Qcov[3] * Bc[3];
   c.QdotBsq = c.QdotB * c.QdotB;
   double Qdotn = -alpha * Qcon[0];
-  double Qsq = 0.0;
-  for (int m = 0; m < 4; m++) Qsq += Qcon[m] * Qcov[m];
-  c.Qtsq = Qsq + Qdotn * Qdotn;
   c.Ep = -Qdotn - c.D;
   double ncon[4];
   for (int m = 0; m < 4; m++) ncon[m] = -alpha * G.gcon[m][0];
   double Qtcon[4];
   for (int m = 0; m < 4; m++) Qtcon[m] = Qcon[m] + Qdotn * ncon[m];
+  // Qt^2 = Q.Q + (Q.n)^2, evaluated as the spatial norm g_ij Qt^i Qt^j of the projected vector (Qt^t = 0
+  // identically): the same number without the cancellation of two O(W^2) terms, so it can never come out
+  // negative by round-off and flip the v^2 >= 0 post-check (S16 / S15b: flags must not depend on rounding).
+  c.Qtsq = 0.0;
+  for (int i = 1; i < 4; i++) for (int j = 1; j < 4; j++) c.Qtsq += G.gcov[i][j] * Qtcon[i] * Qtcon[j];
 
   // guess from the guess primitives: W0 = (rho + Gamma u)(1 + q^2)
   double qsq = 0.0;
@@ -909,6 +945,13 @@ int kho_get_conn(kho_grid* g, double* conn64) {
   return KHO_OK;
 }
 // test hook: run the C9 fix-up (+ floors) on the current primitives with a caller-supplied flag array (with ghosts)
+// test hook: predictor sub-step only; P* becomes the current state
+int kho_debug_predictor(kho_grid* g, double dt) {
+  if (!g || !(dt > 0.0)) return KHO_EINVAL;
+  substep(*g, g->P.data(), g->P.data(), g->Ps.data(), 0.5 * dt);
+  g->P.swap(g->Ps);
+  return KHO_OK;
+}
 int kho_debug_fixup(kho_grid* g, const int* pflag_with_ghosts) {
   if (!g || !pflag_with_ghosts) return KHO_EINVAL;
   for (long n = 0; n < g->ntot; n++) { g->pflag[n] = pflag_with_ghosts[n]; g->fflag[n] = 0; }

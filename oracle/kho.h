@@ -59,7 +59,9 @@ int kho_get_geom(kho_grid* g, int loc, double* gcov16, double* gcon16, double* g
 int kho_get_conn(kho_grid* g, double* conn64);            /* [(n2+6)(n1+6)][lam][mu][nu]  */
 int kho_fill_ghosts(kho_grid* g);
 /* test hook: C9 fix-up (+ floors) of the current primitives for a caller-supplied pflag array [nt] */
-int kho_debug_fixup(kho_grid* g, const int* pflag_with_ghosts);                          /* on the current primitives    */
+int kho_debug_fixup(kho_grid* g, const int* pflag_with_ghosts);
+/* test hook: predictor sub-step only; P* becomes the current state */
+int kho_debug_predictor(kho_grid* g, double dt);
 
 /* ---- point-wise pieces, exposed so tests can pin them one by one ---- */
 /* embedding coordinates (r, theta, phi) or (x,y,z) of a native point */

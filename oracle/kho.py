@@ -249,6 +249,9 @@ class Grid:
         _chk(self.L.kho_get_conn(self.h, _ptr(cn)))
         return cn.reshape(self.shape_gh[2:] + (4, 4, 4))
 
+    def debug_predictor(self, dt):
+        _chk(self.L.kho_debug_predictor(self.h, C.c_double(dt)))
+
     def debug_fixup(self, pflag_with_ghosts):
         pf = np.ascontiguousarray(pflag_with_ghosts, dtype=np.int32)
         assert pf.shape == self.shape_gh[1:]

@@ -1,0 +1,563 @@
+// kharm.cu -- C ABI (include/kharm.h) and host orchestration of the HARM step on one B200.
+// All arithmetic of the path runs in the kernels of kh_kernels.cuh / kh_geometry.cuh; the host
+// only validates arguments, owns device buffers and enqueues launches on the grid's stream.
+#include "../../include/kharm.h"
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "kh_geometry.cuh"
+#include "kh_kernels.cuh"
+
+using namespace kh;
+
+static thread_local char g_cuda_err[256] = "";
+
+#define CK(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess) {                                                                       \
+      snprintf(g_cuda_err, sizeof(g_cuda_err), "%s at %s:%d", cudaGetErrorString(e_), __FILE__, __LINE__); \
+      return (e_ == cudaErrorMemoryAllocation) ? KH_ENOMEM : KH_ECUDA;                             \
+    }                                                                                              \
+  } while (0)
+
+struct kh_grid {
+  kh_params p;
+  GV gv;
+  cudaStream_t stream;
+  bool own_stream;
+  bool flat;
+  // device buffers
+  double* geom[4];
+  double* conn;
+  double* floorp;
+  double* P[3];          // P^n, P*, P^{n+1} (rotating)
+  double* F[3];          // face fluxes per direction, [8][ntot]
+  double* ctop[3];
+  double* emf[3];
+  unsigned char *pflag, *fflag;
+  double* fix;           // [5][ntot] scratch of the fix-up (pre-fix-up snapshot semantics)
+  double* stage;         // lazily allocated [8][ntot] staging buffer for host transfers / debug copies
+  StepScalars* sc;       // device
+  StepScalars* sc_host;  // pinned
+  int cur;               // index of P^n in P[]
+  long long launches;
+  // CUDA graphs of a full step, one per rotation state of the P buffers
+  bool use_graph;
+  cudaGraphExec_t gexec[3];
+  long long graph_launches;   // kernel launches inside one captured step
+};
+
+static inline dim3 zone_grid(int nx, int ny, int nz) { return dim3((nx + 127) / 128, ny, nz); }
+
+static int fill_ghosts(kh_grid* g, double* P, unsigned char* flag, int only_if_failed) {
+  const GV& v = g->gv;
+  long t0 = (long)2 * KH_NGH * v.nt2 * v.nt3, t1 = (long)2 * KH_NGH * v.nt1 * v.nt3, t2 = (long)2 * KH_NGH * v.nt1 * v.nt2;
+  fill_kernel<0><<<(unsigned)((t0 + 127) / 128), 128, 0, g->stream>>>(v, P, flag, g->sc, only_if_failed);
+  fill_kernel<1><<<(unsigned)((t1 + 127) / 128), 128, 0, g->stream>>>(v, P, flag, g->sc, only_if_failed);
+  fill_kernel<2><<<(unsigned)((t2 + 127) / 128), 128, 0, g->stream>>>(v, P, flag, g->sc, only_if_failed);
+  g->launches += 3;
+  CK(cudaGetLastError());
+  return KH_OK;
+}
+
+template <int DIR>
+static void launch_flux(kh_grid* g, const double* Ps) {
+  const GV& v = g->gv;
+  int c1 = v.n1 + (DIR == 1 ? 1 : 2), c2 = v.n2 + (DIR == 2 ? 1 : 2), c3 = v.n3 + (DIR == 3 ? 1 : 2);
+  dim3 grid = zone_grid(c1, c2, c3);
+  double* F = g->F[DIR - 1];
+  double* ct = g->ctop[DIR - 1];
+  if (g->flat) {
+    if (g->p.recon == KH_RECON_MC) flux_kernel<DIR, 0, true><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct);
+    else flux_kernel<DIR, 1, true><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct);
+  } else {
+    if (g->p.recon == KH_RECON_MC) flux_kernel<DIR, 0, false><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct);
+    else flux_kernel<DIR, 1, false><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct);
+  }
+  g->launches++;
+}
+
+static int do_fixup(kh_grid* g, double* Pf, int force) {
+  const GV& v = g->gv;
+  dim3 grid = zone_grid(v.n1, v.n2, v.n3);
+  double* fix = g->fix;
+  fixup_gather_kernel<<<grid, 128, 0, g->stream>>>(v, Pf, g->pflag, fix, g->sc, force);
+  if (g->flat) fixup_apply_kernel<true><<<grid, 128, 0, g->stream>>>(v, Pf, g->pflag, g->fflag, fix, g->sc, force);
+  else fixup_apply_kernel<false><<<grid, 128, 0, g->stream>>>(v, Pf, g->pflag, g->fflag, fix, g->sc, force);
+  g->launches += 2;
+  CK(cudaGetLastError());
+  return KH_OK;
+}
+
+// One sub-step (S22): fluxes from Ps, update of U(Pi), inversion with guess Pi, floors, fill, fix-up, fill.
+static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, double dt_factor, bool corrector) {
+  const GV& v = g->gv;
+  reset_counters_kernel<<<1, 1, 0, g->stream>>>(g->sc);
+  g->launches++;
+  launch_flux<1>(g, Ps);
+  launch_flux<2>(g, Ps);
+  launch_flux<3>(g, Ps);
+  emf_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], g->emf[2]);
+  g->launches++;
+  dim3 grid = zone_grid(v.n1, v.n2, v.n3);
+#define UPD(FL, CO)                                                                                                  \
+  update_kernel<FL, CO><<<grid, 128, 0, g->stream>>>(v, Pi, Ps, Pf, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], \
+                                                     g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, g->fflag, g->sc, dt_factor)
+  if (g->flat) { if (corrector) UPD(true, true); else UPD(true, false); }
+  else { if (corrector) UPD(false, true); else UPD(false, false); }
+#undef UPD
+  g->launches++;
+  CK(cudaGetLastError());
+  int rc = fill_ghosts(g, Pf, g->pflag, 0);
+  if (rc) return rc;
+  rc = do_fixup(g, Pf, 0);
+  if (rc) return rc;
+  return fill_ghosts(g, Pf, nullptr, 1);
+}
+
+static int enqueue_step(kh_grid* g, int cur) {
+  double *Pn = g->P[cur], *Pstar = g->P[(cur + 1) % 3], *Pnew = g->P[(cur + 2) % 3];
+  int rc = substep(g, Pn, Pn, Pstar, 0.5, false);
+  if (rc) return rc;
+  rc = substep(g, Pn, Pstar, Pnew, 1.0, true);
+  if (rc) return rc;
+  finalize_dt_kernel<<<1, 1, 0, g->stream>>>(g->sc, g->p.cfl, g->p.dt_growth_max);
+  g->launches++;
+  CK(cudaGetLastError());
+  return KH_OK;
+}
+
+static int ensure_stage(kh_grid* g) {
+  if (g->stage) return KH_OK;
+  size_t a = sizeof(double) * KH_NP * g->gv.ntot, b = sizeof(double) * 64 * g->gv.n2d;
+  CK(cudaMalloc((void**)&g->stage, a > b ? a : b));
+  return KH_OK;
+}
+
+static void destroy_graphs(kh_grid* g) {
+  for (int c = 0; c < 3; c++)
+    if (g->gexec[c]) { cudaGraphExecDestroy(g->gexec[c]); g->gexec[c] = nullptr; }
+}
+
+extern "C" {
+
+const char* kh_strerror(int code) {
+  switch (code) {
+    case KH_OK: return "ok";
+    case KH_EINVAL: return "invalid argument";
+    case KH_ENOMEM: return "out of memory";
+    case KH_ECUDA: return "CUDA error (see kh_last_cuda_error)";
+    case KH_ENAN: return "non-finite value";
+    default: return "unknown error";
+  }
+}
+const char* kh_last_cuda_error(void) { return g_cuda_err; }
+
+int kh_grid_destroy(kh_grid* g) {
+  if (!g) return KH_OK;
+  destroy_graphs(g);
+  for (int l = 0; l < 4; l++) cudaFree(g->geom[l]);
+  cudaFree(g->conn); cudaFree(g->floorp);
+  for (int b = 0; b < 3; b++) { cudaFree(g->P[b]); cudaFree(g->F[b]); cudaFree(g->ctop[b]); cudaFree(g->emf[b]); }
+  cudaFree(g->pflag); cudaFree(g->fflag); cudaFree(g->sc); cudaFree(g->fix); cudaFree(g->stage);
+  if (g->sc_host) cudaFreeHost(g->sc_host);
+  if (g->own_stream) cudaStreamDestroy(g->stream);
+  delete g;
+  return KH_OK;
+}
+
+int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
+  if (!p || !out) return KH_EINVAL;
+  if (p->n1 < 1 || p->n2 < 1 || p->n3 < 1) return KH_EINVAL;
+  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1) return KH_EINVAL;
+  if (!(p->gamma > 1.0) || !(p->cfl > 0.0) || !(p->dt_growth_max > 0.0)) return KH_EINVAL;
+  const int N[3] = {p->n1, p->n2, p->n3};
+  for (int d = 0; d < 3; d++) {
+    if (!(p->xmax[d] > p->xmin[d])) return KH_EINVAL;
+    for (int s = 0; s < 2; s++) {
+      int bc = p->bc[2 * d + s];
+      if (bc < 0 || bc > 3) return KH_EINVAL;
+      if (bc == KH_BC_POLAR && (d != 1 || N[d] < KH_NGH)) return KH_EINVAL;
+    }
+    if ((p->bc[2 * d] == KH_BC_PERIODIC) != (p->bc[2 * d + 1] == KH_BC_PERIODIC)) return KH_EINVAL;
+  }
+  int ndev = 0;
+  CK(cudaGetDeviceCount(&ndev));
+  if (ndev < 1) { snprintf(g_cuda_err, sizeof(g_cuda_err), "no CUDA device"); return KH_ECUDA; }
+
+  kh_grid* g = new (std::nothrow) kh_grid;
+  if (!g) return KH_ENOMEM;
+  memset(g, 0, sizeof(*g));
+  g->p = *p;
+  g->stream = (cudaStream_t)cuda_stream;
+  if (!g->stream) {
+    // The legacy default stream cannot be captured into a CUDA graph: use an own BLOCKING stream, which
+    // still orders against work the caller enqueues on the legacy default stream.
+    if (cudaStreamCreateWithFlags(&g->stream, cudaStreamDefault) != cudaSuccess) { delete g; return KH_ECUDA; }
+    g->own_stream = true;
+  }
+  g->flat = (p->coords == KH_MINKOWSKI);
+  g->use_graph = true;
+  GV& v = g->gv;
+  v.n1 = p->n1; v.n2 = p->n2; v.n3 = p->n3;
+  v.nt1 = v.n1 + 2 * KH_NGH; v.nt2 = v.n2 + 2 * KH_NGH; v.nt3 = v.n3 + 2 * KH_NGH;
+  v.s2 = v.nt1; v.s3 = (long)v.nt1 * v.nt2; v.ntot = v.s3 * v.nt3;
+  v.n2d = (long)v.nt1 * v.nt2;
+  v.idx1 = v.n1 / (p->xmax[0] - p->xmin[0]); v.idx2 = v.n2 / (p->xmax[1] - p->xmin[1]); v.idx3 = v.n3 / (p->xmax[2] - p->xmin[2]);
+  v.gam = p->gamma;
+  for (int b = 0; b < 6; b++) v.bc[b] = p->bc[b];
+  v.polar_lo = p->bc[2] == KH_BC_POLAR; v.polar_hi = p->bc[3] == KH_BC_POLAR;
+  v.ndim_mask = (v.n1 > 1 ? 1 : 0) | (v.n2 > 1 ? 2 : 0) | (v.n3 > 1 ? 4 : 0);
+  v.fp.bsq_over_rho_max = p->bsq_over_rho_max; v.fp.bsq_over_u_max = p->bsq_over_u_max;
+  v.fp.u_over_rho_max = p->u_over_rho_max; v.fp.gamma_max = p->gamma_max;
+
+#define ALLOC(ptr, bytes)                                                       \
+  do {                                                                          \
+    cudaError_t e_ = cudaMalloc((void**)&(ptr), (bytes));                       \
+    if (e_ != cudaSuccess) { snprintf(g_cuda_err, sizeof(g_cuda_err), "%s (alloc %zu B)", cudaGetErrorString(e_), (size_t)(bytes)); kh_grid_destroy(g); return e_ == cudaErrorMemoryAllocation ? KH_ENOMEM : KH_ECUDA; } \
+    e_ = cudaMemsetAsync((ptr), 0, (bytes), g->stream);                         \
+    if (e_ != cudaSuccess) { kh_grid_destroy(g); return KH_ECUDA; }             \
+  } while (0)
+  const size_t fb = sizeof(double) * v.ntot;
+  for (int l = 0; l < 4; l++) ALLOC(g->geom[l], sizeof(double) * KH_NGEO * v.n2d);
+  ALLOC(g->conn, sizeof(double) * KH_NCONN * v.n2d);
+  ALLOC(g->floorp, sizeof(double) * 2 * v.n2d);
+  for (int b = 0; b < 3; b++) {
+    ALLOC(g->P[b], KH_NP * fb);
+    ALLOC(g->F[b], KH_NP * fb);
+    ALLOC(g->ctop[b], fb);
+    ALLOC(g->emf[b], fb);
+  }
+  ALLOC(g->fix, 5 * fb);
+  ALLOC(g->pflag, v.ntot);
+  ALLOC(g->fflag, v.ntot);
+  ALLOC(g->sc, sizeof(StepScalars));
+#undef ALLOC
+  if (cudaMallocHost((void**)&g->sc_host, sizeof(StepScalars)) != cudaSuccess) { kh_grid_destroy(g); return KH_ENOMEM; }
+  memset(g->sc_host, 0, sizeof(StepScalars));
+  g->sc_host->min_bits = 0x7FF0000000000000ULL;
+  if (cudaMemcpyAsync(g->sc, g->sc_host, sizeof(StepScalars), cudaMemcpyHostToDevice, g->stream) != cudaSuccess) { kh_grid_destroy(g); return KH_ECUDA; }
+  for (int l = 0; l < 4; l++) v.geom[l] = g->geom[l];
+  v.conn = g->conn; v.floorp = g->floorp;
+
+  GeomPar gp;
+  gp.coords = p->coords; gp.a = p->a; gp.hslope = p->hslope; gp.poly_xt = p->poly_xt; gp.poly_alpha = p->poly_alpha;
+  gp.mks_smooth = p->mks_smooth; gp.x1_start = p->xmin[0];
+  gp.xmin1 = p->xmin[0]; gp.xmin2 = p->xmin[1];
+  gp.dx1 = (p->xmax[0] - p->xmin[0]) / v.n1; gp.dx2 = (p->xmax[1] - p->xmin[1]) / v.n2;
+  gp.nt1 = v.nt1; gp.nt2 = v.nt2; gp.n2 = v.n2; gp.polar_lo = v.polar_lo; gp.polar_hi = v.polar_hi;
+  gp.rho_min = p->rho_min; gp.u_min = p->u_min; gp.r_char = p->r_char; gp.gamma = p->gamma;
+  geometry_kernel<<<dim3((v.nt1 + 63) / 64, v.nt2), 64, 0, g->stream>>>(gp, g->geom[0], g->geom[1], g->geom[2], g->geom[3], g->conn, g->floorp);
+  g->launches++;
+  cudaError_t e = cudaStreamSynchronize(g->stream);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) { snprintf(g_cuda_err, sizeof(g_cuda_err), "%s (geometry)", cudaGetErrorString(e)); kh_grid_destroy(g); return KH_ECUDA; }
+  *out = g;
+  return KH_OK;
+}
+
+// copy helper: device<->caller buffer, host buffers synchronise
+static int xfer(kh_grid* g, void* dst, const void* src, size_t bytes, int mem, bool to_caller) {
+  cudaMemcpyKind kind = (mem == KH_MEM_HOST) ? (to_caller ? cudaMemcpyDeviceToHost : cudaMemcpyHostToDevice) : cudaMemcpyDeviceToDevice;
+  CK(cudaMemcpyAsync(dst, src, bytes, kind, g->stream));
+  if (mem == KH_MEM_HOST) CK(cudaStreamSynchronize(g->stream));
+  return KH_OK;
+}
+
+int kh_set_prims(kh_grid* g, const double* p, int with_ghosts, int mem) {
+  if (!g || !p || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  const GV& v = g->gv;
+  double* Pn = g->P[g->cur];
+  int rc;
+  if (with_ghosts) {
+    rc = xfer(g, Pn, p, sizeof(double) * KH_NP * v.ntot, mem, false);
+    if (rc) return rc;
+    // FIXED ghosts must exist in every rotating buffer
+    for (int b = 1; b < 3; b++) CK(cudaMemcpyAsync(g->P[(g->cur + b) % 3], Pn, sizeof(double) * KH_NP * v.ntot, cudaMemcpyDeviceToDevice, g->stream));
+  } else {
+    size_t bytes = sizeof(double) * KH_NP * (size_t)v.n1 * v.n2 * v.n3;
+    const double* src = p;
+    if (mem == KH_MEM_HOST) {
+      rc = ensure_stage(g);
+      if (rc) return rc;
+      rc = xfer(g, g->stage, p, bytes, mem, false);
+      if (rc) return rc;
+      src = g->stage;
+    }
+    pack_interior_kernel<<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, src, Pn, 1, KH_NP);
+    g->launches++;
+    CK(cudaGetLastError());
+  }
+  rc = fill_ghosts(g, Pn, nullptr, 0);
+  if (rc) return rc;
+  if (mem == KH_MEM_HOST) CK(cudaStreamSynchronize(g->stream));
+  return KH_OK;
+}
+
+int kh_get_prims(kh_grid* g, double* p, int with_ghosts, int mem) {
+  if (!g || !p || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  const GV& v = g->gv;
+  if (with_ghosts) return xfer(g, p, g->P[g->cur], sizeof(double) * KH_NP * v.ntot, mem, true);
+  size_t bytes = sizeof(double) * KH_NP * (size_t)v.n1 * v.n2 * v.n3;
+  if (mem == KH_MEM_HOST) { int rc = ensure_stage(g); if (rc) return rc; }
+  double* dst = (mem == KH_MEM_HOST) ? g->stage : p;
+  pack_interior_kernel<<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, g->P[g->cur], dst, 0, KH_NP);
+  g->launches++;
+  CK(cudaGetLastError());
+  if (mem == KH_MEM_HOST) return xfer(g, p, dst, bytes, mem, true);
+  return KH_OK;
+}
+
+int kh_get_cons(kh_grid* g, double* u, int mem) {
+  if (!g || !u || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  const GV& v = g->gv;
+  size_t bytes = sizeof(double) * KH_NP * (size_t)v.n1 * v.n2 * v.n3;
+  if (mem == KH_MEM_HOST) { int rc = ensure_stage(g); if (rc) return rc; }
+  double* dst = (mem == KH_MEM_HOST) ? g->stage : u;
+  if (g->flat) cons_kernel<true><<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, g->P[g->cur], dst);
+  else cons_kernel<false><<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, g->P[g->cur], dst);
+  g->launches++;
+  CK(cudaGetLastError());
+  if (mem == KH_MEM_HOST) return xfer(g, u, dst, bytes, mem, true);
+  return KH_OK;
+}
+
+int kh_get_flags(kh_grid* g, int* pflag, int* fflag, int mem) {
+  if (!g || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  const GV& v = g->gv;
+  size_t nin = (size_t)v.n1 * v.n2 * v.n3;
+  int* outs[2] = {pflag, fflag};
+  unsigned char* srcs[2] = {g->pflag, g->fflag};
+  for (int a = 0; a < 2; a++) {
+    if (!outs[a]) continue;
+    if (mem == KH_MEM_HOST) { int rc = ensure_stage(g); if (rc) return rc; }
+    int* dst = (mem == KH_MEM_HOST) ? (int*)g->stage : outs[a];
+    flags_to_int_kernel<<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, srcs[a], dst);
+    g->launches++;
+    CK(cudaGetLastError());
+    if (mem == KH_MEM_HOST) { int rc = xfer(g, outs[a], dst, sizeof(int) * nin, mem, true); if (rc) return rc; }
+  }
+  return KH_OK;
+}
+
+static int read_scalars(kh_grid* g) {
+  CK(cudaMemcpyAsync(g->sc_host, g->sc, sizeof(StepScalars), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return KH_OK;
+}
+
+int kh_estimate_dt(kh_grid* g, double* dt) {
+  if (!g || !dt) return KH_EINVAL;
+  const GV& v = g->gv;
+  if (g->flat) estimate_dt_kernel<true><<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, g->P[g->cur], g->sc);
+  else estimate_dt_kernel<false><<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, g->P[g->cur], g->sc);
+  g->launches++;
+  CK(cudaGetLastError());
+  int rc = read_scalars(g);
+  if (rc) return rc;
+  double m;
+  memcpy(&m, &g->sc_host->min_bits, sizeof(double));
+  unsigned long long inf = 0x7FF0000000000000ULL;
+  CK(cudaMemcpyAsync(&g->sc->min_bits, &inf, sizeof(inf), cudaMemcpyHostToDevice, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  if (!(m == m)) return KH_ENAN;
+  *dt = g->p.cfl * m;
+  return KH_OK;
+}
+
+int kh_step(kh_grid* g, double dt, double* dt_next) {
+  if (!g || dt != dt) return KH_EINVAL;
+  set_dt_kernel<<<1, 1, 0, g->stream>>>(g->sc, dt, dt > 0.0 ? 0 : 1);
+  g->launches++;
+  CK(cudaGetLastError());
+  int cur = g->cur;
+  if (g->use_graph) {
+    if (!g->gexec[cur]) {
+      long long before = g->launches;
+      cudaGraph_t graph;
+      CK(cudaStreamBeginCapture(g->stream, cudaStreamCaptureModeThreadLocal));
+      int rc = enqueue_step(g, cur);
+      cudaError_t e = cudaStreamEndCapture(g->stream, &graph);
+      if (rc) return rc;
+      CK(e);
+      g->graph_launches = g->launches - before;
+      g->launches = before;
+      CK(cudaGraphInstantiate(&g->gexec[cur], graph, 0));
+      cudaGraphDestroy(graph);
+    }
+    CK(cudaGraphLaunch(g->gexec[cur], g->stream));
+    g->launches += g->graph_launches;
+  } else {
+    int rc = enqueue_step(g, cur);
+    if (rc) return rc;
+  }
+  g->cur = (cur + 2) % 3;
+  if (dt_next) {
+    int rc = read_scalars(g);
+    if (rc) return rc;
+    *dt_next = g->sc_host->dt_next;
+  }
+  return KH_OK;
+}
+
+int kh_divB(kh_grid* g, double* max_abs) {
+  if (!g || !max_abs) return KH_EINVAL;
+  const GV& v = g->gv;
+  int lo[3], cnt[3];
+  const int N[3] = {v.n1, v.n2, v.n3};
+  for (int d = 0; d < 3; d++) { lo[d] = (g->p.bc[2 * d] == KH_BC_PERIODIC) ? 0 : 1; cnt[d] = N[d] - lo[d]; }
+  unsigned long long zero = 0;
+  CK(cudaMemcpyAsync(&g->sc->max_bits, &zero, sizeof(zero), cudaMemcpyHostToDevice, g->stream));
+  if (cnt[0] > 0 && cnt[1] > 0 && cnt[2] > 0) {
+    divb_kernel<<<zone_grid(cnt[0], cnt[1], cnt[2]), 128, 0, g->stream>>>(v, g->P[g->cur], g->sc, lo[0], lo[1], lo[2]);
+    g->launches++;
+    CK(cudaGetLastError());
+  }
+  int rc = read_scalars(g);
+  if (rc) return rc;
+  memcpy(max_abs, &g->sc_host->max_bits, sizeof(double));
+  return KH_OK;
+}
+
+int kh_count_flags(kh_grid* g, long long* n_pflag, long long* n_fflag) {
+  if (!g) return KH_EINVAL;
+  int rc = read_scalars(g);
+  if (rc) return rc;
+  if (n_pflag) *n_pflag = (long long)g->sc_host->n_pflag;
+  if (n_fflag) *n_fflag = (long long)g->sc_host->n_fflag;
+  return KH_OK;
+}
+
+int kh_get_geom(kh_grid* g, int loc, double* gcov16, double* gcon16, double* gdet, double* alpha, int mem) {
+  if (!g || loc < 0 || loc > 3 || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  const long n2d = g->gv.n2d;
+  double *d_cov = gcov16, *d_con = gcon16, *d_det = gdet, *d_al = alpha;
+  if (mem == KH_MEM_HOST) {
+    int rc = ensure_stage(g);
+    if (rc) return rc;
+    double* s = g->stage;   // >= 64 * n2d doubles
+    d_cov = gcov16 ? s : nullptr; d_con = gcon16 ? s + 16 * n2d : nullptr; d_det = gdet ? s + 32 * n2d : nullptr; d_al = alpha ? s + 33 * n2d : nullptr;
+  }
+  geom_export_kernel<<<(unsigned)((n2d + 127) / 128), 128, 0, g->stream>>>(n2d, g->geom[loc], d_cov, d_con, d_det, d_al);
+  g->launches++;
+  CK(cudaGetLastError());
+  if (mem == KH_MEM_HOST) {
+    if (gcov16) CK(cudaMemcpyAsync(gcov16, d_cov, sizeof(double) * 16 * n2d, cudaMemcpyDeviceToHost, g->stream));
+    if (gcon16) CK(cudaMemcpyAsync(gcon16, d_con, sizeof(double) * 16 * n2d, cudaMemcpyDeviceToHost, g->stream));
+    if (gdet) CK(cudaMemcpyAsync(gdet, d_det, sizeof(double) * n2d, cudaMemcpyDeviceToHost, g->stream));
+    if (alpha) CK(cudaMemcpyAsync(alpha, d_al, sizeof(double) * n2d, cudaMemcpyDeviceToHost, g->stream));
+    CK(cudaStreamSynchronize(g->stream));
+  }
+  return KH_OK;
+}
+
+int kh_get_conn(kh_grid* g, double* conn64, int mem) {
+  if (!g || !conn64 || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  const long n2d = g->gv.n2d;
+  if (mem == KH_MEM_HOST) { int rc = ensure_stage(g); if (rc) return rc; }
+  double* dst = (mem == KH_MEM_HOST) ? g->stage : conn64;
+  conn_export_kernel<<<(unsigned)((n2d + 127) / 128), 128, 0, g->stream>>>(n2d, g->conn, dst);
+  g->launches++;
+  CK(cudaGetLastError());
+  if (mem == KH_MEM_HOST) return xfer(g, conn64, dst, sizeof(double) * 64 * n2d, mem, true);
+  return KH_OK;
+}
+
+int kh_get_flux(kh_grid* g, int dir, double* F, double* ctop, int mem) {
+  if (!g || dir < 1 || dir > 3 || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  const GV& v = g->gv;
+  const size_t fb = sizeof(double) * v.ntot;
+  if (F) {
+    int rc = ensure_stage(g);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(g->stage, g->F[dir - 1], KH_NP * fb, cudaMemcpyDeviceToDevice, g->stream));
+    ct_flux_debug_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, dir, g->stage, g->emf[0], g->emf[1], g->emf[2]);
+    g->launches++;
+    CK(cudaGetLastError());
+    rc = xfer(g, F, g->stage, KH_NP * fb, mem, true);
+    if (rc) return rc;
+  }
+  if (ctop) return xfer(g, ctop, g->ctop[dir - 1], fb, mem, true);
+  return KH_OK;
+}
+
+int kh_get_emf(kh_grid* g, int dir, double* emf, int mem) {
+  if (!g || !emf || dir < 1 || dir > 3 || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  return xfer(g, emf, g->emf[dir - 1], sizeof(double) * g->gv.ntot, mem, true);
+}
+
+int kh_debug_predictor(kh_grid* g, double dt) {
+  if (!g || !(dt > 0.0)) return KH_EINVAL;
+  set_dt_kernel<<<1, 1, 0, g->stream>>>(g->sc, dt, 0);
+  g->launches++;
+  int rc = substep(g, g->P[g->cur], g->P[g->cur], g->P[(g->cur + 1) % 3], 0.5, false);
+  if (rc) return rc;
+  g->cur = (g->cur + 1) % 3;
+  CK(cudaStreamSynchronize(g->stream));
+  return KH_OK;
+}
+
+int kh_debug_fixup(kh_grid* g, const int* pflag_with_ghosts, int mem) {
+  if (!g || !pflag_with_ghosts || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  const GV& v = g->gv;
+  const int* src = pflag_with_ghosts;
+  if (mem == KH_MEM_HOST) {
+    int rc = ensure_stage(g);
+    if (rc) return rc;
+    rc = xfer(g, g->stage, pflag_with_ghosts, sizeof(int) * v.ntot, mem, false);
+    if (rc) return rc;
+    src = (const int*)g->stage;
+  }
+  int_to_flags_kernel<<<(unsigned)((v.ntot + 127) / 128), 128, 0, g->stream>>>(v.ntot, src, g->pflag);
+  g->launches++;
+  CK(cudaMemsetAsync(g->fflag, 0, v.ntot, g->stream));
+  int rc = do_fixup(g, g->P[g->cur], 1);
+  if (rc) return rc;
+  CK(cudaStreamSynchronize(g->stream));
+  return KH_OK;
+}
+
+long long kh_launch_count(const kh_grid* g) { return g ? g->launches : 0; }
+
+int kh_set_graph(kh_grid* g, int enable) {
+  if (!g) return KH_EINVAL;
+  g->use_graph = enable != 0;
+  if (!enable) destroy_graphs(g);
+  return KH_OK;
+}
+
+int kh_measure_fp64_peak(double* tflops, double* sm_mhz_est) {
+  if (!tflops) return KH_EINVAL;
+  int dev = 0, sms = 0;
+  CK(cudaGetDevice(&dev));
+  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int threads = 256, blocks = sms * 8, iters = 1 << 15;
+  double* out = nullptr;
+  CK(cudaMalloc((void**)&out, sizeof(double) * threads * blocks));
+  cudaEvent_t e0, e1;
+  CK(cudaEventCreate(&e0));
+  CK(cudaEventCreate(&e1));
+  dfma_peak_kernel<<<blocks, threads>>>(out, iters);   // warm-up
+  double best = 0.0;
+  for (int rep = 0; rep < 5; rep++) {
+    CK(cudaEventRecord(e0));
+    dfma_peak_kernel<<<blocks, threads>>>(out, iters);
+    CK(cudaEventRecord(e1));
+    CK(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, e0, e1));
+    double fl = 2.0 * 8.0 * (double)iters * threads * blocks;
+    double tf = fl / (ms * 1e-3) / 1e12;
+    if (tf > best) best = tf;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(out);
+  *tflops = best;
+  if (sm_mhz_est) *sm_mhz_est = best * 1e12 / (2.0 * 64.0 * sms) / 1e6;   // assuming 64 fp64 FMA lanes per SM
+  return KH_OK;
+}
+
+}  // extern "C"

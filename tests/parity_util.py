@@ -1,0 +1,66 @@
+"""Comparison metric between the CUDA path and the oracle (reading S23).
+
+Per zone: rho, u: |d|/|ref|; velocities: |d ut^i| sqrt(g_ii) / max(sqrt(q^2), 1e-3);
+field: |d B^i| sqrt(g_ii) / max(|B|, 1e-3 max_block |B|).  "After one step": max over interior zones
+<= 1e-10 (BASELINE.json north_star).  "Full run": L1 = sum|d| / sum|ref| per primitive <= 1e-8.
+"""
+import numpy as np
+
+from kharm_inputs import geometry
+
+TOL_ONE_STEP = 1e-10
+TOL_RUN_L1 = 1e-8
+EPS = 2.220446049250313e-16
+
+
+def zone_metric(p):
+    """gcov at zone centres, interior, [n2, n1, 4, 4] (numpy formulas of kharm_inputs)."""
+    x1, x2, _ = geometry.zone_coords(p)
+    X2, X1 = np.meshgrid(x2, x1, indexing="ij")
+    return geometry.gcov_native(p, X1, X2)
+
+
+def rel_diff(p, got, ref):
+    """Per-primitive, per-zone relative difference [8][n3][n2][n1] in the S23 metric."""
+    gcov = zone_metric(p)
+    gs = gcov[..., 1:, 1:]
+    out = np.zeros_like(ref)
+    out[0] = np.abs(got[0] - ref[0]) / np.abs(ref[0])
+    out[1] = np.abs(got[1] - ref[1]) / np.abs(ref[1])
+    v = np.moveaxis(ref[2:5], 0, -1)
+    q = np.sqrt(np.einsum("kjia,jiab,kjib->kji", v, gs, v))
+    B = np.moveaxis(ref[5:8], 0, -1)
+    bn = np.sqrt(np.einsum("kjia,jiab,kjib->kji", B, gs, B))
+    bfloor = 1e-3 * bn.max() if bn.max() > 0 else 1.0
+    for i in range(3):
+        gii = np.sqrt(gcov[..., i + 1, i + 1])[None]
+        out[2 + i] = np.abs(got[2 + i] - ref[2 + i]) * gii / np.maximum(q, 1e-3)
+        out[5 + i] = np.abs(got[5 + i] - ref[5 + i]) * gii / np.maximum(bn, bfloor)
+    return out
+
+
+def conditioning(p, ref, gamma):
+    """eps (rho + b^2) / u: the inherent round-off amplification of the internal energy in U -> P
+    (S16 'conditioning caveat').  b^2 is bounded by |B|^2 gamma^2-ish; we use g_ij B^i B^j."""
+    gcov = zone_metric(p)
+    B = np.moveaxis(ref[5:8], 0, -1)
+    b2 = np.einsum("kjia,jiab,kjib->kji", B, gcov[..., 1:, 1:], B)
+    return EPS * (ref[0] + b2) / ref[1]
+
+
+def l1_diff(p, got, ref):
+    """L1 difference per primitive: sum|d| / sum|ref| for rho, u; for the vector components the denominator
+    is the sum of the vector's norm (sum sqrt(g_ii)|d v^i| / sum |v|), so that a component that vanishes by
+    symmetry is judged against the size of the vector it belongs to (S23)."""
+    gcov = zone_metric(p)
+    gs = gcov[..., 1:, 1:]
+    out = np.zeros(8)
+    for v in (0, 1):
+        out[v] = np.abs(got[v] - ref[v]).sum() / max(np.abs(ref[v]).sum(), 1e-300)
+    for base in (2, 5):
+        vec = np.moveaxis(ref[base:base + 3], 0, -1)
+        norm = np.sqrt(np.einsum("kjia,jiab,kjib->kji", vec, gs, vec)).sum()
+        for i in range(3):
+            gii = np.sqrt(gcov[..., i + 1, i + 1])[None]
+            out[base + i] = (np.abs(got[base + i] - ref[base + i]) * gii).sum() / max(norm, 1e-300)
+    return out
