@@ -120,6 +120,16 @@ int kh_debug_predictor(kh_grid* g, double dt);
 long long kh_launch_count(const kh_grid* g);
 /* Enable/disable CUDA-graph replay of kh_step (default on); the first step after a change captures. */
 int kh_set_graph(kh_grid* g, int enable);
+/* Per-kernel device timing.  While enabled, kh_step enqueues its kernels directly (no graph replay) and
+ * brackets every launch group with a CUDA-event pair on the grid's stream; kh_get_profile synchronises and
+ * returns, per kernel kind (KH_K_*), the summed device milliseconds and the number of bracketed groups since
+ * kh_set_profile(g, 1).  ms and count are HOST arrays of KH_K_COUNT entries.  Used by bench.py for the
+ * per-kernel roofline; the bracketing serialises nothing (one stream) but adds two event records per launch,
+ * so headline throughput is always measured with profiling off. */
+enum { KH_K_FLUX1 = 0, KH_K_FLUX2 = 1, KH_K_FLUX3 = 2, KH_K_EMF = 3, KH_K_UPDATE = 4, KH_K_FILL = 5, KH_K_FIXUP = 6,
+       KH_K_COUNT = 7 };
+int kh_set_profile(kh_grid* g, int enable);
+int kh_get_profile(kh_grid* g, double* ms, long long* count);
 /* Stand-alone DFMA-chain micro-benchmark: returns achieved fp64 TFLOP/s on the current device
  * (HOST double) -- the measured fp64 peak used as an ALU roofline denominator by bench.py. */
 int kh_measure_fp64_peak(double* tflops, double* sm_mhz_est);

@@ -7,4 +7,4 @@ importing works anywhere, but creating a Grid needs libkharm.so and a CUDA devic
 """
 from .binding import (Grid, KharmError, Params, lib, make_params, measure_fp64_peak,  # noqa: F401
                       MINKOWSKI, KS, FMKS, BC_PERIODIC, BC_OUTFLOW, BC_POLAR, BC_FIXED, RECON_MC, RECON_WENO5,
-                      LOC_CENT, LOC_FACE1, LOC_FACE2, LOC_FACE3, NG, EXPORTED_SYMBOLS)
+                      LOC_CENT, LOC_FACE1, LOC_FACE2, LOC_FACE3, NG, EXPORTED_SYMBOLS, KERNEL_KINDS)

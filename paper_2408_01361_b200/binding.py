@@ -12,13 +12,14 @@ MINKOWSKI, KS, FMKS = 0, 1, 2
 BC_PERIODIC, BC_OUTFLOW, BC_POLAR, BC_FIXED = 0, 1, 2, 3
 RECON_MC, RECON_WENO5 = 0, 1
 LOC_CENT, LOC_FACE1, LOC_FACE2, LOC_FACE3 = 0, 1, 2, 3
+KERNEL_KINDS = ("flux1", "flux2", "flux3", "emf", "update", "fill", "fixup")     # KH_K_* of include/kharm.h
 MEM_DEVICE, MEM_HOST = 0, 1
 NG = 3
 
 EXPORTED_SYMBOLS = (
     "kh_grid_create", "kh_grid_destroy", "kh_set_prims", "kh_get_prims", "kh_get_cons", "kh_get_flags",
     "kh_estimate_dt", "kh_step", "kh_divB", "kh_count_flags", "kh_get_geom", "kh_get_conn", "kh_get_flux",
-    "kh_get_emf", "kh_debug_fixup", "kh_debug_predictor", "kh_launch_count", "kh_set_graph", "kh_measure_fp64_peak", "kh_strerror",
+    "kh_get_emf", "kh_debug_fixup", "kh_debug_predictor", "kh_launch_count", "kh_set_graph", "kh_set_profile", "kh_get_profile", "kh_measure_fp64_peak", "kh_strerror",
     "kh_last_cuda_error",
 )
 
@@ -87,6 +88,8 @@ def lib():
         L.kh_debug_fixup.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.kh_debug_predictor.argtypes = [C.c_void_p, C.c_double]
         L.kh_set_graph.argtypes = [C.c_void_p, C.c_int]
+        L.kh_set_profile.argtypes = [C.c_void_p, C.c_int]
+        L.kh_get_profile.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.kh_measure_fp64_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
         _LIB = L
     return _LIB
@@ -248,3 +251,13 @@ class Grid:
 
     def set_graph(self, enable):
         _chk(self.L.kh_set_graph(self.h, int(bool(enable))))
+
+    def set_profile(self, enable):
+        _chk(self.L.kh_set_profile(self.h, int(bool(enable))))
+
+    def get_profile(self):
+        """{kind: (device ms summed, bracketed launch groups)} since set_profile(True)."""
+        n = len(KERNEL_KINDS)
+        ms, cnt = (C.c_double * n)(), (C.c_longlong * n)()
+        _chk(self.L.kh_get_profile(self.h, ms, cnt))
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(KERNEL_KINDS)}

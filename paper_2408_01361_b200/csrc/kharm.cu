@@ -48,16 +48,52 @@ struct kh_grid {
   bool use_graph;
   cudaGraphExec_t gexec[3];
   long long graph_launches;   // kernel launches inside one captured step
+  // per-kernel timing (kh_set_profile): event pairs around every launch, summed per kind on read-out
+  bool profile;
+  cudaEvent_t* pev;           // 2 * KH_PROF_POOL events
+  int* pkind;
+  int npev;
+  double prof_ms[KH_K_COUNT];
+  long long prof_n[KH_K_COUNT];
 };
+
+enum { KH_PROF_POOL = 2048 };
+
+static void prof_flush(kh_grid* g) {
+  if (!g->npev) return;
+  cudaEventSynchronize(g->pev[2 * (g->npev - 1) + 1]);
+  for (int r = 0; r < g->npev; r++) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, g->pev[2 * r], g->pev[2 * r + 1]) == cudaSuccess) {
+      g->prof_ms[g->pkind[r]] += ms;
+      g->prof_n[g->pkind[r]]++;
+    }
+  }
+  g->npev = 0;
+}
+// bracket one launch: PROF_BEGIN(kind); kernel<<<...>>>(...); PROF_END();
+static inline void prof_begin(kh_grid* g, int kind) {
+  if (!g->profile) return;
+  if (g->npev == KH_PROF_POOL) prof_flush(g);
+  g->pkind[g->npev] = kind;
+  cudaEventRecord(g->pev[2 * g->npev], g->stream);
+}
+static inline void prof_end(kh_grid* g) {
+  if (!g->profile) return;
+  cudaEventRecord(g->pev[2 * g->npev + 1], g->stream);
+  g->npev++;
+}
 
 static inline dim3 zone_grid(int nx, int ny, int nz) { return dim3((nx + 127) / 128, ny, nz); }
 
 static int fill_ghosts(kh_grid* g, double* P, unsigned char* flag, int only_if_failed) {
   const GV& v = g->gv;
   long t0 = (long)2 * KH_NGH * v.nt2 * v.nt3, t1 = (long)2 * KH_NGH * v.nt1 * v.nt3, t2 = (long)2 * KH_NGH * v.nt1 * v.nt2;
+  prof_begin(g, KH_K_FILL);
   fill_kernel<0><<<(unsigned)((t0 + 127) / 128), 128, 0, g->stream>>>(v, P, flag, g->sc, only_if_failed);
   fill_kernel<1><<<(unsigned)((t1 + 127) / 128), 128, 0, g->stream>>>(v, P, flag, g->sc, only_if_failed);
   fill_kernel<2><<<(unsigned)((t2 + 127) / 128), 128, 0, g->stream>>>(v, P, flag, g->sc, only_if_failed);
+  prof_end(g);
   g->launches += 3;
   CK(cudaGetLastError());
   return KH_OK;
@@ -70,6 +106,7 @@ static void launch_flux(kh_grid* g, const double* Ps) {
   dim3 grid = zone_grid(c1, c2, c3);
   double* F = g->F[DIR - 1];
   double* ct = g->ctop[DIR - 1];
+  prof_begin(g, KH_K_FLUX1 + DIR - 1);
   if (g->flat) {
     if (g->p.recon == KH_RECON_MC) flux_kernel<DIR, 0, true><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct);
     else flux_kernel<DIR, 1, true><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct);
@@ -77,6 +114,7 @@ static void launch_flux(kh_grid* g, const double* Ps) {
     if (g->p.recon == KH_RECON_MC) flux_kernel<DIR, 0, false><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct);
     else flux_kernel<DIR, 1, false><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct);
   }
+  prof_end(g);
   g->launches++;
 }
 
@@ -84,9 +122,11 @@ static int do_fixup(kh_grid* g, double* Pf, int force) {
   const GV& v = g->gv;
   dim3 grid = zone_grid(v.n1, v.n2, v.n3);
   double* fix = g->fix;
+  prof_begin(g, KH_K_FIXUP);
   fixup_gather_kernel<<<grid, 128, 0, g->stream>>>(v, Pf, g->pflag, fix, g->sc, force);
   if (g->flat) fixup_apply_kernel<true><<<grid, 128, 0, g->stream>>>(v, Pf, g->pflag, g->fflag, fix, g->sc, force);
   else fixup_apply_kernel<false><<<grid, 128, 0, g->stream>>>(v, Pf, g->pflag, g->fflag, fix, g->sc, force);
+  prof_end(g);
   g->launches += 2;
   CK(cudaGetLastError());
   return KH_OK;
@@ -100,14 +140,18 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
   launch_flux<1>(g, Ps);
   launch_flux<2>(g, Ps);
   launch_flux<3>(g, Ps);
+  prof_begin(g, KH_K_EMF);
   emf_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], g->emf[2]);
+  prof_end(g);
   g->launches++;
   dim3 grid = zone_grid(v.n1, v.n2, v.n3);
 #define UPD(FL, CO)                                                                                                  \
   update_kernel<FL, CO><<<grid, 128, 0, g->stream>>>(v, Pi, Ps, Pf, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], \
                                                      g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, g->fflag, g->sc, dt_factor)
+  prof_begin(g, KH_K_UPDATE);
   if (g->flat) { if (corrector) UPD(true, true); else UPD(true, false); }
   else { if (corrector) UPD(false, true); else UPD(false, false); }
+  prof_end(g);
 #undef UPD
   g->launches++;
   CK(cudaGetLastError());
@@ -164,6 +208,8 @@ int kh_grid_destroy(kh_grid* g) {
   for (int b = 0; b < 3; b++) { cudaFree(g->P[b]); cudaFree(g->F[b]); cudaFree(g->ctop[b]); cudaFree(g->emf[b]); }
   cudaFree(g->pflag); cudaFree(g->fflag); cudaFree(g->sc); cudaFree(g->fix); cudaFree(g->stage);
   if (g->sc_host) cudaFreeHost(g->sc_host);
+  if (g->pev) { for (int e = 0; e < 2 * KH_PROF_POOL; e++) if (g->pev[e]) cudaEventDestroy(g->pev[e]); delete[] g->pev; }
+  delete[] g->pkind;
   if (g->own_stream) cudaStreamDestroy(g->stream);
   delete g;
   return KH_OK;
@@ -374,7 +420,7 @@ int kh_step(kh_grid* g, double dt, double* dt_next) {
   g->launches++;
   CK(cudaGetLastError());
   int cur = g->cur;
-  if (g->use_graph) {
+  if (g->use_graph && !g->profile) {
     if (!g->gexec[cur]) {
       long long before = g->launches;
       cudaGraph_t graph;
@@ -526,6 +572,28 @@ int kh_set_graph(kh_grid* g, int enable) {
   if (!g) return KH_EINVAL;
   g->use_graph = enable != 0;
   if (!enable) destroy_graphs(g);
+  return KH_OK;
+}
+
+int kh_set_profile(kh_grid* g, int enable) {
+  if (!g) return KH_EINVAL;
+  if (enable && !g->pev) {
+    g->pev = new (std::nothrow) cudaEvent_t[2 * KH_PROF_POOL];
+    g->pkind = new (std::nothrow) int[KH_PROF_POOL];
+    if (!g->pev || !g->pkind) return KH_ENOMEM;
+    memset(g->pev, 0, sizeof(cudaEvent_t) * 2 * KH_PROF_POOL);
+    for (int e = 0; e < 2 * KH_PROF_POOL; e++) CK(cudaEventCreate(&g->pev[e]));
+  }
+  if (g->profile) prof_flush(g);
+  g->profile = enable != 0;
+  for (int k = 0; k < KH_K_COUNT; k++) { g->prof_ms[k] = 0.0; g->prof_n[k] = 0; }
+  return KH_OK;
+}
+
+int kh_get_profile(kh_grid* g, double* ms, long long* count) {
+  if (!g || !ms || !count) return KH_EINVAL;
+  if (g->profile) prof_flush(g);
+  for (int k = 0; k < KH_K_COUNT; k++) { ms[k] = g->prof_ms[k]; count[k] = g->prof_n[k]; }
   return KH_OK;
 }
 
