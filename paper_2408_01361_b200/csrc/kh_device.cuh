@@ -60,24 +60,59 @@ __device__ __forceinline__ double spatial_norm2(const double* __restrict__ g, do
   return g[G11] * a * a + g[G22] * b * b + g[G33] * c * c + 2.0 * (g[G12] * a * b + g[G13] * a * c + g[G23] * b * c);
 }
 
+// Reciprocal for the hot paths: MUFU.RCP64H seed (rcp.approx.ftz.f64, ~20 bits) + two Newton steps
+// (4 DFMA) -> ~1 ulp.  IEEE division (x/y) costs ~3x the fp64-pipe slots; the step is bound by that
+// pipe.  NOT for arguments that may be 0, inf or subnormal (gives NaN / flushes):
+// callers guarantee a normal, non-zero argument.
+__device__ __forceinline__ double fast_rcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  return r;
+}
+
 // S1: ut^i is the velocity projected into the normal observer's frame:  u^t = gamma/alpha,
 // u^i = ut^i - gamma alpha g^{ti};  b^t = B^i u_i,  b^i = (B^i + b^t u^i)/u^t.
+// Since n_i = 0, u_i = g_ij ut^j exactly and q^2 = ut^i u_i: 12 products instead of 9 + 12.
+// 1/alpha = -g^tt alpha (alpha = (-g^tt)^(-1/2)).
 __device__ __forceinline__ void four_vectors(const Geo& G, const double P[KH_NP], FourVec& D) {
-  double qsq = spatial_norm2(G.gcov, P[U1], P[U2], P[U3]);
+  const double* __restrict__ g = G.gcov;
+  const double v1 = P[U1], v2 = P[U2], v3 = P[U3];
+  D.ucov[1] = g[G11] * v1 + g[G12] * v2 + g[G13] * v3;
+  D.ucov[2] = g[G12] * v1 + g[G22] * v2 + g[G23] * v3;
+  D.ucov[3] = g[G13] * v1 + g[G23] * v2 + g[G33] * v3;
+  double qsq = v1 * D.ucov[1] + v2 * D.ucov[2] + v3 * D.ucov[3];
   double gamma = sqrt(1.0 + qsq);
   double ga = gamma * G.alpha;
-  D.ucon[0] = gamma / G.alpha;
-  D.ucon[1] = P[U1] - ga * G.gcon[G01];
-  D.ucon[2] = P[U2] - ga * G.gcon[G02];
-  D.ucon[3] = P[U3] - ga * G.gcon[G03];
-  lower(G.gcov, D.ucon, D.ucov);
+  D.ucon[0] = -G.gcon[G00] * ga;
+  D.ucon[1] = v1 - ga * G.gcon[G01];
+  D.ucon[2] = v2 - ga * G.gcon[G02];
+  D.ucon[3] = v3 - ga * G.gcon[G03];
+  D.ucov[0] = g[G00] * D.ucon[0] + g[G01] * D.ucon[1] + g[G02] * D.ucon[2] + g[G03] * D.ucon[3];
   D.bcon[0] = P[B1] * D.ucov[1] + P[B2] * D.ucov[2] + P[B3] * D.ucov[3];
-  double iut = 1.0 / D.ucon[0];
+  double iut = fast_rcp(D.ucon[0]);
   D.bcon[1] = (P[B1] + D.bcon[0] * D.ucon[1]) * iut;
   D.bcon[2] = (P[B2] + D.bcon[0] * D.ucon[2]) * iut;
   D.bcon[3] = (P[B3] + D.bcon[0] * D.ucon[3]) * iut;
   lower(G.gcov, D.bcon, D.bcov);
   D.bsq = D.bcon[0] * D.bcov[0] + D.bcon[1] * D.bcov[1] + D.bcon[2] * D.bcov[2] + D.bcon[3] * D.bcov[3];
+}
+
+// b^2 alone (floors): b^2 = (g_ij B^i B^j + (b^t)^2) / (u^t)^2 with b^t = B^i u_i; also returns q^2.
+__device__ __forceinline__ double bsq_only(const Geo& G, const double P[KH_NP], double& qsq) {
+  const double* __restrict__ g = G.gcov;
+  const double v1 = P[U1], v2 = P[U2], v3 = P[U3], b1 = P[B1], b2 = P[B2], b3 = P[B3];
+  double c1 = g[G11] * v1 + g[G12] * v2 + g[G13] * v3;
+  double c2 = g[G12] * v1 + g[G22] * v2 + g[G23] * v3;
+  double c3 = g[G13] * v1 + g[G23] * v2 + g[G33] * v3;
+  qsq = v1 * c1 + v2 * c2 + v3 * c3;
+  double bt = b1 * c1 + b2 * c2 + b3 * c3;
+  double BB = spatial_norm2(g, b1, b2, b3);
+  double iut2 = -fast_rcp((1.0 + qsq) * G.gcon[G00]);      // 1/(u^t)^2 = alpha^2/gamma^2 = -1/(gamma^2 g^tt)
+  return (BB + bt * bt) * iut2;
 }
 
 // T^dir_nu = (w + b^2) u^dir u_nu + (p + b^2/2) delta^dir_nu - b^dir b_nu       [eq. 1.1, P:347]
@@ -117,8 +152,8 @@ __device__ __forceinline__ void vchar(const Geo& G, const double P[KH_NP], const
                                       double& vmax, double& vmin) {
   double ef = P[RHO] + gam * P[UU];
   double ee = D.bsq + ef;
-  double va2 = D.bsq / ee;
-  double cs2 = gam * (gam - 1.0) * P[UU] / ef;
+  double va2 = D.bsq * fast_rcp(ee);
+  double cs2 = gam * (gam - 1.0) * P[UU] * fast_rcp(ef);
   double cms2 = cs2 + va2 - cs2 * va2;
   if (!(cms2 >= 0.0)) cms2 = 0.0;
   if (cms2 > 1.0) cms2 = 1.0;
@@ -126,13 +161,11 @@ __device__ __forceinline__ void vchar(const Geo& G, const double P[KH_NP], const
   double gtt = G.gcon[G00], gtd = G.gcon[sym(0, dir)], gdd = G.gcon[sym(dir, dir)];
   double A = ut * ut - (gtt + ut * ut) * cms2;
   double B = 2.0 * (ud * ut - (gtd + ud * ut) * cms2);
-  double C = ud * ud - (gdd + ud * ud) * cms2;
-  (void)C;
   // B^2 - 4AC reduced algebraically ((u^d u^t)^2 - u^t^2 u^d^2 cancels identically): well conditioned in cold zones
   double disc = 4.0 * cms2 * ((1.0 - cms2) * (ut * ut * gdd - 2.0 * ut * ud * gtd + ud * ud * gtt) + cms2 * (gtd * gtd - gtt * gdd));
   if (!(disc >= 0.0)) disc = 0.0;
   double sq = sqrt(disc);
-  double i2a = 0.5 / A;
+  double i2a = 0.5 * fast_rcp(A);
   double vp = (B + sq) * i2a, vm = (B - sq) * i2a;
   vmax = vp > vm ? vp : vm;
   vmin = vp > vm ? vm : vp;
@@ -171,6 +204,44 @@ __device__ __forceinline__ double weno5_right(double x1, double x2, double x3, d
   return (w1 * v1 + w2 * v2 + w3 * v3) / (w1 + w2 + w3);
 }
 
+// Zone-centred forms: both face values of the zone centred on x3 in one pass.  qm = value at the lower
+// face (the RIGHT state of face i-1/2), qp = value at the upper face (the LEFT state of face i+1/2).
+// The smoothness indicators are shared by the two faces (mirror image: beta1 <-> beta3), and each
+// quotient is one fast reciprocal.
+__device__ __forceinline__ void weno5_zone(double x1, double x2, double x3, double x4, double x5, double& qm, double& qp) {
+  const double eps = 1e-26;
+  double d1 = x1 - 2.0 * x2 + x3, e1 = x1 - 4.0 * x2 + 3.0 * x3;
+  double d2 = x2 - 2.0 * x3 + x4, e2 = x4 - x2;
+  double d3 = x3 - 2.0 * x4 + x5, e3 = 3.0 * x3 - 4.0 * x4 + x5;
+  double b1 = (13.0 / 12.0) * d1 * d1 + 0.25 * e1 * e1 + eps;
+  double b2 = (13.0 / 12.0) * d2 * d2 + 0.25 * e2 * e2 + eps;
+  double b3 = (13.0 / 12.0) * d3 * d3 + 0.25 * e3 * e3 + eps;
+  double a1 = b1 * b1, a2 = b2 * b2, a3 = b3 * b3;
+  double p23 = a2 * a3, p13 = 0.6 * (a1 * a3), p12 = a1 * a2;
+  // upper face: weights (0.1, 0.6, 0.3) on the stencils (x1..x3), (x2..x4), (x3..x5)
+  double w1 = 0.1 * p23, w3 = 0.3 * p12;
+  double v1 = (1.0 / 3.0) * x1 - (7.0 / 6.0) * x2 + (11.0 / 6.0) * x3;
+  double v2 = -(1.0 / 6.0) * x2 + (5.0 / 6.0) * x3 + (1.0 / 3.0) * x4;
+  double v3 = (1.0 / 3.0) * x3 + (5.0 / 6.0) * x4 - (1.0 / 6.0) * x5;
+  qp = (w1 * v1 + p13 * v2 + w3 * v3) * fast_rcp(w1 + p13 + w3);
+  // lower face: the mirror image, weights (0.1, 0.6, 0.3) on (x5..x3), (x4..x2), (x3..x1)
+  double m1 = 0.1 * p12, m3 = 0.3 * p23;
+  double u1 = (1.0 / 3.0) * x5 - (7.0 / 6.0) * x4 + (11.0 / 6.0) * x3;
+  double u2 = -(1.0 / 6.0) * x4 + (5.0 / 6.0) * x3 + (1.0 / 3.0) * x2;
+  double u3 = (1.0 / 3.0) * x3 + (5.0 / 6.0) * x2 - (1.0 / 6.0) * x1;
+  qm = (m1 * u1 + p13 * u2 + m3 * u3) * fast_rcp(m1 + p13 + m3);
+}
+__device__ __forceinline__ void mc_zone(double x2, double x3, double x4, double& qm, double& qp) {
+  double h = 0.5 * mc_slope(x2, x3, x4);
+  qm = x3 - h;
+  qp = x3 + h;
+}
+template <int RECON>
+__device__ __forceinline__ void recon_zone(const double* __restrict__ A, long st, double& qm, double& qp) {
+  if (RECON == 0) mc_zone(A[-st], A[0], A[st], qm, qp);
+  else weno5_zone(A[-2 * st], A[-st], A[0], A[st], A[2 * st], qm, qp);
+}
+
 // ---------------------------------------------------------------------------------------------
 // 1D_W inversion (ref [37]) in the W' = W - D variable (S16).
 // ---------------------------------------------------------------------------------------------
@@ -180,19 +251,22 @@ struct U2P {
     double WB = Bsq + W;
     return (Qtsq * W * W + QdotBsq * (Bsq + 2.0 * W)) / (WB * WB * W * W);
   }
+  // f(W') and f'(W') (S16).  Reciprocals by fast_rcp: W, W + B^2, 1 - v^2 (clamped) and 1 + gamma are
+  // positive normal numbers here.
   __device__ __forceinline__ void func(double Wp, double& f, double& df) const {
-    double W = Wp + D;
-    double v2 = vsq(W);
+    double W = Wp + D, WB = W + Bsq;
+    double iW = fast_rcp(W), iWB = fast_rcp(WB);
+    double iW2 = iW * iW, iW3 = iW2 * iW, iWB2 = iWB * iWB, iWB3 = iWB2 * iWB;
+    double v2 = (Qtsq * W * W + QdotBsq * (Bsq + 2.0 * W)) * (iWB2 * iW2);
     v2 = fmax(v2, 0.0);
     v2 = fmin(v2, 1.0 - 1e-12);
-    double gsq = 1.0 / (1.0 - v2), g = sqrt(gsq);
+    double omv = 1.0 - v2;
+    double gsq = fast_rcp(omv), g = sqrt(gsq);
     double k = (gam - 1.0) / gam;
-    double p = k * (Wp - D * v2 * gsq / (1.0 + g)) / gsq;
-    double iW = 1.0 / W, iW2 = iW * iW, iW3 = iW2 * iW;
+    double p = k * (Wp - D * v2 * gsq * fast_rcp(1.0 + g)) * omv;
     f = Wp - p + 0.5 * Bsq * (1.0 + v2) - 0.5 * QdotBsq * iW2 - Ep;
-    double WB = W + Bsq, iWB = 1.0 / WB, iWB3 = iWB * iWB * iWB;
     double dv2 = -2.0 * (Qtsq * W * W * W + QdotBsq * (3.0 * W * W + 3.0 * W * Bsq + Bsq * Bsq)) * iW3 * iWB3;
-    double dp = k * ((1.0 - v2) - (W - 0.5 * D * g) * dv2);
+    double dp = k * (omv - (W - 0.5 * D * g) * dv2);
     df = 1.0 - dp + 0.5 * Bsq * dv2 + QdotBsq * iW3;
   }
 };
@@ -240,7 +314,7 @@ __device__ __forceinline__ int u_to_p(const Geo& G, const double U[KH_NP], const
     double f, df;
     c.func(Wp, f, df);
     double Wold = Wp + c.D;
-    double Wpn = Wp - f / df;
+    double Wpn = Wp - f * fast_rcp(df);
     if (!(Wpn + c.D > 0.0)) Wpn = 0.5 * Wold - c.D;
     double dW = Wpn - Wp;
     Wp = Wpn;
@@ -271,20 +345,19 @@ __device__ __forceinline__ int u_to_p(const Geo& G, const double U[KH_NP], const
 // Floors and ceilings in the fluid frame (S18).  rho_g, u_g: tabulated geometric floors.
 // ---------------------------------------------------------------------------------------------
 struct FloorPar {
-  double bsq_over_rho_max, bsq_over_u_max, u_over_rho_max, gamma_max;
+  double inv_bsq_over_rho_max, inv_bsq_over_u_max, u_over_rho_max, gamma_max;   // inverses formed once on the host
 };
 
 __device__ __forceinline__ int apply_floors(const Geo& G, const FloorPar& fp, double rho_g, double u_g, double P[KH_NP]) {
   int flag = 0;
-  FourVec D;
-  four_vectors(G, P, D);
-  double rho_b = D.bsq / fp.bsq_over_rho_max, u_b = D.bsq / fp.bsq_over_u_max;
+  double qsq;
+  const double bsq = bsq_only(G, P, qsq);
+  double rho_b = bsq * fp.inv_bsq_over_rho_max, u_b = bsq * fp.inv_bsq_over_u_max;
   double rho_fl = rho_b > rho_g ? rho_b : rho_g;
   double u_fl = u_b > u_g ? u_b : u_g;
   if (P[RHO] < rho_fl) { P[RHO] = rho_fl; flag |= (rho_b > rho_g) ? 2 : 1; }
   if (P[UU] < u_fl) { P[UU] = u_fl; flag |= (u_b > u_g) ? 8 : 4; }
   if (P[UU] > fp.u_over_rho_max * P[RHO]) { P[UU] = fp.u_over_rho_max * P[RHO]; flag |= 16; }
-  double qsq = spatial_norm2(G.gcov, P[U1], P[U2], P[U3]);
   double gamma = sqrt(1.0 + qsq);
   if (gamma > fp.gamma_max) {
     double f = sqrt((fp.gamma_max * fp.gamma_max - 1.0) / (gamma * gamma - 1.0));

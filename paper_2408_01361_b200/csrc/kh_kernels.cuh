@@ -44,45 +44,24 @@ __device__ __forceinline__ bool polar_face(const GV& g, int j) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// K2: one thread per face.  Faces i_d in [0, N_d], transverse indices in [-1, N_t] (one ghost row
-// each side, needed by Flux-CT).  Writes 5 hydro + 2 induction components and ctop.
+// K2: reconstruction + LLF flux.  Faces i_d in [0, N_d], transverse indices in [-1, N_t] (one ghost
+// row each side, needed by Flux-CT).  Writes 5 hydro + 2 induction components and ctop.
+//
+// The step is bound by the fp64 pipe, not by HBM, so the layout of the work
+// minimises fp64 instructions: reconstruction is done ONCE PER ZONE (both face values share the
+// WENO smoothness indicators / the MC slope) and the two states of a face meet in registers:
+//   x1: one zone per lane, the zone's upper-face value goes to the next lane by warp shuffle
+//       (warps overlap by one zone: 31 faces per warp);
+//   x2, x3: each thread marches along the direction over a chunk of faces and carries the previous
+//       zone's upper-face value in registers; lanes run along x1, so every access is coalesced.
+// Every primitive is fetched from HBM once per direction (the stencil re-reads hit L1/L2:
+// profiles/ shows dram bytes = algorithmic bytes).
 // ---------------------------------------------------------------------------------------------
-template <int DIR, int RECON, bool FLAT>
-__global__ void __launch_bounds__(128)
-flux_kernel(GV g, const double* __restrict__ P, double* __restrict__ F, double* __restrict__ ctop) {
-  const int lo1 = (DIR == 1) ? 0 : -1, lo2 = (DIR == 2) ? 0 : -1, lo3 = (DIR == 3) ? 0 : -1;
-  int i = blockIdx.x * blockDim.x + threadIdx.x + lo1;
-  int j = blockIdx.y + lo2, k = blockIdx.z + lo3;
-  if (i > g.n1) return;
-  const long n = zidx(g, i, j, k);
-  const long st = (DIR == 1) ? 1 : (DIR == 2 ? g.s2 : g.s3);
-  const long nt = g.ntot;
-
-  if (DIR == 2 && polar_face(g, j)) {   // S7 / S10: nothing crosses the axis
-#pragma unroll
-    for (int v = 0; v < KH_NP; v++) F[v * nt + n] = 0.0;
-    ctop[n] = 0.0;
-    return;
-  }
-
-  double PL[KH_NP], PR[KH_NP];
-#pragma unroll
-  for (int v = 0; v < KH_NP; v++) {
-    const double* A = P + v * nt + n;
-    if (RECON == 0) {
-      double qm2 = A[-2 * st], qm1 = A[-st], q0 = A[0], qp1 = A[st];
-      PL[v] = qm1 + 0.5 * mc_slope(qm2, qm1, q0);
-      PR[v] = q0 - 0.5 * mc_slope(qm1, q0, qp1);
-    } else {
-      double qm3 = A[-3 * st], qm2 = A[-2 * st], qm1 = A[-st], q0 = A[0], qp1 = A[st], qp2 = A[2 * st];
-      PL[v] = weno5_right(qm3, qm2, qm1, q0, qp1);
-      PR[v] = weno5_right(qp2, qp1, q0, qm1, qm2);
-    }
-  }
-
+template <int DIR, bool FLAT>
+__device__ __forceinline__ void face_flux(const GV& g, const double PL[KH_NP], const double PR[KH_NP], long p2, long n,
+                                          double* __restrict__ F, double* __restrict__ ctop) {
   Geo G;
-  load_geo<FLAT>(G, g.geom[DIR], g.n2d, pidx(g, i, j));
-
+  load_geo<FLAT>(G, g.geom[DIR], g.n2d, p2);
   double UL[KH_NP], FL[KH_NP], vmaxL, vminL;
   {
     FourVec D;
@@ -102,12 +81,75 @@ flux_kernel(GV g, const double* __restrict__ P, double* __restrict__ F, double* 
   double cmax = fmax(0.0, fmax(vmaxL, vmaxR));
   double cmin = fmax(0.0, fmax(-vminL, -vminR));
   double c = fmax(cmax, cmin);
+  const long nt = g.ntot;
 #pragma unroll
   for (int v = 0; v < KH_NP; v++) {
     if (v == B1 + DIR - 1) continue;     // F^d[B^d] = 0, never read
     F[v * nt + n] = 0.5 * (FL[v] + FR[v] - c * (UR[v] - UL[v]));
   }
   ctop[n] = c;
+}
+
+template <int RECON, bool FLAT>
+__global__ void __launch_bounds__(128)
+flux_x1_kernel(GV g, const double* __restrict__ P, double* __restrict__ F, double* __restrict__ ctop) {
+  const int c1 = g.n1 + 2, c2 = g.n2 + 2;                // zones -1 .. N per row; rows (j, k) in [-1, N]
+  const long Z = (long)c1 * c2 * (g.n3 + 2);
+  const int lane = threadIdx.x & 31;
+  const long warp = ((long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const long z = warp * 31 + lane;                       // consecutive warps overlap by one zone
+  const bool valid = z < Z;
+  const long zc = valid ? z : Z - 1;
+  const int i = (int)(zc % c1) - 1;
+  const long row = zc / c1;
+  const int j = (int)(row % c2) - 1, k = (int)(row / c2) - 1;
+  const long n = zidx(g, i, j, k), nt = g.ntot;
+  double PL[KH_NP], PR[KH_NP];
+#pragma unroll
+  for (int v = 0; v < KH_NP; v++) {
+    double qp;
+    recon_zone<RECON>(P + v * nt + n, 1, PR[v], qp);
+    PL[v] = __shfl_up_sync(0xffffffffu, qp, 1);          // upper-face value of zone i-1 = left state of face i
+  }
+  if (!valid || lane == 0 || i < 0) return;              // lane 0's face belongs to the previous warp
+  face_flux<1, FLAT>(g, PL, PR, pidx(g, i, j), n, F, ctop);
+}
+
+// x2 / x3: thread <-> (i, transverse index), marching over faces [f0, f1) of chunk blockIdx.y.
+template <int DIR, int RECON, bool FLAT>
+__global__ void __launch_bounds__(128)
+flux_march_kernel(GV g, const double* __restrict__ P, double* __restrict__ F, double* __restrict__ ctop, int J) {
+  const int c1 = g.n1 + 2;
+  const int cb = (DIR == 2 ? g.n3 : g.n2) + 2;
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (long)c1 * cb) return;
+  const int i = (int)(t % c1) - 1, b = (int)(t / c1) - 1;
+  const int N = (DIR == 2) ? g.n2 : g.n3;
+  const int f0 = blockIdx.y * J;
+  const int f1 = (f0 + J < N + 1) ? f0 + J : N + 1;
+  const long st = (DIR == 2) ? g.s2 : g.s3, nt = g.ntot;
+  long n = (DIR == 2) ? zidx(g, i, f0 - 1, b) : zidx(g, i, b, f0 - 1);
+  double PL[KH_NP];
+#pragma unroll
+  for (int v = 0; v < KH_NP; v++) {
+    double qm;
+    recon_zone<RECON>(P + v * nt + n, st, qm, PL[v]);
+  }
+  for (int f = f0; f < f1; f++) {
+    n += st;
+    double PR[KH_NP], PLn[KH_NP];
+#pragma unroll
+    for (int v = 0; v < KH_NP; v++) recon_zone<RECON>(P + v * nt + n, st, PR[v], PLn[v]);
+    if (DIR == 2 && polar_face(g, f)) {   // S7 / S10: nothing crosses the axis
+#pragma unroll
+      for (int v = 0; v < KH_NP; v++) F[v * nt + n] = 0.0;
+      ctop[n] = 0.0;
+    } else {
+      face_flux<DIR, FLAT>(g, PL, PR, (DIR == 2) ? pidx(g, i, f) : pidx(g, i, b), n, F, ctop);
+    }
+#pragma unroll
+    for (int v = 0; v < KH_NP; v++) PL[v] = PLn[v];
+  }
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -53,6 +53,7 @@ struct kh_grid {
   cudaEvent_t* pev;           // 2 * KH_PROF_POOL events
   int* pkind;
   int npev;
+  int sm_count, flux_blocks_per_sm;
   double prof_ms[KH_K_COUNT];
   long long prof_n[KH_K_COUNT];
 };
@@ -99,20 +100,52 @@ static int fill_ghosts(kh_grid* g, double* P, unsigned char* flag, int only_if_f
   return KH_OK;
 }
 
+// Chunk length of the marching kernels: long enough that the one extra reconstruction per chunk is
+// small, short enough that the grid fills the SMs in an almost whole number of waves.
+static int march_chunk(const kh_grid* g, long columns, int faces) {
+  const double resident = (double)g->sm_count * g->flux_blocks_per_sm * 128.0;
+  int best = 16;
+  double best_eff = 0.0;
+  for (int J = 6; J <= 32; J++) {
+    int chunks = (faces + J - 1) / J;
+    double waves = (double)columns * chunks / resident;
+    double eff = waves / ceil(waves) * ((double)faces / (double)(faces + chunks));
+    if (eff > best_eff + 1e-9) { best_eff = eff; best = J; }
+  }
+  return best;
+}
+
 template <int DIR>
 static void launch_flux(kh_grid* g, const double* Ps) {
   const GV& v = g->gv;
-  int c1 = v.n1 + (DIR == 1 ? 1 : 2), c2 = v.n2 + (DIR == 2 ? 1 : 2), c3 = v.n3 + (DIR == 3 ? 1 : 2);
-  dim3 grid = zone_grid(c1, c2, c3);
   double* F = g->F[DIR - 1];
   double* ct = g->ctop[DIR - 1];
+  const bool mc = g->p.recon == KH_RECON_MC;
   prof_begin(g, KH_K_FLUX1 + DIR - 1);
-  if (g->flat) {
-    if (g->p.recon == KH_RECON_MC) flux_kernel<DIR, 0, true><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct);
-    else flux_kernel<DIR, 1, true><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct);
+  if (DIR == 1) {
+    const long zones = (long)(v.n1 + 2) * (v.n2 + 2) * (v.n3 + 2);
+    const long warps = (zones + 30) / 31;
+    const unsigned blocks = (unsigned)((warps + 3) / 4);
+    if (g->flat) {
+      if (mc) flux_x1_kernel<0, true><<<blocks, 128, 0, g->stream>>>(v, Ps, F, ct);
+      else flux_x1_kernel<1, true><<<blocks, 128, 0, g->stream>>>(v, Ps, F, ct);
+    } else {
+      if (mc) flux_x1_kernel<0, false><<<blocks, 128, 0, g->stream>>>(v, Ps, F, ct);
+      else flux_x1_kernel<1, false><<<blocks, 128, 0, g->stream>>>(v, Ps, F, ct);
+    }
   } else {
-    if (g->p.recon == KH_RECON_MC) flux_kernel<DIR, 0, false><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct);
-    else flux_kernel<DIR, 1, false><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct);
+    const int N = (DIR == 2) ? v.n2 : v.n3;
+    const long cols = (long)(v.n1 + 2) * ((DIR == 2 ? v.n3 : v.n2) + 2);
+    const int J = march_chunk(g, cols, N + 1);
+    dim3 grid((unsigned)((cols + 127) / 128), (unsigned)((N + 1 + J - 1) / J));
+    constexpr int D = (DIR == 1) ? 2 : DIR;   // (keeps the DIR == 1 instantiation of this branch well-formed)
+    if (g->flat) {
+      if (mc) flux_march_kernel<D, 0, true><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct, J);
+      else flux_march_kernel<D, 1, true><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct, J);
+    } else {
+      if (mc) flux_march_kernel<D, 0, false><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct, J);
+      else flux_march_kernel<D, 1, false><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct, J);
+    }
   }
   prof_end(g);
   g->launches++;
@@ -246,6 +279,16 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
     g->own_stream = true;
   }
   g->flat = (p->coords == KH_MINKOWSKI);
+  {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    int nb = 0;
+    cudaError_t eo = g->flat ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, flux_march_kernel<2, 1, true>, 128, 0)
+                             : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, flux_march_kernel<2, 1, false>, 128, 0);
+    g->flux_blocks_per_sm = (eo == cudaSuccess && nb > 0) ? nb : 4;
+    if (g->sm_count < 1) g->sm_count = 148;
+  }
   g->use_graph = true;
   GV& v = g->gv;
   v.n1 = p->n1; v.n2 = p->n2; v.n3 = p->n3;
@@ -257,7 +300,7 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   for (int b = 0; b < 6; b++) v.bc[b] = p->bc[b];
   v.polar_lo = p->bc[2] == KH_BC_POLAR; v.polar_hi = p->bc[3] == KH_BC_POLAR;
   v.ndim_mask = (v.n1 > 1 ? 1 : 0) | (v.n2 > 1 ? 2 : 0) | (v.n3 > 1 ? 4 : 0);
-  v.fp.bsq_over_rho_max = p->bsq_over_rho_max; v.fp.bsq_over_u_max = p->bsq_over_u_max;
+  v.fp.inv_bsq_over_rho_max = 1.0 / p->bsq_over_rho_max; v.fp.inv_bsq_over_u_max = 1.0 / p->bsq_over_u_max;
   v.fp.u_over_rho_max = p->u_over_rho_max; v.fp.gamma_max = p->gamma_max;
 
 #define ALLOC(ptr, bytes)                                                       \
