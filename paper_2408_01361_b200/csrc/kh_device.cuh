@@ -1,9 +1,15 @@
 // kh_device.cuh -- device-side building blocks of libkharm (sm_100a): packed symmetric metric,
-// four-vectors, stress tensor rows, conserved variables / fluxes, fast-magnetosonic speeds,
-// MC / WENO5 reconstruction, the 1D_W inversion and the floors.
+// four-vectors, conserved variables / fluxes, fast-magnetosonic speeds, MC / WENO5 reconstruction,
+// the 1D_W inversion and the floors.
 //
 // Written from the published scheme (DESIGN.md readings
 // S1..S23).  Shares nothing with oracle/ (the CPU oracle is test infrastructure only).
+//
+// The step is bound by the fp64 pipe (one DFMA/DMUL/DADD holds a sub-partition's
+// pipe for 2 cycles per warp), so everything here is written for a minimal fp64 INSTRUCTION count:
+// algebraically reduced forms, shared sub-expressions between the L and R state of a face and between a
+// zone's two faces, reciprocals / square roots from the MUFU seeds with one third-order correction, and
+// the structural zeros of the Kerr-Schild family (g_02 = g_23 = g^03 = 0, also in FMKS) skipped.
 #pragma once
 #include <cuda_runtime.h>
 #include <math.h>
@@ -23,157 +29,206 @@ enum { G00 = 0, G01 = 1, G02 = 2, G03 = 3, G11 = 4, G12 = 5, G13 = 6, G22 = 7, G
 
 // geometry table components per location: 10 gcov, 10 gcon, gdet, alpha
 #define KH_NGEO 22
-#define KH_NCONN 40   // Gamma^lam_{mu nu}: lam * 10 + sym(mu, nu)
+#define KH_NCONN 40   // Gamma^lam_{mu nu}: lam * 10 + sym(mu, nu)       (kh_get_conn only)
+#define KH_NDG 20     // source table: sqrt(-g) w_c d_nu g_c, nu = 1,2, c = packed pair (w = 1/2 diagonal, 1 off-diagonal)
 
-struct Geo {
-  double gcov[10], gcon[10], gdet, alpha;
-};
-
-template <bool FLAT>
-__device__ __forceinline__ void load_geo(Geo& G, const double* __restrict__ tab, long n2d, long p) {
-  if (FLAT) {
-#pragma unroll
-    for (int c = 0; c < 10; c++) { G.gcov[c] = 0.0; G.gcon[c] = 0.0; }
-    G.gcov[G00] = -1.0; G.gcov[G11] = 1.0; G.gcov[G22] = 1.0; G.gcov[G33] = 1.0;
-    G.gcon[G00] = -1.0; G.gcon[G11] = 1.0; G.gcon[G22] = 1.0; G.gcon[G33] = 1.0;
-    G.gdet = 1.0; G.alpha = 1.0;
-  } else {
-#pragma unroll
-    for (int c = 0; c < 10; c++) { G.gcov[c] = __ldg(tab + c * n2d + p); G.gcon[c] = __ldg(tab + (10 + c) * n2d + p); }
-    G.gdet = __ldg(tab + 20 * n2d + p);
-    G.alpha = __ldg(tab + 21 * n2d + p);
-  }
-}
-
-struct FourVec {
-  double ucon[4], ucov[4], bcon[4], bcov[4], bsq;
-};
-
-__device__ __forceinline__ void lower(const double* __restrict__ g, const double v[4], double out[4]) {
-  out[0] = g[G00] * v[0] + g[G01] * v[1] + g[G02] * v[2] + g[G03] * v[3];
-  out[1] = g[G01] * v[0] + g[G11] * v[1] + g[G12] * v[2] + g[G13] * v[3];
-  out[2] = g[G02] * v[0] + g[G12] * v[1] + g[G22] * v[2] + g[G23] * v[3];
-  out[3] = g[G03] * v[0] + g[G13] * v[1] + g[G23] * v[2] + g[G33] * v[3];
-}
-
-__device__ __forceinline__ double spatial_norm2(const double* __restrict__ g, double a, double b, double c) {
-  return g[G11] * a * a + g[G22] * b * b + g[G33] * c * c + 2.0 * (g[G12] * a * b + g[G13] * a * c + g[G23] * b * c);
-}
-
-// Reciprocal for the hot paths: MUFU.RCP64H seed (rcp.approx.ftz.f64, ~20 bits) + two Newton steps
-// (4 DFMA) -> ~1 ulp.  IEEE division (x/y) costs ~3x the fp64-pipe slots; the step is bound by that
-// pipe.  NOT for arguments that may be 0, inf or subnormal (gives NaN / flushes):
-// callers guarantee a normal, non-zero argument.
+// ---------------------------------------------------------------------------------------------
+// Fast reciprocal / reciprocal square root / square root: MUFU seed (rcp/rsqrt.approx.ftz.f64,
+// relative error < 2^-20) + ONE third-order correction -> error ~ seed^3 < 2^-60, i.e. the result is
+// within 1 ulp of the IEEE one.  IEEE x/y and sqrt() cost ~3x the fp64-pipe slots.
+// NOT for arguments that may be 0, inf, NaN-producing or subnormal: callers guarantee normal, positive
+// (rcp: non-zero) arguments.
+// ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ double fast_rcp(double x) {
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  double e = fma(-x, r, 1.0);
-  r = fma(r, e, r);
-  e = fma(-x, r, 1.0);
-  r = fma(r, e, r);
-  return r;
+  double e = fma(-x, r, 1.0);          // 1/x = r / (1 - e) = r (1 + e + e^2 + O(e^3))
+  double t = fma(e, e, e);
+  return fma(r, t, r);
 }
-
-// S1: ut^i is the velocity projected into the normal observer's frame:  u^t = gamma/alpha,
-// u^i = ut^i - gamma alpha g^{ti};  b^t = B^i u_i,  b^i = (B^i + b^t u^i)/u^t.
-// Since n_i = 0, u_i = g_ij ut^j exactly and q^2 = ut^i u_i: 12 products instead of 9 + 12.
-// 1/alpha = -g^tt alpha (alpha = (-g^tt)^(-1/2)).
-__device__ __forceinline__ void four_vectors(const Geo& G, const double P[KH_NP], FourVec& D) {
-  const double* __restrict__ g = G.gcov;
-  const double v1 = P[U1], v2 = P[U2], v3 = P[U3];
-  D.ucov[1] = g[G11] * v1 + g[G12] * v2 + g[G13] * v3;
-  D.ucov[2] = g[G12] * v1 + g[G22] * v2 + g[G23] * v3;
-  D.ucov[3] = g[G13] * v1 + g[G23] * v2 + g[G33] * v3;
-  double qsq = v1 * D.ucov[1] + v2 * D.ucov[2] + v3 * D.ucov[3];
-  double gamma = sqrt(1.0 + qsq);
-  double ga = gamma * G.alpha;
-  D.ucon[0] = -G.gcon[G00] * ga;
-  D.ucon[1] = v1 - ga * G.gcon[G01];
-  D.ucon[2] = v2 - ga * G.gcon[G02];
-  D.ucon[3] = v3 - ga * G.gcon[G03];
-  D.ucov[0] = g[G00] * D.ucon[0] + g[G01] * D.ucon[1] + g[G02] * D.ucon[2] + g[G03] * D.ucon[3];
-  D.bcon[0] = P[B1] * D.ucov[1] + P[B2] * D.ucov[2] + P[B3] * D.ucov[3];
-  double iut = fast_rcp(D.ucon[0]);
-  D.bcon[1] = (P[B1] + D.bcon[0] * D.ucon[1]) * iut;
-  D.bcon[2] = (P[B2] + D.bcon[0] * D.ucon[2]) * iut;
-  D.bcon[3] = (P[B3] + D.bcon[0] * D.ucon[3]) * iut;
-  lower(G.gcov, D.bcon, D.bcov);
-  D.bsq = D.bcon[0] * D.bcov[0] + D.bcon[1] * D.bcov[1] + D.bcon[2] * D.bcov[2] + D.bcon[3] * D.bcov[3];
+__device__ __forceinline__ double fast_rsqrt(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double xy = x * y;
+  double e = fma(-xy, y, 1.0);         // x^(-1/2) = y (1 - e)^(-1/2) = y (1 + e/2 + 3 e^2/8 + O(e^3))
+  double p = fma(0.375, e, 0.5);
+  return fma(y, p * e, y);
 }
-
-// b^2 alone (floors): b^2 = (g_ij B^i B^j + (b^t)^2) / (u^t)^2 with b^t = B^i u_i; also returns q^2.
-__device__ __forceinline__ double bsq_only(const Geo& G, const double P[KH_NP], double& qsq) {
-  const double* __restrict__ g = G.gcov;
-  const double v1 = P[U1], v2 = P[U2], v3 = P[U3], b1 = P[B1], b2 = P[B2], b3 = P[B3];
-  double c1 = g[G11] * v1 + g[G12] * v2 + g[G13] * v3;
-  double c2 = g[G12] * v1 + g[G22] * v2 + g[G23] * v3;
-  double c3 = g[G13] * v1 + g[G23] * v2 + g[G33] * v3;
-  qsq = v1 * c1 + v2 * c2 + v3 * c3;
-  double bt = b1 * c1 + b2 * c2 + b3 * c3;
-  double BB = spatial_norm2(g, b1, b2, b3);
-  double iut2 = -fast_rcp((1.0 + qsq) * G.gcon[G00]);      // 1/(u^t)^2 = alpha^2/gamma^2 = -1/(gamma^2 g^tt)
-  return (BB + bt * bt) * iut2;
-}
-
-// T^dir_nu = (w + b^2) u^dir u_nu + (p + b^2/2) delta^dir_nu - b^dir b_nu       [eq. 1.1, P:347]
-__device__ __forceinline__ void stress_row(const double P[KH_NP], const FourVec& D, double gam, int dir, double T[4]) {
-  double pg = (gam - 1.0) * P[UU];
-  double eta = P[RHO] + P[UU] + pg + D.bsq;
-  double ptot = pg + 0.5 * D.bsq;
-  double eu = eta * D.ucon[dir], bd = D.bcon[dir];
-#pragma unroll
-  for (int nu = 0; nu < 4; nu++) T[nu] = eu * D.ucov[nu] - bd * D.bcov[nu];
-  T[dir] += ptot;
-}
-
-// dir = 0 -> U (S8: energy slot T^t_t + rho u^t);  dir = 1..3 -> F^dir.  Only the five hydro slots
-// and, for dir > 0, the two non-trivial induction slots are meaningful; F^dir[B^dir] = 0.
-__device__ __forceinline__ void prim_to_flux(const Geo& G, const double P[KH_NP], const FourVec& D, double gam, int dir,
-                                             double F[KH_NP]) {
-  double T[4];
-  stress_row(P, D, gam, dir, T);
-  double rhou = P[RHO] * D.ucon[dir];
-  F[RHO] = G.gdet * rhou;
-  F[UU] = G.gdet * (T[0] + rhou);
-  F[U1] = G.gdet * T[1];
-  F[U2] = G.gdet * T[2];
-  F[U3] = G.gdet * T[3];
-  if (dir == 0) {
-    F[B1] = G.gdet * P[B1]; F[B2] = G.gdet * P[B2]; F[B3] = G.gdet * P[B3];
-  } else {
-#pragma unroll
-    for (int i = 1; i < 4; i++)
-      F[B1 + i - 1] = (i == dir) ? 0.0 : G.gdet * (D.bcon[i] * D.ucon[dir] - D.bcon[dir] * D.ucon[i]);
-  }
-}
-
-// S9: fast-magnetosonic bound.  Roots of A v^2 - B v + C = 0.
-__device__ __forceinline__ void vchar(const Geo& G, const double P[KH_NP], const FourVec& D, double gam, int dir,
-                                      double& vmax, double& vmin) {
-  double ef = P[RHO] + gam * P[UU];
-  double ee = D.bsq + ef;
-  double va2 = D.bsq * fast_rcp(ee);
-  double cs2 = gam * (gam - 1.0) * P[UU] * fast_rcp(ef);
-  double cms2 = cs2 + va2 - cs2 * va2;
-  if (!(cms2 >= 0.0)) cms2 = 0.0;
-  if (cms2 > 1.0) cms2 = 1.0;
-  double ut = D.ucon[0], ud = D.ucon[dir];
-  double gtt = G.gcon[G00], gtd = G.gcon[sym(0, dir)], gdd = G.gcon[sym(dir, dir)];
-  double A = ut * ut - (gtt + ut * ut) * cms2;
-  double B = 2.0 * (ud * ut - (gtd + ud * ut) * cms2);
-  // B^2 - 4AC reduced algebraically ((u^d u^t)^2 - u^t^2 u^d^2 cancels identically): well conditioned in cold zones
-  double disc = 4.0 * cms2 * ((1.0 - cms2) * (ut * ut * gdd - 2.0 * ut * ud * gtd + ud * ud * gtt) + cms2 * (gtd * gtd - gtt * gdd));
-  if (!(disc >= 0.0)) disc = 0.0;
-  double sq = sqrt(disc);
-  double i2a = 0.5 * fast_rcp(A);
-  double vp = (B + sq) * i2a, vm = (B - sq) * i2a;
-  vmax = vp > vm ? vp : vm;
-  vmin = vp > vm ? vm : vp;
+__device__ __forceinline__ double fast_sqrt(double x) {   // x > 0 normal
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double g = x * y;
+  double e = fma(-g, y, 1.0);
+  double p = fma(0.375, e, 0.5);
+  return fma(g, p * e, g);
 }
 
 // ---------------------------------------------------------------------------------------------
-// Reconstruction.  Both return the face value on the side of x3 towards x4 given the
-// stencil (x1..x5) centred on x3 ("right" value); the left value is the mirror image.
+// Metric at one table point.  FLAT (Minkowski-Cartesian): compile-time constants, no loads (the paper's
+// own compile-time switch).  Otherwise the Kerr-Schild family (KS, FMKS): g_02 = g_23 = 0 and
+// g^03 = 0 identically (the geometry kernel stores exact zeros), so those entries are neither loaded nor
+// multiplied -- bit-identical to the general contraction for finite operands.
+// ---------------------------------------------------------------------------------------------
+struct Geo {
+  double c00, c01, c03, c11, c12, c13, c22, c33;           // g_{mu nu} (non-zero entries)
+  double n00, n01, n02, n11, n12, n13, n22, n23, n33;      // g^{mu nu} (non-zero entries)
+  double gdet, alpha;
+};
+
+// LEVEL 0: what a face flux of direction DIR needs (g^dd and g^td besides the covariant metric);
+// LEVEL 1: everything (zone centres: source term, inversion).
+template <bool FLAT, int DIR, int LEVEL>
+__device__ __forceinline__ void load_geo(Geo& G, const double* __restrict__ tab, long n2d, long p) {
+  if (FLAT) {
+    G.c00 = -1.0; G.c11 = G.c22 = G.c33 = 1.0; G.c01 = G.c03 = G.c12 = G.c13 = 0.0;
+    G.n00 = -1.0; G.n11 = G.n22 = G.n33 = 1.0; G.n01 = G.n02 = G.n12 = G.n13 = G.n23 = 0.0;
+    G.gdet = 1.0; G.alpha = 1.0;
+    return;
+  }
+#define KH_LD(c) __ldg(tab + (long)(c) * n2d + p)
+  G.c00 = KH_LD(G00); G.c01 = KH_LD(G01); G.c03 = KH_LD(G03); G.c11 = KH_LD(G11); G.c12 = KH_LD(G12);
+  G.c13 = KH_LD(G13); G.c22 = KH_LD(G22); G.c33 = KH_LD(G33);
+  G.n00 = KH_LD(10 + G00); G.n01 = KH_LD(10 + G01); G.n02 = KH_LD(10 + G02);
+  if (LEVEL == 1 || DIR == 1) G.n11 = KH_LD(10 + G11);
+  if (LEVEL == 1 || DIR == 2) G.n22 = KH_LD(10 + G22);
+  if (LEVEL == 1 || DIR == 3) G.n33 = KH_LD(10 + G33);
+  if (LEVEL == 1) { G.n12 = KH_LD(10 + G12); G.n13 = KH_LD(10 + G13); G.n23 = KH_LD(10 + G23); }
+  G.gdet = KH_LD(20); G.alpha = KH_LD(21);
+#undef KH_LD
+}
+
+// g_ij a^i b^j pieces
+template <bool FLAT>
+__device__ __forceinline__ void lower3(const Geo& G, double a1, double a2, double a3, double& o1, double& o2, double& o3) {
+  if (FLAT) { o1 = a1; o2 = a2; o3 = a3; return; }
+  o1 = fma(G.c13, a3, fma(G.c12, a2, G.c11 * a1));
+  o2 = fma(G.c22, a2, G.c12 * a1);
+  o3 = fma(G.c33, a3, G.c13 * a1);
+}
+template <bool FLAT>
+__device__ __forceinline__ double spatial_norm2(const Geo& G, double a, double b, double c) {
+  double o1, o2, o3;
+  lower3<FLAT>(G, a, b, c, o1, o2, o3);
+  return fma(c, o3, fma(b, o2, a * o1));
+}
+
+// ---------------------------------------------------------------------------------------------
+// Four-vectors of a primitive state (S1): ut^i is the velocity projected into the normal observer's frame,
+//   u^t = gamma/alpha, u^i = ut^i - gamma alpha g^{ti};  b^t = B^i u_i,  b^i = (B^i + b^t u^i)/u^t.
+// Since n_i = 0, u_i = g_ij ut^j exactly and q^2 = ut^i u_i.  gamma and 1/gamma come from one rsqrt.
+// ---------------------------------------------------------------------------------------------
+struct FourVec {
+  double ucon[4], ucov[4], bcon[4], bcov[4], bsq;
+  double x;       // 1 + q^2 = gamma^2
+};
+
+template <bool FLAT>
+__device__ __forceinline__ void four_vectors(const Geo& G, double ialpha, const double P[KH_NP], FourVec& D) {
+  const double v1 = P[U1], v2 = P[U2], v3 = P[U3];
+  lower3<FLAT>(G, v1, v2, v3, D.ucov[1], D.ucov[2], D.ucov[3]);
+  double qsq = fma(v3, D.ucov[3], fma(v2, D.ucov[2], v1 * D.ucov[1]));
+  D.x = 1.0 + qsq;
+  double rg = fast_rsqrt(D.x), gamma = D.x * rg;
+  if (FLAT) {
+    D.ucon[0] = gamma; D.ucon[1] = v1; D.ucon[2] = v2; D.ucon[3] = v3;
+    D.ucov[0] = -gamma;
+  } else {
+    double ga = gamma * G.alpha;
+    D.ucon[0] = gamma * ialpha;
+    D.ucon[1] = fma(-ga, G.n01, v1);
+    D.ucon[2] = fma(-ga, G.n02, v2);
+    D.ucon[3] = v3;                                  // g^03 = 0
+    D.ucov[0] = fma(G.c03, D.ucon[3], fma(G.c01, D.ucon[1], G.c00 * D.ucon[0]));   // g_02 = 0
+  }
+  D.bcon[0] = fma(P[B3], D.ucov[3], fma(P[B2], D.ucov[2], P[B1] * D.ucov[1]));
+  double iut = FLAT ? rg : G.alpha * rg;             // 1/u^t = alpha/gamma
+  D.bcon[1] = fma(D.bcon[0], D.ucon[1], P[B1]) * iut;
+  D.bcon[2] = fma(D.bcon[0], D.ucon[2], P[B2]) * iut;
+  D.bcon[3] = fma(D.bcon[0], D.ucon[3], P[B3]) * iut;
+  if (FLAT) {
+    D.bcov[0] = -D.bcon[0]; D.bcov[1] = D.bcon[1]; D.bcov[2] = D.bcon[2]; D.bcov[3] = D.bcon[3];
+  } else {
+    D.bcov[0] = fma(G.c03, D.bcon[3], fma(G.c01, D.bcon[1], G.c00 * D.bcon[0]));
+    D.bcov[1] = fma(G.c13, D.bcon[3], fma(G.c12, D.bcon[2], fma(G.c11, D.bcon[1], G.c01 * D.bcon[0])));
+    D.bcov[2] = fma(G.c22, D.bcon[2], G.c12 * D.bcon[1]);
+    D.bcov[3] = fma(G.c33, D.bcon[3], fma(G.c13, D.bcon[1], G.c03 * D.bcon[0]));
+  }
+  D.bsq = fma(D.bcon[3], D.bcov[3], fma(D.bcon[2], D.bcov[2], fma(D.bcon[1], D.bcov[1], D.bcon[0] * D.bcov[0])));
+}
+
+// Row `dir` of the flux matrix WITHOUT the sqrt(-g) factor (applied once per face / zone by the caller):
+//   dir = 0: U/sqrt(-g) = (rho u^t, T^t_t + rho u^t, T^t_i, B^i)          (S8)
+//   dir > 0: F^dir/sqrt(-g) = (rho u^d, T^d_t + rho u^d, T^d_i, b^i u^d - b^d u^i), F^d[B^d] = 0
+// with T^mu_nu = (w + b^2) u^mu u_nu + (p + b^2/2) delta^mu_nu - b^mu b_nu  [eq. 1.1, P:347]; eu[nu] = (w+b^2) u_nu.
+__device__ __forceinline__ void flux_row(const double P[KH_NP], const FourVec& D, const double eu[4], double ptot, int dir,
+                                         double F[KH_NP]) {
+  const double ud = D.ucon[dir], bd = D.bcon[dir];
+  double T0 = fma(ud, eu[0], -bd * D.bcov[0]);
+  double T1 = fma(ud, eu[1], -bd * D.bcov[1]);
+  double T2 = fma(ud, eu[2], -bd * D.bcov[2]);
+  double T3 = fma(ud, eu[3], -bd * D.bcov[3]);
+  if (dir == 0) T0 += ptot;
+  if (dir == 1) T1 += ptot;
+  if (dir == 2) T2 += ptot;
+  if (dir == 3) T3 += ptot;
+  F[RHO] = P[RHO] * ud;
+  F[UU] = fma(P[RHO], ud, T0);
+  F[U1] = T1; F[U2] = T2; F[U3] = T3;
+  if (dir == 0) {
+    F[B1] = P[B1]; F[B2] = P[B2]; F[B3] = P[B3];
+  } else {
+#pragma unroll
+    for (int i = 1; i < 4; i++) F[B1 + i - 1] = (i == dir) ? 0.0 : fma(D.bcon[i], ud, -bd * D.ucon[i]);
+  }
+}
+
+// S9: fast-magnetosonic bound.  c_m^2 = c_s^2 + v_A^2 - c_s^2 v_A^2 = (b^2 + Gamma (Gamma-1) u) / (rho + Gamma u + b^2)
+// (one quotient).  The characteristic speeds are the roots of A v^2 - 2 Bh v + C = 0; LLF and the CFL rule
+// only need max(|v+|, |v-|) = (|Bh| + sqrt(Bh^2 - A C)) / A (A > 0), and Bh^2 - A C reduces algebraically to
+//   c_m^2 [ (1 - c_m^2)(u^t^2 g^dd - 2 u^t u^d g^td + u^d^2 g^tt) + c_m^2 (g^td^2 - g^tt g^dd) ]
+// (the (u^d u^t)^2 terms cancel identically: well conditioned in cold zones).  k2 = g^td^2 - g^tt g^dd.
+template <bool FLAT>
+__device__ __forceinline__ double cfast(const FourVec& D, double ee, double gg1u, double gtt, double gtd, double gdd, double k2,
+                                        int dir) {
+  double cms2 = (D.bsq + gg1u) * fast_rcp(ee);
+  if (!(cms2 >= 0.0)) cms2 = 0.0;
+  if (cms2 > 1.0) cms2 = 1.0;
+  const double ut = D.ucon[0], ud = D.ucon[dir];
+  double ut2 = ut * ut, udut = ud * ut, ud2 = ud * ud;
+  double A, Bh, inner;
+  if (FLAT) {
+    A = fma(-(ut2 - 1.0), cms2, ut2);
+    Bh = fma(-udut, cms2, udut);
+    inner = fma(1.0 - cms2, ut2 - ud2, cms2);
+  } else {
+    A = fma(-(gtt + ut2), cms2, ut2);
+    Bh = fma(-(gtd + udut), cms2, udut);
+    double q = fma(ud2, gtt, fma(-2.0 * udut, gtd, ut2 * gdd));
+    inner = fma(1.0 - cms2, q, cms2 * k2);
+  }
+  double disc = fmax(cms2 * inner, 1e-200);       // also maps NaN to the floor; sqrt(1e-200) = 1e-100 is invisible
+  return (fabs(Bh) + fast_sqrt(disc)) * fast_rcp(A);
+}
+
+// Both flux-matrix rows a face needs from one state (without sqrt(-g)) and its signal-speed bound.
+template <int DIR, bool FLAT>
+__device__ __forceinline__ void state_terms(const Geo& G, double ialpha, double gtd, double gdd, double k2, const double P[KH_NP],
+                                            double gam, double gm1, double U[KH_NP], double F[KH_NP], double& c) {
+  FourVec D;
+  four_vectors<FLAT>(G, ialpha, P, D);
+  double pg = gm1 * P[UU];
+  double ee = fma(gam, P[UU], P[RHO]) + D.bsq;      // w + b^2 = rho + Gamma u + b^2
+  double ptot = fma(0.5, D.bsq, pg);
+  double eu[4] = {ee * D.ucov[0], ee * D.ucov[1], ee * D.ucov[2], ee * D.ucov[3]};
+  flux_row(P, D, eu, ptot, 0, U);
+  flux_row(P, D, eu, ptot, DIR, F);
+  c = cfast<FLAT>(D, ee, gam * pg, G.n00, gtd, gdd, k2, DIR);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Reconstruction, zone-centred: both face values of the zone centred on x3 in one pass.
+// qm = value at the lower face (the RIGHT state of face i-1/2), qp = value at the upper face (the LEFT
+// state of face i+1/2).
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ double mc_slope(double qm, double q0, double qp) {   // S11
   double dm = 2.0 * (q0 - qm), dp = 2.0 * (qp - q0), dc = 0.5 * (qp - qm);
@@ -185,160 +240,47 @@ __device__ __forceinline__ double mc_slope(double qm, double q0, double qp) {   
   }
   return s;
 }
-
-// S12: Jiang-Shu WENO5 with eps = 1e-26.  The three non-linear weights d_k/(eps+beta_k)^2 are
-// formed over the common denominator so that one division serves the whole face value.
-__device__ __forceinline__ double weno5_right(double x1, double x2, double x3, double x4, double x5) {
-  const double eps = 1e-26;
-  double d1 = x1 - 2.0 * x2 + x3, e1 = x1 - 4.0 * x2 + 3.0 * x3;
-  double d2 = x2 - 2.0 * x3 + x4, e2 = x4 - x2;
-  double d3 = x3 - 2.0 * x4 + x5, e3 = 3.0 * x3 - 4.0 * x4 + x5;
-  double b1 = (13.0 / 12.0) * d1 * d1 + 0.25 * e1 * e1 + eps;
-  double b2 = (13.0 / 12.0) * d2 * d2 + 0.25 * e2 * e2 + eps;
-  double b3 = (13.0 / 12.0) * d3 * d3 + 0.25 * e3 * e3 + eps;
-  double a1 = b1 * b1, a2 = b2 * b2, a3 = b3 * b3;
-  double w1 = 0.1 * (a2 * a3), w2 = 0.6 * (a1 * a3), w3 = 0.3 * (a1 * a2);
-  double v1 = (1.0 / 3.0) * x1 - (7.0 / 6.0) * x2 + (11.0 / 6.0) * x3;
-  double v2 = -(1.0 / 6.0) * x2 + (5.0 / 6.0) * x3 + (1.0 / 3.0) * x4;
-  double v3 = (1.0 / 3.0) * x3 + (5.0 / 6.0) * x4 - (1.0 / 6.0) * x5;
-  return (w1 * v1 + w2 * v2 + w3 * v3) / (w1 + w2 + w3);
-}
-
-// Zone-centred forms: both face values of the zone centred on x3 in one pass.  qm = value at the lower
-// face (the RIGHT state of face i-1/2), qp = value at the upper face (the LEFT state of face i+1/2).
-// The smoothness indicators are shared by the two faces (mirror image: beta1 <-> beta3), and each
-// quotient is one fast reciprocal.
-__device__ __forceinline__ void weno5_zone(double x1, double x2, double x3, double x4, double x5, double& qm, double& qp) {
-  const double eps = 1e-26;
-  double d1 = x1 - 2.0 * x2 + x3, e1 = x1 - 4.0 * x2 + 3.0 * x3;
-  double d2 = x2 - 2.0 * x3 + x4, e2 = x4 - x2;
-  double d3 = x3 - 2.0 * x4 + x5, e3 = 3.0 * x3 - 4.0 * x4 + x5;
-  double b1 = (13.0 / 12.0) * d1 * d1 + 0.25 * e1 * e1 + eps;
-  double b2 = (13.0 / 12.0) * d2 * d2 + 0.25 * e2 * e2 + eps;
-  double b3 = (13.0 / 12.0) * d3 * d3 + 0.25 * e3 * e3 + eps;
-  double a1 = b1 * b1, a2 = b2 * b2, a3 = b3 * b3;
-  double p23 = a2 * a3, p13 = 0.6 * (a1 * a3), p12 = a1 * a2;
-  // upper face: weights (0.1, 0.6, 0.3) on the stencils (x1..x3), (x2..x4), (x3..x5)
-  double w1 = 0.1 * p23, w3 = 0.3 * p12;
-  double v1 = (1.0 / 3.0) * x1 - (7.0 / 6.0) * x2 + (11.0 / 6.0) * x3;
-  double v2 = -(1.0 / 6.0) * x2 + (5.0 / 6.0) * x3 + (1.0 / 3.0) * x4;
-  double v3 = (1.0 / 3.0) * x3 + (5.0 / 6.0) * x4 - (1.0 / 6.0) * x5;
-  qp = (w1 * v1 + p13 * v2 + w3 * v3) * fast_rcp(w1 + p13 + w3);
-  // lower face: the mirror image, weights (0.1, 0.6, 0.3) on (x5..x3), (x4..x2), (x3..x1)
-  double m1 = 0.1 * p12, m3 = 0.3 * p23;
-  double u1 = (1.0 / 3.0) * x5 - (7.0 / 6.0) * x4 + (11.0 / 6.0) * x3;
-  double u2 = -(1.0 / 6.0) * x4 + (5.0 / 6.0) * x3 + (1.0 / 3.0) * x2;
-  double u3 = (1.0 / 3.0) * x3 + (5.0 / 6.0) * x2 - (1.0 / 6.0) * x1;
-  qm = (m1 * u1 + p13 * u2 + m3 * u3) * fast_rcp(m1 + p13 + m3);
-}
 __device__ __forceinline__ void mc_zone(double x2, double x3, double x4, double& qm, double& qp) {
   double h = 0.5 * mc_slope(x2, x3, x4);
   qm = x3 - h;
   qp = x3 + h;
 }
+
+// S12: Jiang-Shu WENO5, eps = 1e-26, written on the differences D_k = x_{k+1} - x_k:
+//   12 (beta_k + eps) = 13 d_k^2 + 3 e_k^2 + 12 eps      (the common factor 12 cancels in the weights)
+//   weights d_k / (beta_k + eps)^2 over the common denominator: (1, 6, 3) x products of the other two squares
+//   candidate values as offsets from x3, times 6:  upper face (5 D2 - 2 D1, D2 + 2 D3, 4 D3 - D4),
+//   lower face the mirror image (2 D4 - 5 D3, -(D3 + 2 D2), D1 - 4 D2); the smoothness indicators are shared.
+// 59 fp64 instructions per variable for both faces.
+__device__ __forceinline__ void weno5_zone(double x1, double x2, double x3, double x4, double x5, double& qm, double& qp) {
+  const double c = 12.0e-26;
+  double D1 = x2 - x1, D2 = x3 - x2, D3 = x4 - x3, D4 = x5 - x4;
+  double d1 = D2 - D1, d2 = D3 - D2, d3 = D4 - D3;
+  double e1 = fma(3.0, D2, -D1), e2 = D2 + D3, e3 = fma(-3.0, D3, D4);
+  double b1 = fma(13.0 * d1, d1, fma(3.0 * e1, e1, c));
+  double b2 = fma(13.0 * d2, d2, fma(3.0 * e2, e2, c));
+  double b3 = fma(13.0 * d3, d3, fma(3.0 * e3, e3, c));
+  double a1 = b1 * b1, a2 = b2 * b2, a3 = b3 * b3;
+  double p23 = a2 * a3, p13 = 6.0 * (a1 * a3), p12 = a1 * a2;
+  {
+    double w3 = 3.0 * p12;
+    double V1 = fma(5.0, D2, -2.0 * D1), V2 = fma(2.0, D3, D2), V3 = fma(4.0, D3, -D4);
+    double N = fma(w3, V3, fma(p13, V2, p23 * V1));
+    double S = p23 + p13 + w3;
+    qp = fma(N * fast_rcp(S), 1.0 / 6.0, x3);
+  }
+  {
+    double m3 = 3.0 * p23;
+    double M1 = fma(-5.0, D3, 2.0 * D4), M2 = fma(2.0, D2, D3), M3 = fma(-4.0, D2, D1);
+    double N = fma(m3, M3, fma(-p13, M2, p12 * M1));
+    double S = p12 + p13 + m3;
+    qm = fma(N * fast_rcp(S), 1.0 / 6.0, x3);
+  }
+}
 template <int RECON>
 __device__ __forceinline__ void recon_zone(const double* __restrict__ A, long st, double& qm, double& qp) {
   if (RECON == 0) mc_zone(A[-st], A[0], A[st], qm, qp);
   else weno5_zone(A[-2 * st], A[-st], A[0], A[st], A[2 * st], qm, qp);
-}
-
-// ---------------------------------------------------------------------------------------------
-// 1D_W inversion (ref [37]) in the W' = W - D variable (S16).
-// ---------------------------------------------------------------------------------------------
-struct U2P {
-  double D, Bsq, QdotB, QdotBsq, Qtsq, Ep, gam;
-  __device__ __forceinline__ double vsq(double W) const {
-    double WB = Bsq + W;
-    return (Qtsq * W * W + QdotBsq * (Bsq + 2.0 * W)) / (WB * WB * W * W);
-  }
-  // f(W') and f'(W') (S16).  Reciprocals by fast_rcp: W, W + B^2, 1 - v^2 (clamped) and 1 + gamma are
-  // positive normal numbers here.
-  __device__ __forceinline__ void func(double Wp, double& f, double& df) const {
-    double W = Wp + D, WB = W + Bsq;
-    double iW = fast_rcp(W), iWB = fast_rcp(WB);
-    double iW2 = iW * iW, iW3 = iW2 * iW, iWB2 = iWB * iWB, iWB3 = iWB2 * iWB;
-    double v2 = (Qtsq * W * W + QdotBsq * (Bsq + 2.0 * W)) * (iWB2 * iW2);
-    v2 = fmax(v2, 0.0);
-    v2 = fmin(v2, 1.0 - 1e-12);
-    double omv = 1.0 - v2;
-    double gsq = fast_rcp(omv), g = sqrt(gsq);
-    double k = (gam - 1.0) / gam;
-    double p = k * (Wp - D * v2 * gsq * fast_rcp(1.0 + g)) * omv;
-    f = Wp - p + 0.5 * Bsq * (1.0 + v2) - 0.5 * QdotBsq * iW2 - Ep;
-    double dv2 = -2.0 * (Qtsq * W * W * W + QdotBsq * (3.0 * W * W + 3.0 * W * Bsq + Bsq * Bsq)) * iW3 * iWB3;
-    double dp = k * (omv - (W - 0.5 * D * g) * dv2);
-    df = 1.0 - dp + 0.5 * Bsq * dv2 + QdotBsq * iW3;
-  }
-};
-
-// Returns the flag; on failure the hydro primitives of Pout keep the guess, B is always updated.
-__device__ __forceinline__ int u_to_p(const Geo& G, const double U[KH_NP], const double Pg[KH_NP], double gam,
-                                      double Pout[KH_NP]) {
-#pragma unroll
-  for (int v = 0; v < 5; v++) Pout[v] = Pg[v];
-  double igdet = 1.0 / G.gdet;
-  Pout[B1] = U[B1] * igdet; Pout[B2] = U[B2] * igdet; Pout[B3] = U[B3] * igdet;
-  bool fin = true;
-#pragma unroll
-  for (int v = 0; v < KH_NP; v++) fin = fin && isfinite(U[v]);
-  if (!fin || !(U[RHO] > 0.0)) return 1;
-
-  double alpha = G.alpha, k = alpha * igdet;
-  U2P c;
-  c.gam = gam;
-  c.D = k * U[RHO];
-  double Bc[4] = {0.0, k * U[B1], k * U[B2], k * U[B3]};
-  double Qcov[4] = {k * (U[UU] - U[RHO]), k * U[U1], k * U[U2], k * U[U3]};
-  double Qcon[4];
-  lower(G.gcon, Qcov, Qcon);   // raising with the packed inverse metric
-  c.Bsq = spatial_norm2(G.gcov, Bc[1], Bc[2], Bc[3]);
-  c.QdotB = Qcov[1] * Bc[1] + Qcov[2] * Bc[2] + Qcov[3] * Bc[3];
-  c.QdotBsq = c.QdotB * c.QdotB;
-  double Qdotn = -alpha * Qcon[0];
-  c.Ep = -Qdotn - c.D;
-  double Qt1 = Qcon[1] + Qdotn * (-alpha * G.gcon[G01]);
-  double Qt2 = Qcon[2] + Qdotn * (-alpha * G.gcon[G02]);
-  double Qt3 = Qcon[3] + Qdotn * (-alpha * G.gcon[G03]);
-  // Qt^2 = Q.Q + (Q.n)^2 as the spatial norm of the projected vector (its time component vanishes):
-  // no cancellation, never negative (S16).
-  c.Qtsq = spatial_norm2(G.gcov, Qt1, Qt2, Qt3);
-
-  double qsq = spatial_norm2(G.gcov, Pg[U1], Pg[U2], Pg[U3]);
-  double W = (Pg[RHO] + gam * Pg[UU]) * (1.0 + qsq);
-  if (!(W > 0.0) || !isfinite(W)) W = c.D;
-  for (int it = 0; it < 30 && !(c.vsq(W) < 1.0); it++) W *= 10.0;
-  double Wp = W - c.D;
-
-  bool conv = false;
-  for (int it = 0; it < 20; it++) {
-    double f, df;
-    c.func(Wp, f, df);
-    double Wold = Wp + c.D;
-    double Wpn = Wp - f * fast_rcp(df);
-    if (!(Wpn + c.D > 0.0)) Wpn = 0.5 * Wold - c.D;
-    double dW = Wpn - Wp;
-    Wp = Wpn;
-    if (fabs(dW) <= 1e-12 * (Wp + c.D)) { conv = true; break; }
-  }
-  if (!conv) return 2;
-
-  W = Wp + c.D;
-  double v2 = c.vsq(W);
-  if (!(v2 >= 0.0) || !(v2 < 1.0) || !(W > 0.0)) return 3;
-  double gsq = 1.0 / (1.0 - v2), g = sqrt(gsq);
-  double rho = c.D / g;
-  double u = (Wp - c.D * v2 * gsq / (1.0 + g)) / (gsq * gam);
-  double fac = g / (W + c.Bsq), qbw = c.QdotB / W;
-  double ut1 = fac * (Qt1 + qbw * Bc[1]);
-  double ut2 = fac * (Qt2 + qbw * Bc[2]);
-  double ut3 = fac * (Qt3 + qbw * Bc[3]);
-  if (!isfinite(rho) || !isfinite(u) || !isfinite(ut1) || !isfinite(ut2) || !isfinite(ut3)) return 7;
-  bool badrho = !(rho > 0.0), badu = (u < 0.0);
-  if (badrho && badu) return 6;
-  if (badrho) return 4;
-  if (badu) return 5;
-  Pout[RHO] = rho; Pout[UU] = u; Pout[U1] = ut1; Pout[U2] = ut2; Pout[U3] = ut3;
-  return 0;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -348,23 +290,149 @@ struct FloorPar {
   double inv_bsq_over_rho_max, inv_bsq_over_u_max, u_over_rho_max, gamma_max;   // inverses formed once on the host
 };
 
-__device__ __forceinline__ int apply_floors(const Geo& G, const FloorPar& fp, double rho_g, double u_g, double P[KH_NP]) {
+// Limits on (rho, u) and the Lorentz-factor ceiling given b^2 and gamma of the state; returns the fflag bits and
+// the factor (1 = none) by which the caller scales ut^i.
+__device__ __forceinline__ int floor_limits(const FloorPar& fp, double rho_g, double u_g, double bsq, double gamma, double& rho,
+                                            double& u, double& vfac) {
   int flag = 0;
-  double qsq;
-  const double bsq = bsq_only(G, P, qsq);
   double rho_b = bsq * fp.inv_bsq_over_rho_max, u_b = bsq * fp.inv_bsq_over_u_max;
   double rho_fl = rho_b > rho_g ? rho_b : rho_g;
   double u_fl = u_b > u_g ? u_b : u_g;
-  if (P[RHO] < rho_fl) { P[RHO] = rho_fl; flag |= (rho_b > rho_g) ? 2 : 1; }
-  if (P[UU] < u_fl) { P[UU] = u_fl; flag |= (u_b > u_g) ? 8 : 4; }
-  if (P[UU] > fp.u_over_rho_max * P[RHO]) { P[UU] = fp.u_over_rho_max * P[RHO]; flag |= 16; }
-  double gamma = sqrt(1.0 + qsq);
-  if (gamma > fp.gamma_max) {
-    double f = sqrt((fp.gamma_max * fp.gamma_max - 1.0) / (gamma * gamma - 1.0));
-    P[U1] *= f; P[U2] *= f; P[U3] *= f;
+  if (rho < rho_fl) { rho = rho_fl; flag |= (rho_b > rho_g) ? 2 : 1; }
+  if (u < u_fl) { u = u_fl; flag |= (u_b > u_g) ? 8 : 4; }
+  double ucap = fp.u_over_rho_max * rho;
+  if (u > ucap) { u = ucap; flag |= 16; }
+  vfac = 1.0;
+  if (gamma > fp.gamma_max) {      // rare: IEEE sqrt and division
+    vfac = sqrt((fp.gamma_max * fp.gamma_max - 1.0) / (gamma * gamma - 1.0));
     flag |= 32;
   }
   return flag;
+}
+
+// Floors of a primitive state (fix-up path): b^2 = (g_ij B^i B^j + (b^t)^2)/(u^t)^2 with b^t = B^i u_i.
+template <bool FLAT>
+__device__ __forceinline__ int apply_floors(const Geo& G, const FloorPar& fp, double rho_g, double u_g, double P[KH_NP]) {
+  double c1, c2, c3;
+  lower3<FLAT>(G, P[U1], P[U2], P[U3], c1, c2, c3);
+  double qsq = fma(P[U3], c3, fma(P[U2], c2, P[U1] * c1));
+  double bt = fma(P[B3], c3, fma(P[B2], c2, P[B1] * c1));
+  double BB = spatial_norm2<FLAT>(G, P[B1], P[B2], P[B3]);
+  double bsq = fma(bt, bt, BB) / (-(1.0 + qsq) * G.n00);      // 1/(u^t)^2 = alpha^2/gamma^2 = -1/(gamma^2 g^tt)
+  double vfac;
+  int flag = floor_limits(fp, rho_g, u_g, bsq, sqrt(1.0 + qsq), P[RHO], P[UU], vfac);
+  if (flag & 32) { P[U1] *= vfac; P[U2] *= vfac; P[U3] *= vfac; }
+  return flag;
+}
+
+// ---------------------------------------------------------------------------------------------
+// 1D_W inversion (ref [37]) in the W' = W - D variable (S16), fused with the floors (S18).
+// Input Uh = U / sqrt(-g).  W0 = guess (rho + Gamma u)(1 + q^2) of the guess primitives.
+// Returns the pflag; on success writes the five hydro primitives to Pout (floors applied, bits in fflag); B is
+// always written; on failure the caller keeps the guess primitives (S16).
+// Per Newton step: one reciprocal serves 1/W and 1/(W+B^2), one rsqrt gives gamma and gamma^2.
+// After convergence b^2 = B^2 (1 - v^2) + (Q.B)^2 / W^2 and gamma are known from the conserved side, so the
+// floors need no second pass through the four-vectors.
+// ---------------------------------------------------------------------------------------------
+template <bool FLAT>
+__device__ __forceinline__ int u_to_p_floors(const Geo& G, const double Uh[KH_NP], double W0, double gam, const FloorPar& fp,
+                                             double rho_g, double u_g, double Pout[KH_NP], int& fflag) {
+  fflag = 0;
+  Pout[B1] = Uh[B1]; Pout[B2] = Uh[B2]; Pout[B3] = Uh[B3];
+  bool fin = true;
+#pragma unroll
+  for (int v = 0; v < KH_NP; v++) fin = fin && isfinite(Uh[v]);
+  if (!fin || !(Uh[RHO] > 0.0)) return 1;
+
+  const double alpha = G.alpha;
+  const double D = alpha * Uh[RHO];
+  const double Bc1 = alpha * Uh[B1], Bc2 = alpha * Uh[B2], Bc3 = alpha * Uh[B3];        // script-B^i = alpha B^i
+  const double Qc0 = alpha * (Uh[UU] - Uh[RHO]), Qc1 = alpha * Uh[U1], Qc2 = alpha * Uh[U2], Qc3 = alpha * Uh[U3];
+  double Qdotn, Qt1, Qt2, Qt3;
+  if (FLAT) {
+    Qdotn = Qc0; Qt1 = Qc1; Qt2 = Qc2; Qt3 = Qc3;
+  } else {
+    double Q0 = fma(G.n02, Qc2, fma(G.n01, Qc1, G.n00 * Qc0));                           // g^03 = 0
+    double Q1 = fma(G.n13, Qc3, fma(G.n12, Qc2, fma(G.n11, Qc1, G.n01 * Qc0)));
+    double Q2 = fma(G.n23, Qc3, fma(G.n22, Qc2, fma(G.n12, Qc1, G.n02 * Qc0)));
+    double Q3 = fma(G.n33, Qc3, fma(G.n23, Qc2, G.n13 * Qc1));
+    Qdotn = -alpha * Q0;
+    double qa = -alpha * Qdotn;                       // Qt^i = Q^i + (Q.n) n^i, n^i = -alpha g^{ti}
+    Qt1 = fma(qa, G.n01, Q1); Qt2 = fma(qa, G.n02, Q2); Qt3 = Q3;
+  }
+  const double Bsq = spatial_norm2<FLAT>(G, Bc1, Bc2, Bc3);
+  const double QdotB = fma(Qc3, Bc3, fma(Qc2, Bc2, Qc1 * Bc1));
+  const double QdotBsq = QdotB * QdotB;
+  const double Ep = -Qdotn - D;
+  // Qt^2 as the spatial norm of the projected vector (its time component vanishes): no cancellation (S16)
+  const double Qtsq = spatial_norm2<FLAT>(G, Qt1, Qt2, Qt3);
+
+  double W = W0;
+  if (!(W > 0.0) || !isfinite(W)) W = D;
+#pragma unroll 1
+  for (int it = 0; it < 30; it++) {                   // v^2(W0) < 1  <=>  numerator < denominator
+    double WB = Bsq + W, den = (WB * WB) * (W * W);
+    double num = fma(Qtsq * W, W, QdotBsq * fma(2.0, W, Bsq));
+    if (num < den) break;
+    W *= 10.0;
+  }
+  double Wp = W - D;
+  const double k = (gam - 1.0) / gam, hB = 0.5 * Bsq, hQ = 0.5 * QdotBsq, hD = 0.5 * D, Bsq2 = Bsq * Bsq;
+  const double WpmE0 = -Ep;
+
+  bool conv = false;
+#pragma unroll 1
+  for (int it = 0; it < 20; it++) {
+    W = Wp + D;
+    double WB = W + Bsq;
+    double r = fast_rcp(W * WB), iW = r * WB, iWB = r * W;      // iW iWB = r
+    double iW2 = iW * iW, s2 = iW2 * (iWB * iWB);
+    double QW = Qtsq * W;
+    double v2 = fma(QW, W, QdotBsq * fma(2.0, W, Bsq)) * s2;
+    v2 = fmin(fmax(v2, 0.0), 1.0 - 1e-12);
+    double omv = 1.0 - v2;
+    double g = fast_rsqrt(omv), gsq = g * g;
+    double t = (D * v2) * (gsq * fast_rcp(1.0 + g));
+    double p = k * ((Wp - t) * omv);
+    double f = fma(-hQ, iW2, fma(hB, v2, hB)) + ((Wp + WpmE0) - p);
+    double dv2 = -2.0 * (fma(QW, W * W, QdotBsq * fma(3.0 * W, WB, Bsq2)) * (s2 * r));
+    double dp = k * fma(-fma(-hD, g, W), dv2, omv);
+    double df = fma(hB, dv2, fma(QdotBsq, iW2 * iW, 1.0 - dp));
+    double Wold = W;
+    double Wpn = fma(-f, fast_rcp(df), Wp);
+    if (!(Wpn + D > 0.0)) Wpn = 0.5 * Wold - D;       // new W <= 0: halve the old W instead
+    double dW = Wpn - Wp;
+    Wp = Wpn;
+    if (fabs(dW) <= 1e-12 * (Wp + D)) { conv = true; break; }
+  }
+  if (!conv) return 2;
+
+  W = Wp + D;
+  if (!(W > 0.0)) return 3;
+  double WB = W + Bsq;
+  double r = fast_rcp(W * WB), iW = r * WB, iWB = r * W;
+  double v2 = fma(Qtsq * W, W, QdotBsq * fma(2.0, W, Bsq)) * (r * r);
+  if (!(v2 >= 0.0) || !(v2 < 1.0)) return 3;
+  double omv = 1.0 - v2;
+  double g = fast_rsqrt(omv), gsq = g * g;
+  double rho = D * (omv * g);                          // D / gamma
+  double u = ((Wp - (D * v2) * (gsq * fast_rcp(1.0 + g))) * omv) * (1.0 / gam);
+  double fac = g * iWB, qbw = QdotB * iW;
+  double ut1 = fac * fma(qbw, Bc1, Qt1);
+  double ut2 = fac * fma(qbw, Bc2, Qt2);
+  double ut3 = fac * fma(qbw, Bc3, Qt3);
+  if (!isfinite(rho) || !isfinite(u) || !isfinite(ut1) || !isfinite(ut2) || !isfinite(ut3)) return 7;
+  bool badrho = !(rho > 0.0), badu = (u < 0.0);
+  if (badrho && badu) return 6;
+  if (badrho) return 4;
+  if (badu) return 5;
+  // floors (S18): b^2 and gamma of the recovered state from the conserved side
+  double bsq = fma(Bsq, omv, QdotBsq * (iW * iW));
+  double vfac;
+  fflag = floor_limits(fp, rho_g, u_g, bsq, g, rho, u, vfac);
+  if (fflag & 32) { ut1 *= vfac; ut2 *= vfac; ut3 *= vfac; }
+  Pout[RHO] = rho; Pout[UU] = u; Pout[U1] = ut1; Pout[U2] = ut2; Pout[U3] = ut3;
+  return 0;
 }
 
 }  // namespace kh

@@ -115,9 +115,10 @@ __device__ inline double invert_sym4(const double g[10], double inv[10]) {
   return det;
 }
 
-// tab[loc]: KH_NGEO components x n2d; conn: KH_NCONN x n2d; floorp: 2 x n2d (rho, u geometric floors)
+// tab[loc]: KH_NGEO components x n2d; conn: KH_NCONN x n2d; dgt: KH_NDG x n2d (source table of the update
+// kernel: sqrt(-g) w d_nu g_{kap lam}, nu = 1, 2); floorp: 2 x n2d (rho, u geometric floors)
 __global__ void geometry_kernel(GeomPar p, double* __restrict__ tab0, double* __restrict__ tab1, double* __restrict__ tab2,
-                                double* __restrict__ tab3, double* __restrict__ conn, double* __restrict__ floorp) {
+                                double* __restrict__ tab3, double* __restrict__ conn, double* __restrict__ dgt, double* __restrict__ floorp) {
   int ii = blockIdx.x * blockDim.x + threadIdx.x, jj = blockIdx.y;
   if (ii >= p.nt1 || jj >= p.nt2) return;
   long n2d = (long)p.nt1 * p.nt2, pt = (long)jj * p.nt1 + ii;
@@ -178,6 +179,13 @@ __global__ void geometry_kernel(GeomPar p, double* __restrict__ tab0, double* __
             }
             conn[(lam * 10 + sym(mu, nu)) * n2d + pt] = 0.5 * s;
           }
+      // source table: S_nu = sqrt(-g) 1/2 T^{kap lam} d_nu g_{kap lam} = sum over packed pairs c of T^c dgt[nu][c]
+      for (int c = 0; c < 10; c++) {
+        bool diag = (c == G00 || c == G11 || c == G22 || c == G33);
+        double w = diag ? 0.5 : 1.0;
+        dgt[c * n2d + pt] = gdet * w * g[c].a;
+        dgt[(10 + c) * n2d + pt] = gdet * w * g[c].b;
+      }
       double sfl = (p.coords == 0) ? 1.0 : 1.0 / (radius * radius) / (1.0 + radius / p.r_char);
       floorp[pt] = p.rho_min * sfl;
       floorp[n2d + pt] = p.u_min * pow(sfl, p.gamma);

@@ -21,7 +21,8 @@ struct GV {                 // grid view, passed by value
   int polar_lo, polar_hi;
   int ndim_mask;            // bit d set if N_d > 1 (enters the CFL sum)
   const double* geom[4];    // CENT, FACE1, FACE2, FACE3 tables
-  const double* conn;
+  const double* conn;       // Gamma table (kh_get_conn only)
+  const double* dg;         // source table, KH_NDG x n2d
   const double* floorp;
   FloorPar fp;
 };
@@ -29,7 +30,7 @@ struct GV {                 // grid view, passed by value
 struct StepScalars {        // device-resident scalars of the time stepping
   double dt;                // step used by the current kh_step
   double dt_next;           // result of the last corrector
-  unsigned long long min_bits;   // running min of 1/sum(c/dx) as ordered bits (positive doubles)
+  unsigned long long rate_bits;  // running max of sum_d(c^d/dx_d) as ordered bits (non-negative doubles): dt = cfl / max
   unsigned long long max_bits;   // scratch for max reductions
   unsigned long long n_pflag, n_fflag;
 };
@@ -61,31 +62,25 @@ template <int DIR, bool FLAT>
 __device__ __forceinline__ void face_flux(const GV& g, const double PL[KH_NP], const double PR[KH_NP], long p2, long n,
                                           double* __restrict__ F, double* __restrict__ ctop) {
   Geo G;
-  load_geo<FLAT>(G, g.geom[DIR], g.n2d, p2);
-  double UL[KH_NP], FL[KH_NP], vmaxL, vminL;
-  {
-    FourVec D;
-    four_vectors(G, PL, D);
-    prim_to_flux(G, PL, D, g.gam, 0, UL);
-    prim_to_flux(G, PL, D, g.gam, DIR, FL);
-    vchar(G, PL, D, g.gam, DIR, vmaxL, vminL);
-  }
-  double UR[KH_NP], FR[KH_NP], vmaxR, vminR;
-  {
-    FourVec D;
-    four_vectors(G, PR, D);
-    prim_to_flux(G, PR, D, g.gam, 0, UR);
-    prim_to_flux(G, PR, D, g.gam, DIR, FR);
-    vchar(G, PR, D, g.gam, DIR, vmaxR, vminR);
-  }
-  double cmax = fmax(0.0, fmax(vmaxL, vmaxR));
-  double cmin = fmax(0.0, fmax(-vminL, -vminR));
-  double c = fmax(cmax, cmin);
+  load_geo<FLAT, DIR, 0>(G, g.geom[DIR], g.n2d, p2);
+  // per-face quantities shared by the two states
+  const double ialpha = FLAT ? 1.0 : -G.n00 * G.alpha;                       // 1/alpha = -g^tt alpha
+  const double gtd = FLAT ? 0.0 : (DIR == 1 ? G.n01 : (DIR == 2 ? G.n02 : 0.0));
+  const double gdd = FLAT ? 1.0 : (DIR == 1 ? G.n11 : (DIR == 2 ? G.n22 : G.n33));
+  const double k2 = FLAT ? 1.0 : fma(gtd, gtd, -G.n00 * gdd);
+  const double gm1 = g.gam - 1.0;
+  double UL[KH_NP], FL[KH_NP], cL;
+  state_terms<DIR, FLAT>(G, ialpha, gtd, gdd, k2, PL, g.gam, gm1, UL, FL, cL);
+  double UR[KH_NP], FR[KH_NP], cR;
+  state_terms<DIR, FLAT>(G, ialpha, gtd, gdd, k2, PR, g.gam, gm1, UR, FR, cR);
+  // S14: c_top = max(0, v+L, v+R, -v-L, -v-R) = max over the states of max(|v+|, |v-|)
+  const double c = fmax(cL, cR);
+  const double hg = FLAT ? 0.5 : 0.5 * G.gdet;
   const long nt = g.ntot;
 #pragma unroll
   for (int v = 0; v < KH_NP; v++) {
     if (v == B1 + DIR - 1) continue;     // F^d[B^d] = 0, never read
-    F[v * nt + n] = 0.5 * (FL[v] + FR[v] - c * (UR[v] - UL[v]));
+    F[v * nt + n] = hg * fma(-c, UR[v] - UL[v], FL[v] + FR[v]);
   }
   ctop[n] = c;
 }
@@ -181,96 +176,125 @@ emf_kernel(GV g, const double* __restrict__ F1, const double* __restrict__ F2, c
 //   U_f = U(P_i) + Dt [ -sum_d (F^d(+1) - F^d)/dx_d + S(P_s) ],  S_nu = sqrt(-g) T^kap_lam Gamma^lam_{nu kap}
 //   P_f = floors(1D_W(U_f; guess P_i))
 // U_f never touches HBM.  The induction fluxes are formed from the edge EMFs on the fly.
+//
+// Everything is carried per sqrt(-g) (Uh = U / sqrt(-g)), which is what the inversion wants.
+// Source term: for a symmetric T, T^kap_lam Gamma^lam_{nu kap} = 1/2 T^{kap lam} d_nu g_{kap lam}; the metric is
+// stationary and axisymmetric, so only nu = 1, 2 survive and the table g.dg holds sqrt(-g) w d_nu g_{kap lam}
+// (w = 1/2 on the diagonal, 1 off it; d g_02 = d g_23 = 0 in the Kerr-Schild family): 16 table numbers and
+// ~50 fp64 instructions instead of the 40-entry Gamma table and a 64-term contraction.
+// One thread per interior zone, flattened index (no idle lanes when n1 is not a multiple of the block).
 // ---------------------------------------------------------------------------------------------
 template <bool FLAT, bool CORR>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 4)
 update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps, double* __restrict__ Pf,
               const double* __restrict__ F1, const double* __restrict__ F2, const double* __restrict__ F3,
               const double* __restrict__ e1, const double* __restrict__ e2, const double* __restrict__ e3,
               const double* __restrict__ ct1, const double* __restrict__ ct2, const double* __restrict__ ct3,
               unsigned char* __restrict__ pflag, unsigned char* __restrict__ fflag, StepScalars* __restrict__ sc,
               double dt_factor) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
-  bool active = i < g.n1;
-  double dtz = 1e300;
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long nzone = (long)g.n1 * g.n2 * g.n3;
+  const bool active = t < nzone;
+  double rate = 0.0;
   int pf_flag = 0, ff = 0;
   if (active) {
+    const unsigned tu = (unsigned)t, n1 = (unsigned)g.n1, n12 = n1 * (unsigned)g.n2;
+    const int k = (int)(tu / n12);
+    const unsigned rem = tu - (unsigned)k * n12;
+    const int j = (int)(rem / n1), i = (int)(rem - (unsigned)j * n1);
     const long n = zidx(g, i, j, k), nt = g.ntot;
     const long p2 = pidx(g, i, j);
     const double Dt = dt_factor * sc->dt;
     Geo G;
-    load_geo<FLAT>(G, g.geom[0], g.n2d, p2);
-    double pi[KH_NP], Uf[KH_NP];
-#pragma unroll
-    for (int v = 0; v < KH_NP; v++) pi[v] = Pi[v * nt + n];
+    load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, p2);
+    const double ialpha = FLAT ? 1.0 : -G.n00 * G.alpha;
+    const double gm1 = g.gam - 1.0;
+    double Uh[KH_NP], W0, S1 = 0.0, S2 = 0.0;
     {
+      double pi[KH_NP];
+#pragma unroll
+      for (int v = 0; v < KH_NP; v++) pi[v] = Pi[v * nt + n];
       FourVec D;
-      four_vectors(G, pi, D);
-      prim_to_flux(G, pi, D, g.gam, 0, Uf);
-    }
-    double S[4] = {0.0, 0.0, 0.0, 0.0};
-    if (!FLAT) {
-      double ps[KH_NP];
+      four_vectors<FLAT>(G, ialpha, pi, D);
+      double pg = gm1 * pi[UU], ef = fma(g.gam, pi[UU], pi[RHO]);
+      double ee = ef + D.bsq, ptot = fma(0.5, D.bsq, pg);
+      double eu[4] = {ee * D.ucov[0], ee * D.ucov[1], ee * D.ucov[2], ee * D.ucov[3]};
+      flux_row(pi, D, eu, ptot, 0, Uh);
+      W0 = ef * D.x;
+      if (!FLAT) {
+        double ps[KH_NP];
+        if (CORR) {
 #pragma unroll
-      for (int v = 0; v < KH_NP; v++) ps[v] = CORR ? Ps[v * nt + n] : pi[v];
-      FourVec D;
-      four_vectors(G, ps, D);
-      double pg = (g.gam - 1.0) * ps[UU];
-      double eta = ps[RHO] + ps[UU] + pg + D.bsq, ptot = pg + 0.5 * D.bsq;
-#pragma unroll
-      for (int kap = 0; kap < 4; kap++) {
-#pragma unroll
-        for (int lam = 0; lam < 4; lam++) {
-          double T = eta * D.ucon[kap] * D.ucov[lam] - D.bcon[kap] * D.bcov[lam] + (kap == lam ? ptot : 0.0);
-#pragma unroll
-          for (int nu = 0; nu < 4; nu++) S[nu] += T * __ldg(g.conn + (lam * 10 + sym(nu, kap)) * g.n2d + p2);
+          for (int v = 0; v < KH_NP; v++) ps[v] = Ps[v * nt + n];
+          four_vectors<FLAT>(G, ialpha, ps, D);
+          pg = gm1 * ps[UU];
+          ee = fma(g.gam, ps[UU], ps[RHO]) + D.bsq;
+          ptot = fma(0.5, D.bsq, pg);
         }
+        // T^{kap lam} = (w + b^2) u^kap u^lam + (p + b^2/2) g^{kap lam} - b^kap b^lam on the packed pairs with d g != 0
+        const double* __restrict__ dg = g.dg + p2;
+        const long m = g.n2d;
+        double eu0 = ee * D.ucon[0], eu1 = ee * D.ucon[1], eu2 = ee * D.ucon[2], eu3 = ee * D.ucon[3];
+#define KH_T(a, b, gc) fma(eu##a, D.ucon[b], fma(ptot, gc, -D.bcon[a] * D.bcon[b]))
+#define KH_ACC(c, T) { double T_ = (T); S1 = fma(T_, __ldg(dg + (long)(c) * m), S1); S2 = fma(T_, __ldg(dg + (long)(10 + (c)) * m), S2); }
+        KH_ACC(G00, KH_T(0, 0, G.n00));
+        KH_ACC(G01, KH_T(0, 1, G.n01));
+        KH_ACC(G03, fma(eu0, D.ucon[3], -D.bcon[0] * D.bcon[3]));            // g^03 = 0
+        KH_ACC(G11, KH_T(1, 1, G.n11));
+        KH_ACC(G12, KH_T(1, 2, G.n12));
+        KH_ACC(G13, KH_T(1, 3, G.n13));
+        KH_ACC(G22, KH_T(2, 2, G.n22));
+        KH_ACC(G33, KH_T(3, 3, G.n33));
+#undef KH_T
+#undef KH_ACC
       }
     }
+    const double dtg = FLAT ? Dt : Dt * fast_rcp(G.gdet);
     // hydro flux divergence
 #pragma unroll
     for (int v = 0; v < 5; v++) {
-      double div = (F1[v * nt + n + 1] - F1[v * nt + n]) * g.idx1 + (F2[v * nt + n + g.s2] - F2[v * nt + n]) * g.idx2 +
-                   (F3[v * nt + n + g.s3] - F3[v * nt + n]) * g.idx3;
-      double src = (v >= 1) ? G.gdet * S[v - 1] : 0.0;
-      Uf[v] += Dt * (src - div);
+      const double* f1 = F1 + v * nt + n;
+      const double* f2 = F2 + v * nt + n;
+      const double* f3 = F3 + v * nt + n;
+      double div = fma(f3[g.s3] - f3[0], g.idx3, fma(f2[g.s2] - f2[0], g.idx2, (f1[1] - f1[0]) * g.idx1));
+      double src = (v == 2) ? S1 : (v == 3 ? S2 : 0.0);
+      Uh[v] = fma(dtg, src - div, Uh[v]);
     }
-    // induction: Flux-CT fluxes from the edge EMFs (S15a)
+    // induction: Flux-CT fluxes from the edge EMFs (S15a); the factors 1/2 are applied once per component
     {
       const long s2 = g.s2, s3 = g.s3;
-      // F2[B1] = -1/2 (e3(i,j)+e3(i+1,j)) ; F3[B1] = 1/2 (e2(i,k)+e2(i+1,k))
-      double f2b1_lo = -0.5 * (e3[n] + e3[n + 1]), f2b1_hi = -0.5 * (e3[n + s2] + e3[n + s2 + 1]);
-      double f3b1_lo = 0.5 * (e2[n] + e2[n + 1]), f3b1_hi = 0.5 * (e2[n + s3] + e2[n + s3 + 1]);
-      Uf[B1] -= Dt * ((f2b1_hi - f2b1_lo) * g.idx2 + (f3b1_hi - f3b1_lo) * g.idx3);
-      // F1[B2] = 1/2 (e3(i,j)+e3(i,j+1)) ; F3[B2] = -1/2 (e1(j,k)+e1(j+1,k))
-      double f1b2_lo = 0.5 * (e3[n] + e3[n + s2]), f1b2_hi = 0.5 * (e3[n + 1] + e3[n + 1 + s2]);
-      double f3b2_lo = -0.5 * (e1[n] + e1[n + s2]), f3b2_hi = -0.5 * (e1[n + s3] + e1[n + s3 + s2]);
-      Uf[B2] -= Dt * ((f1b2_hi - f1b2_lo) * g.idx1 + (f3b2_hi - f3b2_lo) * g.idx3);
-      // F1[B3] = -1/2 (e2(i,k)+e2(i,k+1)) ; F2[B3] = 1/2 (e1(j,k)+e1(j,k+1))
-      double f1b3_lo = -0.5 * (e2[n] + e2[n + s3]), f1b3_hi = -0.5 * (e2[n + 1] + e2[n + 1 + s3]);
-      double f2b3_lo = 0.5 * (e1[n] + e1[n + s3]), f2b3_hi = 0.5 * (e1[n + s2] + e1[n + s2 + s3]);
-      Uf[B3] -= Dt * ((f1b3_hi - f1b3_lo) * g.idx1 + (f2b3_hi - f2b3_lo) * g.idx2);
+      const double a00 = e3[n], a10 = e3[n + 1], a01 = e3[n + s2], a11 = e3[n + s2 + 1];          // emf3 at (i,j) corners
+      const double b00 = e2[n], b10 = e2[n + 1], b01 = e2[n + s3], b11 = e2[n + s3 + 1];          // emf2 at (i,k) corners
+      const double c00 = e1[n], c10 = e1[n + s2], c01 = e1[n + s3], c11 = e1[n + s2 + s3];        // emf1 at (j,k) corners
+      const double h = 0.5 * dtg;
+      // dB1/dt = -[d2 F2[B1] + d3 F3[B1]],  F2[B1] = -1/2 (e3(i,j)+e3(i+1,j)),  F3[B1] = 1/2 (e2(i,k)+e2(i+1,k))
+      Uh[B1] = fma(h, ((a01 + a11) - (a00 + a10)) * g.idx2 - ((b01 + b11) - (b00 + b10)) * g.idx3, Uh[B1]);
+      // dB2/dt = -[d1 F1[B2] + d3 F3[B2]],  F1[B2] = 1/2 (e3(i,j)+e3(i,j+1)),  F3[B2] = -1/2 (e1(j,k)+e1(j+1,k))
+      Uh[B2] = fma(h, ((c01 + c11) - (c00 + c10)) * g.idx3 - ((a10 + a11) - (a00 + a01)) * g.idx1, Uh[B2]);
+      // dB3/dt = -[d1 F1[B3] + d2 F2[B3]],  F1[B3] = -1/2 (e2(i,k)+e2(i,k+1)),  F2[B3] = 1/2 (e1(j,k)+e1(j,k+1))
+      Uh[B3] = fma(h, ((b10 + b11) - (b00 + b01)) * g.idx1 - ((c10 + c11) - (c00 + c01)) * g.idx2, Uh[B3]);
     }
     double pf[KH_NP];
-    pf_flag = u_to_p(G, Uf, pi, g.gam, pf);
-    if (pf_flag == 0) {
-      double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2);
-      double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
-      ff = apply_floors(G, g.fp, rho_g, u_g, pf);
+    {
+      const double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2);
+      const double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
+      pf_flag = u_to_p_floors<FLAT>(G, Uh, W0, g.gam, g.fp, rho_g, u_g, pf, ff);
+    }
+    if (pf_flag != 0) {          // rare: the hydro primitives keep the guess (S16)
+#pragma unroll
+      for (int v = 0; v < 5; v++) pf[v] = Pi[v * nt + n];
     }
 #pragma unroll
     for (int v = 0; v < KH_NP; v++) Pf[v * nt + n] = pf[v];
     pflag[n] = (unsigned char)pf_flag;
     fflag[n] = (unsigned char)ff;
-    if (CORR) {   // K6: CFL from the corrector's face speeds (S22)
-      double s = 0.0;
-      if (g.ndim_mask & 1) s += fmax(ct1[n], ct1[n + 1]) * g.idx1;
-      if (g.ndim_mask & 2) s += fmax(ct2[n], ct2[n + g.s2]) * g.idx2;
-      if (g.ndim_mask & 4) s += fmax(ct3[n], ct3[n + g.s3]) * g.idx3;
-      dtz = 1.0 / s;
+    if (CORR) {   // K6: CFL from the corrector's face speeds (S22): dt_zone = 1 / rate
+      if (g.ndim_mask & 1) rate = fmax(ct1[n], ct1[n + 1]) * g.idx1;
+      if (g.ndim_mask & 2) rate = fma(fmax(ct2[n], ct2[n + g.s2]), g.idx2, rate);
+      if (g.ndim_mask & 4) rate = fma(fmax(ct3[n], ct3[n + g.s3]), g.idx3, rate);
     }
   }
-  // block-level bookkeeping: failure counters and the CFL minimum
+  // block-level bookkeeping: failure counters and the CFL rate maximum (min over zones of 1/rate = 1/max rate)
   unsigned np = __syncthreads_count(pf_flag != 0);
   unsigned nf = __syncthreads_count(ff != 0);
   if (threadIdx.x == 0) {
@@ -279,23 +303,23 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
   }
   if (CORR) {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) dtz = fmin(dtz, __shfl_xor_sync(0xffffffffu, dtz, o));
-    __shared__ double wmin[4];
-    if ((threadIdx.x & 31) == 0) wmin[threadIdx.x >> 5] = dtz;
+    for (int o = 16; o > 0; o >>= 1) rate = fmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
+    __shared__ double wmax[4];
+    if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = rate;
     __syncthreads();
     if (threadIdx.x == 0) {
-      double m = fmin(fmin(wmin[0], wmin[1]), fmin(wmin[2], wmin[3]));
-      atomicMin(&sc->min_bits, (unsigned long long)__double_as_longlong(m));   // positive doubles order as integers
+      double m = fmax(fmax(wmax[0], wmax[1]), fmax(wmax[2], wmax[3]));
+      atomicMax(&sc->rate_bits, (unsigned long long)__double_as_longlong(m));   // non-negative doubles order as integers
     }
   }
 }
 
-// dt_next = min(cfl * min_zones, growth * dt); reset accumulators.
+// dt_next = min(cfl / max_zones rate, growth * dt); reset the accumulator.
 __global__ void finalize_dt_kernel(StepScalars* sc, double cfl, double growth) {
-  double m = __longlong_as_double((long long)sc->min_bits);
+  double m = 1.0 / __longlong_as_double((long long)sc->rate_bits);
   double d = cfl * m, cap = growth * sc->dt;
   sc->dt_next = d < cap ? d : cap;
-  sc->min_bits = 0x7FF0000000000000ULL;   // +inf
+  sc->rate_bits = 0ULL;
 }
 __global__ void set_dt_kernel(StepScalars* sc, double dt, int from_next) { sc->dt = from_next ? sc->dt_next : dt; }
 __global__ void reset_counters_kernel(StepScalars* sc) { sc->n_pflag = 0; sc->n_fflag = 0; }
@@ -396,10 +420,10 @@ fixup_apply_kernel(GV g, double* __restrict__ Pf, const unsigned char* __restric
 #pragma unroll
   for (int v = 5; v < KH_NP; v++) P[v] = Pf[v * nt + n];
   Geo G;
-  load_geo<FLAT>(G, g.geom[0], g.n2d, p2);
+  load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, p2);
   double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2);
   double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
-  int ff = apply_floors(G, g.fp, rho_g, u_g, P);
+  int ff = apply_floors<FLAT>(G, g.fp, rho_g, u_g, P);
 #pragma unroll
   for (int v = 0; v < 5; v++) Pf[v * nt + n] = P[v];
   fflag[n] |= (unsigned char)ff;
@@ -414,36 +438,38 @@ __global__ void cons_kernel(GV g, const double* __restrict__ P, double* __restri
   if (i >= g.n1) return;
   const long n = zidx(g, i, j, k), nt = g.ntot;
   Geo G;
-  load_geo<FLAT>(G, g.geom[0], g.n2d, pidx(g, i, j));
+  load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, pidx(g, i, j));
   double p[KH_NP], U[KH_NP];
   for (int v = 0; v < KH_NP; v++) p[v] = P[v * nt + n];
   FourVec D;
-  four_vectors(G, p, D);
-  prim_to_flux(G, p, D, g.gam, 0, U);
+  four_vectors<FLAT>(G, FLAT ? 1.0 : -G.n00 * G.alpha, p, D);
+  double pg = (g.gam - 1.0) * p[UU], ee = fma(g.gam, p[UU], p[RHO]) + D.bsq, ptot = fma(0.5, D.bsq, pg);
+  double eu[4] = {ee * D.ucov[0], ee * D.ucov[1], ee * D.ucov[2], ee * D.ucov[3]};
+  flux_row(p, D, eu, ptot, 0, U);
   long nin = (long)g.n1 * g.n2 * g.n3, m = ((long)k * g.n2 + j) * g.n1 + i;
-  for (int v = 0; v < KH_NP; v++) Uout[v * nin + m] = U[v];
+  for (int v = 0; v < KH_NP; v++) Uout[v * nin + m] = G.gdet * U[v];
 }
 
+// First-step CFL estimate from zone-centred speeds (S22): max over zones of sum_d c^d / dx_d.
 template <bool FLAT>
 __global__ void estimate_dt_kernel(GV g, const double* __restrict__ P, StepScalars* __restrict__ sc) {
   int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
-  double dtz = 1e300;
+  double rate = 0.0;
   if (i < g.n1) {
     const long n = zidx(g, i, j, k), nt = g.ntot;
     Geo G;
-    load_geo<FLAT>(G, g.geom[0], g.n2d, pidx(g, i, j));
+    load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, pidx(g, i, j));
     double p[KH_NP];
     for (int v = 0; v < KH_NP; v++) p[v] = P[v * nt + n];
     FourVec D;
-    four_vectors(G, p, D);
-    double s = 0.0, vmax, vmin;
-    if (g.ndim_mask & 1) { vchar(G, p, D, g.gam, 1, vmax, vmin); s += fmax(fabs(vmax), fabs(vmin)) * g.idx1; }
-    if (g.ndim_mask & 2) { vchar(G, p, D, g.gam, 2, vmax, vmin); s += fmax(fabs(vmax), fabs(vmin)) * g.idx2; }
-    if (g.ndim_mask & 4) { vchar(G, p, D, g.gam, 3, vmax, vmin); s += fmax(fabs(vmax), fabs(vmin)) * g.idx3; }
-    dtz = 1.0 / s;
+    four_vectors<FLAT>(G, FLAT ? 1.0 : -G.n00 * G.alpha, p, D);
+    double pg = (g.gam - 1.0) * p[UU], ee = fma(g.gam, p[UU], p[RHO]) + D.bsq, gg1u = g.gam * pg;
+    if (g.ndim_mask & 1) rate = fma(cfast<FLAT>(D, ee, gg1u, G.n00, G.n01, G.n11, fma(G.n01, G.n01, -G.n00 * G.n11), 1), g.idx1, rate);
+    if (g.ndim_mask & 2) rate = fma(cfast<FLAT>(D, ee, gg1u, G.n00, G.n02, G.n22, fma(G.n02, G.n02, -G.n00 * G.n22), 2), g.idx2, rate);
+    if (g.ndim_mask & 4) rate = fma(cfast<FLAT>(D, ee, gg1u, G.n00, 0.0, G.n33, -G.n00 * G.n33, 3), g.idx3, rate);
   }
-  for (int o = 16; o > 0; o >>= 1) dtz = fmin(dtz, __shfl_xor_sync(0xffffffffu, dtz, o));
-  if ((threadIdx.x & 31) == 0) atomicMin(&sc->min_bits, (unsigned long long)__double_as_longlong(dtz));
+  for (int o = 16; o > 0; o >>= 1) rate = fmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
+  if ((threadIdx.x & 31) == 0) atomicMax(&sc->rate_bits, (unsigned long long)__double_as_longlong(rate));
 }
 
 // corner-centred divergence preserved by Flux-CT; corners (i-1/2, j-1/2, k-1/2)

@@ -32,6 +32,7 @@ struct kh_grid {
   // device buffers
   double* geom[4];
   double* conn;
+  double* dg;
   double* floorp;
   double* P[3];          // P^n, P*, P^{n+1} (rotating)
   double* F[3];          // face fluxes per direction, [8][ntot]
@@ -177,7 +178,7 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
   emf_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], g->emf[2]);
   prof_end(g);
   g->launches++;
-  dim3 grid = zone_grid(v.n1, v.n2, v.n3);
+  const unsigned grid = (unsigned)(((long)v.n1 * v.n2 * v.n3 + 127) / 128);
 #define UPD(FL, CO)                                                                                                  \
   update_kernel<FL, CO><<<grid, 128, 0, g->stream>>>(v, Pi, Ps, Pf, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], \
                                                      g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, g->fflag, g->sc, dt_factor)
@@ -237,7 +238,7 @@ int kh_grid_destroy(kh_grid* g) {
   if (!g) return KH_OK;
   destroy_graphs(g);
   for (int l = 0; l < 4; l++) cudaFree(g->geom[l]);
-  cudaFree(g->conn); cudaFree(g->floorp);
+  cudaFree(g->conn); cudaFree(g->dg); cudaFree(g->floorp);
   for (int b = 0; b < 3; b++) { cudaFree(g->P[b]); cudaFree(g->F[b]); cudaFree(g->ctop[b]); cudaFree(g->emf[b]); }
   cudaFree(g->pflag); cudaFree(g->fflag); cudaFree(g->sc); cudaFree(g->fix); cudaFree(g->stage);
   if (g->sc_host) cudaFreeHost(g->sc_host);
@@ -313,6 +314,7 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   const size_t fb = sizeof(double) * v.ntot;
   for (int l = 0; l < 4; l++) ALLOC(g->geom[l], sizeof(double) * KH_NGEO * v.n2d);
   ALLOC(g->conn, sizeof(double) * KH_NCONN * v.n2d);
+  ALLOC(g->dg, sizeof(double) * KH_NDG * v.n2d);
   ALLOC(g->floorp, sizeof(double) * 2 * v.n2d);
   for (int b = 0; b < 3; b++) {
     ALLOC(g->P[b], KH_NP * fb);
@@ -327,10 +329,9 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
 #undef ALLOC
   if (cudaMallocHost((void**)&g->sc_host, sizeof(StepScalars)) != cudaSuccess) { kh_grid_destroy(g); return KH_ENOMEM; }
   memset(g->sc_host, 0, sizeof(StepScalars));
-  g->sc_host->min_bits = 0x7FF0000000000000ULL;
   if (cudaMemcpyAsync(g->sc, g->sc_host, sizeof(StepScalars), cudaMemcpyHostToDevice, g->stream) != cudaSuccess) { kh_grid_destroy(g); return KH_ECUDA; }
   for (int l = 0; l < 4; l++) v.geom[l] = g->geom[l];
-  v.conn = g->conn; v.floorp = g->floorp;
+  v.conn = g->conn; v.dg = g->dg; v.floorp = g->floorp;
 
   GeomPar gp;
   gp.coords = p->coords; gp.a = p->a; gp.hslope = p->hslope; gp.poly_xt = p->poly_xt; gp.poly_alpha = p->poly_alpha;
@@ -339,7 +340,7 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   gp.dx1 = (p->xmax[0] - p->xmin[0]) / v.n1; gp.dx2 = (p->xmax[1] - p->xmin[1]) / v.n2;
   gp.nt1 = v.nt1; gp.nt2 = v.nt2; gp.n2 = v.n2; gp.polar_lo = v.polar_lo; gp.polar_hi = v.polar_hi;
   gp.rho_min = p->rho_min; gp.u_min = p->u_min; gp.r_char = p->r_char; gp.gamma = p->gamma;
-  geometry_kernel<<<dim3((v.nt1 + 63) / 64, v.nt2), 64, 0, g->stream>>>(gp, g->geom[0], g->geom[1], g->geom[2], g->geom[3], g->conn, g->floorp);
+  geometry_kernel<<<dim3((v.nt1 + 63) / 64, v.nt2), 64, 0, g->stream>>>(gp, g->geom[0], g->geom[1], g->geom[2], g->geom[3], g->conn, g->dg, g->floorp);
   g->launches++;
   cudaError_t e = cudaStreamSynchronize(g->stream);
   if (e == cudaSuccess) e = cudaGetLastError();
@@ -447,13 +448,12 @@ int kh_estimate_dt(kh_grid* g, double* dt) {
   CK(cudaGetLastError());
   int rc = read_scalars(g);
   if (rc) return rc;
-  double m;
-  memcpy(&m, &g->sc_host->min_bits, sizeof(double));
-  unsigned long long inf = 0x7FF0000000000000ULL;
-  CK(cudaMemcpyAsync(&g->sc->min_bits, &inf, sizeof(inf), cudaMemcpyHostToDevice, g->stream));
+  double rate;
+  memcpy(&rate, &g->sc_host->rate_bits, sizeof(double));
+  CK(cudaMemsetAsync(&g->sc->rate_bits, 0, sizeof(unsigned long long), g->stream));
   CK(cudaStreamSynchronize(g->stream));
-  if (!(m == m)) return KH_ENAN;
-  *dt = g->p.cfl * m;
+  if (!(rate == rate)) return KH_ENAN;
+  *dt = g->p.cfl * (1.0 / rate);            // min over zones of 1/rate = 1/max rate
   return KH_OK;
 }
 
