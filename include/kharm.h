@@ -110,7 +110,7 @@ int kh_get_conn(kh_grid* g, double* conn64, int mem);
 int kh_get_flux(kh_grid* g, int dir, double* F, double* ctop, int mem);
 /* Edge EMFs of the last sub-step, with ghosts [nt], index = lower edge of the zone. */
 int kh_get_emf(kh_grid* g, int dir, double* emf, int mem);
-/* Run the fix-up (K5b) + floors on the current primitives for a caller-supplied flag array
+/* Run the fix-up (K5b) + floors + refresh of the fixed zones' ghost images on the current primitives for a caller-supplied flag array
  * (int32, with ghosts [nt]); test hook for hand-built neighbourhoods. */
 int kh_debug_fixup(kh_grid* g, const int* pflag_with_ghosts, int mem);
 /* Run only the predictor sub-step P* = substep(P^n, P^n, dt/2) and make P* the current state (test hook:

@@ -8,6 +8,17 @@
 #pragma once
 #include "kh_device.cuh"
 
+// Minimum resident blocks per SM of the hot kernels (register caps: 4 -> 128, 5 -> 102, 6 -> 85 registers).
+#ifndef KH_MINB_X1
+#define KH_MINB_X1 4
+#endif
+#ifndef KH_MINB_MARCH
+#define KH_MINB_MARCH 3
+#endif
+#ifndef KH_MINB_UPDATE
+#define KH_MINB_UPDATE 4
+#endif
+
 namespace kh {
 
 struct GV {                 // grid view, passed by value
@@ -34,6 +45,8 @@ struct StepScalars {        // device-resident scalars of the time stepping
   unsigned long long max_bits;   // scratch for max reductions
   unsigned long long n_pflag, n_fflag;
 };
+
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 __device__ __forceinline__ long zidx(const GV& g, int i, int j, int k) {
   return (long)(k + KH_NGH) * g.s3 + (long)(j + KH_NGH) * g.s2 + (i + KH_NGH);
@@ -86,7 +99,7 @@ __device__ __forceinline__ void face_flux(const GV& g, const double PL[KH_NP], c
 }
 
 template <int RECON, bool FLAT>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, KH_MINB_X1)
 flux_x1_kernel(GV g, const double* __restrict__ P, double* __restrict__ F, double* __restrict__ ctop) {
   const int c1 = g.n1 + 2, c2 = g.n2 + 2;                // zones -1 .. N per row; rows (j, k) in [-1, N]
   const long Z = (long)c1 * c2 * (g.n3 + 2);
@@ -112,7 +125,7 @@ flux_x1_kernel(GV g, const double* __restrict__ P, double* __restrict__ F, doubl
 
 // x2 / x3: thread <-> (i, transverse index), marching over faces [f0, f1) of chunk blockIdx.y.
 template <int DIR, int RECON, bool FLAT>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, KH_MINB_MARCH)
 flux_march_kernel(GV g, const double* __restrict__ P, double* __restrict__ F, double* __restrict__ ctop, int J) {
   const int c1 = g.n1 + 2;
   const int cb = (DIR == 2 ? g.n3 : g.n2) + 2;
@@ -185,13 +198,13 @@ emf_kernel(GV g, const double* __restrict__ F1, const double* __restrict__ F2, c
 // One thread per interior zone, flattened index (no idle lanes when n1 is not a multiple of the block).
 // ---------------------------------------------------------------------------------------------
 template <bool FLAT, bool CORR>
-__global__ void __launch_bounds__(128, 4)
+__global__ void __launch_bounds__(128, KH_MINB_UPDATE)
 update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps, double* __restrict__ Pf,
               const double* __restrict__ F1, const double* __restrict__ F2, const double* __restrict__ F3,
               const double* __restrict__ e1, const double* __restrict__ e2, const double* __restrict__ e3,
               const double* __restrict__ ct1, const double* __restrict__ ct2, const double* __restrict__ ct3,
-              unsigned char* __restrict__ pflag, unsigned char* __restrict__ fflag, StepScalars* __restrict__ sc,
-              double dt_factor) {
+              unsigned char* __restrict__ pflag, unsigned char* __restrict__ fflag, unsigned* __restrict__ faillist,
+              StepScalars* __restrict__ sc, double dt_factor) {
   const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
   const long nzone = (long)g.n1 * g.n2 * g.n3;
   const bool active = t < nzone;
@@ -204,6 +217,16 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
     const int j = (int)(rem / n1), i = (int)(rem - (unsigned)j * n1);
     const long n = zidx(g, i, j, k), nt = g.ntot;
     const long p2 = pidx(g, i, j);
+    // Pull this zone's streamed inputs (fluxes, EMFs, P_s, c_top) towards L2 now: they are consumed only after the
+    // geometry loads and the four-vector arithmetic below, and a prefetch holds no register.
+#pragma unroll
+    for (int v = 0; v < 5; v++) { prefetch_l2(F1 + v * nt + n); prefetch_l2(F2 + v * nt + n); prefetch_l2(F3 + v * nt + n); }
+    prefetch_l2(e1 + n); prefetch_l2(e2 + n); prefetch_l2(e3 + n);
+    if (CORR) {
+#pragma unroll
+      for (int v = 0; v < KH_NP; v++) prefetch_l2(Ps + v * nt + n);
+      prefetch_l2(ct1 + n); prefetch_l2(ct2 + n); prefetch_l2(ct3 + n);
+    }
     const double Dt = dt_factor * sc->dt;
     Geo G;
     load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, p2);
@@ -280,9 +303,10 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
       const double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
       pf_flag = u_to_p_floors<FLAT>(G, Uh, W0, g.gam, g.fp, rho_g, u_g, pf, ff);
     }
-    if (pf_flag != 0) {          // rare: the hydro primitives keep the guess (S16)
+    if (pf_flag != 0) {          // rare: the hydro primitives keep the guess (S16); queue the zone for the fix-up
 #pragma unroll
       for (int v = 0; v < 5; v++) pf[v] = Pi[v * nt + n];
+      faillist[atomicAdd(&sc->n_pflag, 1ULL)] = (unsigned)n;
     }
 #pragma unroll
     for (int v = 0; v < KH_NP; v++) Pf[v * nt + n] = pf[v];
@@ -295,12 +319,8 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
     }
   }
   // block-level bookkeeping: failure counters and the CFL rate maximum (min over zones of 1/rate = 1/max rate)
-  unsigned np = __syncthreads_count(pf_flag != 0);
   unsigned nf = __syncthreads_count(ff != 0);
-  if (threadIdx.x == 0) {
-    if (np) atomicAdd(&sc->n_pflag, (unsigned long long)np);
-    if (nf) atomicAdd(&sc->n_fflag, (unsigned long long)nf);
-  }
+  if (threadIdx.x == 0 && nf) atomicAdd(&sc->n_fflag, (unsigned long long)nf);
   if (CORR) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) rate = fmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
@@ -325,49 +345,67 @@ __global__ void set_dt_kernel(StepScalars* sc, double dt, int from_next) { sc->d
 __global__ void reset_counters_kernel(StepScalars* sc) { sc->n_pflag = 0; sc->n_fflag = 0; }
 
 // ---------------------------------------------------------------------------------------------
-// K7: ghost fill along DIR (0,1,2), spanning the full extent of the other directions (S20).
-// One thread per ghost zone of that direction; all 8 primitives (and optionally the flag byte).
+// K7: ghost fill (S20).  The scheme's definition is three sequential passes x1 -> x2 -> x3, each spanning the
+// full extent of the other directions.  Every pass copies along one index, so their composition is a gather
+// from ONE interior-or-fixed source zone per ghost zone: source index = (m1(a), m2(b), m3(c)) with the per-
+// direction maps below, value transforms applied in pass order (outflow: B rescaled by the ratio of tabulated
+// sqrt(-g), S20b; polar: sign of ut^2, B^2).  One launch, bit-identical to the three passes.
 // ---------------------------------------------------------------------------------------------
-template <int DIR>
+enum { KH_MAP_ID = 0, KH_MAP_COPY = 1, KH_MAP_OUTFLOW = 2, KH_MAP_POLAR = 3 };
+
+// index gi in [-NG, N+NG) along one direction -> source index and the kind of the map
+__device__ __forceinline__ int ghost_map(int gi, int N, int bc_lo, int bc_hi, int& kind) {
+  kind = KH_MAP_ID;
+  if (gi >= 0 && gi < N) return gi;
+  const int side = gi >= N;
+  const int bc = side ? bc_hi : bc_lo;
+  if (bc == 3) return gi;                                   // fixed: the ghost keeps its content
+  if (bc == 0) { kind = KH_MAP_COPY; return ((gi % N) + N) % N; }
+  if (bc == 1) { kind = KH_MAP_OUTFLOW; return side ? N - 1 : 0; }
+  kind = KH_MAP_POLAR;
+  return side ? 2 * N - 1 - gi : -1 - gi;                   // ghost -1-m <- m ; ghost N+m <- N-1-m
+}
+
 __global__ void __launch_bounds__(128)
-fill_kernel(GV g, double* __restrict__ P, unsigned char* __restrict__ flag, const StepScalars* __restrict__ sc, int only_if_failed) {
-  if (only_if_failed && sc->n_pflag == 0) return;
-  // thread -> (m in [0, 2 NG), a, b) with a the faster transverse index
-  const int na = (DIR == 0) ? g.nt2 : g.nt1;
-  const int nb = (DIR == 2) ? g.nt2 : g.nt3;
+fill_kernel(GV g, double* __restrict__ P, unsigned char* __restrict__ flag) {
+  // ghost shell = slab A (k ghost, all i, j) + slab B (j ghost, k interior, all i) + slab C (i ghost, j, k interior)
+  const long nA = (long)g.nt1 * g.nt2 * (2 * KH_NGH), nB = (long)g.nt1 * (2 * KH_NGH) * g.n3, nC = (long)(2 * KH_NGH) * g.n2 * g.n3;
   long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
-  long total = (long)2 * KH_NGH * na * nb;
-  if (t >= total) return;
-  int a, b, m;
-  if (DIR == 0) { m = t % (2 * KH_NGH); a = (t / (2 * KH_NGH)) % na; b = t / ((long)2 * KH_NGH * na); }
-  else { a = t % na; m = (t / na) % (2 * KH_NGH); b = t / ((long)na * 2 * KH_NGH); }
-  const int N = (DIR == 0) ? g.n1 : (DIR == 1 ? g.n2 : g.n3);
-  const int side = m >= KH_NGH;
-  const int mm = side ? m - KH_NGH : m;
-  const int bc = g.bc[2 * DIR + side];
-  if (bc == 3) return;   // fixed
-  const int gi = side ? N + mm : -1 - mm;
-  int si;
-  double sign = 1.0;
-  if (bc == 0) { si = ((gi % N) + N) % N; }
-  else if (bc == 1) { si = side ? N - 1 : 0; }
-  else { si = side ? N - 1 - mm : mm; sign = -1.0; }
-  int ig, jg, kg, is, js, ks;   // interior-based indices of ghost / source
-  if (DIR == 0) { ig = gi; is = si; jg = js = a - KH_NGH; kg = ks = b - KH_NGH; }
-  else if (DIR == 1) { ig = is = a - KH_NGH; jg = gi; js = si; kg = ks = b - KH_NGH; }
-  else { ig = is = a - KH_NGH; jg = js = b - KH_NGH; kg = gi; ks = si; }
-  const long ng = zidx(g, ig, jg, kg), ns = zidx(g, is, js, ks), nt = g.ntot;
-  double bscale = 1.0;
-  if (bc == 1) {   // S20b: outflow ghosts keep sqrt(-g) B^i
-    const double* gd = g.geom[0] + 20 * g.n2d;
-    bscale = __ldg(gd + pidx(g, is, js)) / __ldg(gd + pidx(g, ig, jg));
+  int a, b, c;    // interior-based indices of the ghost zone
+  if (t < nA) {
+    a = (int)(t % g.nt1) - KH_NGH; long r = t / g.nt1;
+    b = (int)(r % g.nt2) - KH_NGH; int m = (int)(r / g.nt2);
+    c = m < KH_NGH ? m - KH_NGH : g.n3 + m - KH_NGH;
+  } else if (t < nA + nB) {
+    t -= nA;
+    a = (int)(t % g.nt1) - KH_NGH; long r = t / g.nt1;
+    int m = (int)(r % (2 * KH_NGH)); c = (int)(r / (2 * KH_NGH));
+    b = m < KH_NGH ? m - KH_NGH : g.n2 + m - KH_NGH;
+  } else if (t < nA + nB + nC) {
+    t -= nA + nB;
+    int m = (int)(t % (2 * KH_NGH)); long r = t / (2 * KH_NGH);
+    b = (int)(r % g.n2); c = (int)(r / g.n2);
+    a = m < KH_NGH ? m - KH_NGH : g.n1 + m - KH_NGH;
+  } else {
+    return;
   }
+  int k1, k2, k3;
+  const int s1 = ghost_map(a, g.n1, g.bc[0], g.bc[1], k1);
+  const int s2 = ghost_map(b, g.n2, g.bc[2], g.bc[3], k2);
+  const int s3 = ghost_map(c, g.n3, g.bc[4], g.bc[5], k3);
+  if (k1 == KH_MAP_ID && k2 == KH_MAP_ID && k3 == KH_MAP_ID) return;      // fixed ghost (or nothing to do)
+  const long ng = zidx(g, a, b, c), ns = zidx(g, s1, s2, s3), nt = g.ntot;
   if (P) {
+    const double* gd = g.geom[0] + 20 * g.n2d;
+    double r1 = 1.0, r2 = 1.0;
+    if (k1 == KH_MAP_OUTFLOW) r1 = __ldg(gd + pidx(g, s1, s2)) / __ldg(gd + pidx(g, a, s2));     // pass 1 acts on row s2
+    if (k2 == KH_MAP_OUTFLOW) r2 = __ldg(gd + pidx(g, a, s2)) / __ldg(gd + pidx(g, a, b));       // pass 2 acts on column a
 #pragma unroll
     for (int v = 0; v < KH_NP; v++) {
       double val = P[v * nt + ns];
-      if (bc == 2 && (v == U2 || v == B2)) val = sign * val;
-      if (v >= B1) val *= bscale;
+      if (v >= B1) { if (k1 == KH_MAP_OUTFLOW) val *= r1; }
+      if (k2 == KH_MAP_POLAR && (v == U2 || v == B2)) val = -val;
+      if (v >= B1) { if (k2 == KH_MAP_OUTFLOW) val *= r2; }
       P[v * nt + ng] = val;
     }
   }
@@ -375,58 +413,111 @@ fill_kernel(GV g, double* __restrict__ P, unsigned char* __restrict__ flag, cons
 }
 
 // ---------------------------------------------------------------------------------------------
-// K5b: fix-up of failed inversions (S19): 26-neighbour weighted mean of good zones from the
-// pre-fix-up snapshot (two kernels: gather into scratch, then apply + floors).
+// K5b: fix-up of failed inversions (S19): 26-neighbour weighted mean of good zones from the pre-fix-up
+// snapshot.  The update kernel appends every failed zone to a list, so both kernels run over the list only
+// (one small grid-stride launch each): gather into scratch, then apply + floors + refresh of the zone's
+// ghost images (which replaces the second ghost fill of the sub-step: only the five hydro primitives of the
+// fixed zones change).
 // ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void zone_of(const GV& g, long n, int& i, int& j, int& k) {
+  k = (int)(n / g.s3) - KH_NGH;
+  long r = n % g.s3;
+  j = (int)(r / g.s2) - KH_NGH;
+  i = (int)(r % g.s2) - KH_NGH;
+}
+
+// One warp per failed zone: lane l < 26 owns one neighbour (independent loads in flight), butterfly sums.
 __global__ void __launch_bounds__(128)
-fixup_gather_kernel(GV g, const double* __restrict__ Pf, const unsigned char* __restrict__ pflag, double* __restrict__ fix,
-                    const StepScalars* __restrict__ sc, int force) {
-  if (!force && sc->n_pflag == 0) return;
-  int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
-  if (i >= g.n1) return;
-  const long n = zidx(g, i, j, k), nt = g.ntot;
-  if (pflag[n] == 0) return;
-  double sum[5] = {0, 0, 0, 0, 0}, wsum = 0.0, sall[5] = {0, 0, 0, 0, 0}, wall = 0.0;
-  for (int dk = -1; dk <= 1; dk++)
-    for (int dj = -1; dj <= 1; dj++)
-      for (int di = -1; di <= 1; di++) {
-        if (di == 0 && dj == 0 && dk == 0) continue;
-        long m = n + dk * g.s3 + dj * g.s2 + di;
-        double w = 1.0 / (double)(abs(di) + abs(dj) + abs(dk) + 1);
-        bool good = pflag[m] == 0;
-        for (int v = 0; v < 5; v++) {
-          double val = Pf[v * nt + m];
-          sall[v] += w * val;
-          if (good) sum[v] += w * val;
-        }
-        wall += w;
-        if (good) wsum += w;
+fixup_gather_kernel(GV g, const double* __restrict__ Pf, const unsigned char* __restrict__ pflag, const unsigned* __restrict__ list,
+                    double* __restrict__ fix, const StepScalars* __restrict__ sc) {
+  const long count = (long)sc->n_pflag, nt = g.ntot;
+  const int lane = threadIdx.x & 31;
+  const long warp = ((long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = ((long)gridDim.x * blockDim.x) >> 5;
+  // lane -> neighbour offset (skipping the centre, index 13 of the 3x3x3 box)
+  const int c = lane < 13 ? lane : lane + 1;
+  const int di = c % 3 - 1, dj = (c / 3) % 3 - 1, dk = c / 9 - 1;
+  const bool nb = lane < 26;
+  const double w = nb ? 1.0 / (double)(abs(di) + abs(dj) + abs(dk) + 1) : 0.0;
+  for (long q = warp; q < count; q += nwarp) {
+    const long n = list[q];
+    const long m = nb ? n + dk * g.s3 + dj * g.s2 + di : n;
+    const double wg = (nb && pflag[m] == 0) ? w : 0.0;
+    double sum[5], sall[5], wsum = wg, wall = w;
+#pragma unroll
+    for (int v = 0; v < 5; v++) { double val = Pf[v * nt + m]; sall[v] = w * val; sum[v] = wg * val; }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      wsum += __shfl_xor_sync(0xffffffffu, wsum, o);
+      wall += __shfl_xor_sync(0xffffffffu, wall, o);
+#pragma unroll
+      for (int v = 0; v < 5; v++) {
+        sum[v] += __shfl_xor_sync(0xffffffffu, sum[v], o);
+        sall[v] += __shfl_xor_sync(0xffffffffu, sall[v], o);
       }
-  for (int v = 0; v < 5; v++) fix[v * nt + n] = (wsum > 0.0) ? sum[v] / wsum : sall[v] / wall;
+    }
+    if (lane == 0) {
+#pragma unroll
+      for (int v = 0; v < 5; v++) fix[v * count + q] = (wsum > 0.0) ? sum[v] / wsum : sall[v] / wall;
+    }
+  }
+}
+
+// ghost images of interior index s along one direction: writes up to 2*NG indices into img[], returns how many
+__device__ __forceinline__ int ghost_images(int s, int N, int bc_lo, int bc_hi, int img[2 * KH_NGH]) {
+  int cnt = 0;
+  for (int m = 0; m < 2 * KH_NGH; m++) {
+    int gi = m < KH_NGH ? m - KH_NGH : N + m - KH_NGH, kind;
+    if (ghost_map(gi, N, bc_lo, bc_hi, kind) == s && kind != KH_MAP_ID) img[cnt++] = gi;
+  }
+  return cnt;
 }
 
 template <bool FLAT>
 __global__ void __launch_bounds__(128)
-fixup_apply_kernel(GV g, double* __restrict__ Pf, const unsigned char* __restrict__ pflag, unsigned char* __restrict__ fflag,
-                   const double* __restrict__ fix, const StepScalars* __restrict__ sc, int force) {
-  if (!force && sc->n_pflag == 0) return;
+fixup_apply_kernel(GV g, double* __restrict__ Pf, const unsigned* __restrict__ list, unsigned char* __restrict__ fflag,
+                   const double* __restrict__ fix, const StepScalars* __restrict__ sc) {
+  const long count = (long)sc->n_pflag, nt = g.ntot;
+  for (long q = (long)blockIdx.x * blockDim.x + threadIdx.x; q < count; q += (long)gridDim.x * blockDim.x) {
+    const long n = list[q];
+    int i, j, k;
+    zone_of(g, n, i, j, k);
+    const long p2 = pidx(g, i, j);
+    double P[KH_NP];
+#pragma unroll
+    for (int v = 0; v < 5; v++) P[v] = fix[v * count + q];
+#pragma unroll
+    for (int v = 5; v < KH_NP; v++) P[v] = Pf[v * nt + n];
+    Geo G;
+    load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, p2);
+    double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2);
+    double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
+    int ff = apply_floors<FLAT>(G, g.fp, rho_g, u_g, P);
+    fflag[n] |= (unsigned char)ff;
+    // the zone and its ghost images (S20: copies; polar images flip ut^2)
+    int i1[2 * KH_NGH + 1], i2[2 * KH_NGH + 1], i3[2 * KH_NGH + 1];
+    int c1 = ghost_images(i, g.n1, g.bc[0], g.bc[1], i1), c2 = ghost_images(j, g.n2, g.bc[2], g.bc[3], i2),
+        c3 = ghost_images(k, g.n3, g.bc[4], g.bc[5], i3);
+    i1[c1++] = i; i2[c2++] = j; i3[c3++] = k;
+    for (int z = 0; z < c3; z++)
+      for (int y = 0; y < c2; y++) {
+        int kind;
+        ghost_map(i2[y], g.n2, g.bc[2], g.bc[3], kind);
+        const double sgn = (kind == KH_MAP_POLAR) ? -1.0 : 1.0;
+        for (int x = 0; x < c1; x++) {
+          const long m = zidx(g, i1[x], i2[y], i3[z]);
+#pragma unroll
+          for (int v = 0; v < 5; v++) Pf[v * nt + m] = (v == U2) ? sgn * P[v] : P[v];
+        }
+      }
+  }
+}
+
+// debug hook support: failure list from a caller-supplied flag array (interior zones, any order)
+__global__ void build_faillist_kernel(GV g, const unsigned char* __restrict__ pflag, unsigned* __restrict__ list, StepScalars* __restrict__ sc) {
   int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
   if (i >= g.n1) return;
-  const long n = zidx(g, i, j, k), nt = g.ntot, p2 = pidx(g, i, j);
-  if (pflag[n] == 0) return;
-  double P[KH_NP];
-#pragma unroll
-  for (int v = 0; v < 5; v++) P[v] = fix[v * nt + n];
-#pragma unroll
-  for (int v = 5; v < KH_NP; v++) P[v] = Pf[v * nt + n];
-  Geo G;
-  load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, p2);
-  double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2);
-  double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
-  int ff = apply_floors<FLAT>(G, g.fp, rho_g, u_g, P);
-#pragma unroll
-  for (int v = 0; v < 5; v++) Pf[v * nt + n] = P[v];
-  fflag[n] |= (unsigned char)ff;
+  const long n = zidx(g, i, j, k);
+  if (pflag[n] != 0) list[atomicAdd(&sc->n_pflag, 1ULL)] = (unsigned)n;
 }
 
 // ---------------------------------------------------------------------------------------------

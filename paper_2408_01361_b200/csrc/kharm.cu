@@ -39,6 +39,7 @@ struct kh_grid {
   double* ctop[3];
   double* emf[3];
   unsigned char *pflag, *fflag;
+  unsigned* faillist;    // zones (device-layout index) whose inversion failed in the current sub-step
   double* fix;           // [5][ntot] scratch of the fix-up (pre-fix-up snapshot semantics)
   double* stage;         // lazily allocated [8][ntot] staging buffer for host transfers / debug copies
   StepScalars* sc;       // device
@@ -88,15 +89,13 @@ static inline void prof_end(kh_grid* g) {
 
 static inline dim3 zone_grid(int nx, int ny, int nz) { return dim3((nx + 127) / 128, ny, nz); }
 
-static int fill_ghosts(kh_grid* g, double* P, unsigned char* flag, int only_if_failed) {
+static int fill_ghosts(kh_grid* g, double* P, unsigned char* flag) {
   const GV& v = g->gv;
-  long t0 = (long)2 * KH_NGH * v.nt2 * v.nt3, t1 = (long)2 * KH_NGH * v.nt1 * v.nt3, t2 = (long)2 * KH_NGH * v.nt1 * v.nt2;
+  const long shell = (long)v.nt1 * v.nt2 * (2 * KH_NGH) + (long)v.nt1 * (2 * KH_NGH) * v.n3 + (long)(2 * KH_NGH) * v.n2 * v.n3;
   prof_begin(g, KH_K_FILL);
-  fill_kernel<0><<<(unsigned)((t0 + 127) / 128), 128, 0, g->stream>>>(v, P, flag, g->sc, only_if_failed);
-  fill_kernel<1><<<(unsigned)((t1 + 127) / 128), 128, 0, g->stream>>>(v, P, flag, g->sc, only_if_failed);
-  fill_kernel<2><<<(unsigned)((t2 + 127) / 128), 128, 0, g->stream>>>(v, P, flag, g->sc, only_if_failed);
+  fill_kernel<<<(unsigned)((shell + 127) / 128), 128, 0, g->stream>>>(v, P, flag);
   prof_end(g);
-  g->launches += 3;
+  g->launches += 1;
   CK(cudaGetLastError());
   return KH_OK;
 }
@@ -152,14 +151,13 @@ static void launch_flux(kh_grid* g, const double* Ps) {
   g->launches++;
 }
 
-static int do_fixup(kh_grid* g, double* Pf, int force) {
+// Fix-up of the zones on the failure list (+ floors, + their ghost images).
+static int do_fixup(kh_grid* g, double* Pf) {
   const GV& v = g->gv;
-  dim3 grid = zone_grid(v.n1, v.n2, v.n3);
-  double* fix = g->fix;
   prof_begin(g, KH_K_FIXUP);
-  fixup_gather_kernel<<<grid, 128, 0, g->stream>>>(v, Pf, g->pflag, fix, g->sc, force);
-  if (g->flat) fixup_apply_kernel<true><<<grid, 128, 0, g->stream>>>(v, Pf, g->pflag, g->fflag, fix, g->sc, force);
-  else fixup_apply_kernel<false><<<grid, 128, 0, g->stream>>>(v, Pf, g->pflag, g->fflag, fix, g->sc, force);
+  fixup_gather_kernel<<<64, 128, 0, g->stream>>>(v, Pf, g->pflag, g->faillist, g->fix, g->sc);
+  if (g->flat) fixup_apply_kernel<true><<<64, 128, 0, g->stream>>>(v, Pf, g->faillist, g->fflag, g->fix, g->sc);
+  else fixup_apply_kernel<false><<<64, 128, 0, g->stream>>>(v, Pf, g->faillist, g->fflag, g->fix, g->sc);
   prof_end(g);
   g->launches += 2;
   CK(cudaGetLastError());
@@ -181,7 +179,7 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
   const unsigned grid = (unsigned)(((long)v.n1 * v.n2 * v.n3 + 127) / 128);
 #define UPD(FL, CO)                                                                                                  \
   update_kernel<FL, CO><<<grid, 128, 0, g->stream>>>(v, Pi, Ps, Pf, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], \
-                                                     g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, g->fflag, g->sc, dt_factor)
+                                                     g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, g->fflag, g->faillist, g->sc, dt_factor)
   prof_begin(g, KH_K_UPDATE);
   if (g->flat) { if (corrector) UPD(true, true); else UPD(true, false); }
   else { if (corrector) UPD(false, true); else UPD(false, false); }
@@ -189,11 +187,9 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
 #undef UPD
   g->launches++;
   CK(cudaGetLastError());
-  int rc = fill_ghosts(g, Pf, g->pflag, 0);
+  int rc = fill_ghosts(g, Pf, g->pflag);
   if (rc) return rc;
-  rc = do_fixup(g, Pf, 0);
-  if (rc) return rc;
-  return fill_ghosts(g, Pf, nullptr, 1);
+  return do_fixup(g, Pf);      // also refreshes the ghost images of the fixed zones (the second fill of S22)
 }
 
 static int enqueue_step(kh_grid* g, int cur) {
@@ -240,7 +236,7 @@ int kh_grid_destroy(kh_grid* g) {
   for (int l = 0; l < 4; l++) cudaFree(g->geom[l]);
   cudaFree(g->conn); cudaFree(g->dg); cudaFree(g->floorp);
   for (int b = 0; b < 3; b++) { cudaFree(g->P[b]); cudaFree(g->F[b]); cudaFree(g->ctop[b]); cudaFree(g->emf[b]); }
-  cudaFree(g->pflag); cudaFree(g->fflag); cudaFree(g->sc); cudaFree(g->fix); cudaFree(g->stage);
+  cudaFree(g->pflag); cudaFree(g->fflag); cudaFree(g->faillist); cudaFree(g->sc); cudaFree(g->fix); cudaFree(g->stage);
   if (g->sc_host) cudaFreeHost(g->sc_host);
   if (g->pev) { for (int e = 0; e < 2 * KH_PROF_POOL; e++) if (g->pev[e]) cudaEventDestroy(g->pev[e]); delete[] g->pev; }
   delete[] g->pkind;
@@ -325,6 +321,7 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   ALLOC(g->fix, 5 * fb);
   ALLOC(g->pflag, v.ntot);
   ALLOC(g->fflag, v.ntot);
+  ALLOC(g->faillist, sizeof(unsigned) * (size_t)v.n1 * v.n2 * v.n3);
   ALLOC(g->sc, sizeof(StepScalars));
 #undef ALLOC
   if (cudaMallocHost((void**)&g->sc_host, sizeof(StepScalars)) != cudaSuccess) { kh_grid_destroy(g); return KH_ENOMEM; }
@@ -381,7 +378,7 @@ int kh_set_prims(kh_grid* g, const double* p, int with_ghosts, int mem) {
     g->launches++;
     CK(cudaGetLastError());
   }
-  rc = fill_ghosts(g, Pn, nullptr, 0);
+  rc = fill_ghosts(g, Pn, nullptr);
   if (rc) return rc;
   if (mem == KH_MEM_HOST) CK(cudaStreamSynchronize(g->stream));
   return KH_OK;
@@ -603,7 +600,10 @@ int kh_debug_fixup(kh_grid* g, const int* pflag_with_ghosts, int mem) {
   int_to_flags_kernel<<<(unsigned)((v.ntot + 127) / 128), 128, 0, g->stream>>>(v.ntot, src, g->pflag);
   g->launches++;
   CK(cudaMemsetAsync(g->fflag, 0, v.ntot, g->stream));
-  int rc = do_fixup(g, g->P[g->cur], 1);
+  reset_counters_kernel<<<1, 1, 0, g->stream>>>(g->sc);
+  build_faillist_kernel<<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, g->pflag, g->faillist, g->sc);
+  g->launches += 2;
+  int rc = do_fixup(g, g->P[g->cur]);
   if (rc) return rc;
   CK(cudaStreamSynchronize(g->stream));
   return KH_OK;

@@ -175,6 +175,11 @@ def test_fixup_hook_parity(kh, kho):
     a, b = gg.get_prims(), go.get_prims()
     assert np.abs(a - b).max() <= 1e-13 * np.abs(b).max() and np.allclose(a, b, rtol=1e-12, atol=1e-300)
     assert np.array_equal(gg.get_flags()[1], go.get_flags()[1])
+    # the CUDA fix-up also refreshes the ghost images of the zones it fixed (the second fill of the sub-step, S22);
+    # the oracle's hook stops before that fill, so run it to bring both sides to the same point of the sequence
+    go.fill_ghosts()
+    assert np.array_equal(gg.get_prims(with_ghosts=True)[:5], go.get_prims(with_ghosts=True)[:5]) or \
+        np.allclose(gg.get_prims(with_ghosts=True)[:5], go.get_prims(with_ghosts=True)[:5], rtol=1e-12, atol=1e-300)
     allbad = np.ones_like(pf)
     gg.debug_fixup(allbad); go.debug_fixup(allbad)
     assert np.allclose(gg.get_prims(), go.get_prims(), rtol=1e-12, atol=1e-300)
