@@ -124,30 +124,99 @@ flux_x1_kernel(GV g, const double* __restrict__ P, double* __restrict__ F, doubl
 }
 
 // x2 / x3: thread <-> (i, transverse index), marching over faces [f0, f1) of chunk blockIdx.y.
+// The stencil rows are staged through a PRIVATE ring in shared memory filled by cp.async (LDGSTS): each thread
+// copies only the column it will read itself, so no barrier is needed -- shared memory acts as an asynchronous
+// prefetch buffer that costs no registers.  The row needed by the NEXT face is in flight while this face's ~1200
+// instructions run, so the HBM / L2 latency of the primitives never stalls the fp64 pipe.
+// Ring: R = 2H + 2 rows (H = stencil half width) x 8 variables x 128 threads, [row][var][thread] (conflict free).
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gmem_src) {
+  unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
+template <int RECON>
+struct MarchRing {
+  static constexpr int H = (RECON == 1) ? 2 : 1;
+  static constexpr int R = 2 * H + 2;
+  static constexpr int ROW = KH_NP * 128;            // doubles per ring row
+  static constexpr int BYTES = R * ROW * 8;
+};
+
+// zone-centred reconstruction of variable v from the ring rows starting at slot s0 (rows z-H .. z+H)
+template <int RECON>
+__device__ __forceinline__ void recon_ring(const double* __restrict__ col, int s0, double& qm, double& qp) {
+  constexpr int R = MarchRing<RECON>::R, ROW = MarchRing<RECON>::ROW;
+  int s1 = s0 + 1; if (s1 >= R) s1 -= R;
+  int s2 = s1 + 1; if (s2 >= R) s2 -= R;
+  if (RECON == 0) {
+    mc_zone(col[s0 * ROW], col[s1 * ROW], col[s2 * ROW], qm, qp);
+  } else {
+    int s3 = s2 + 1; if (s3 >= R) s3 -= R;
+    int s4 = s3 + 1; if (s4 >= R) s4 -= R;
+    weno5_zone(col[s0 * ROW], col[s1 * ROW], col[s2 * ROW], col[s3 * ROW], col[s4 * ROW], qm, qp);
+  }
+}
+
 template <int DIR, int RECON, bool FLAT>
 __global__ void __launch_bounds__(128, KH_MINB_MARCH)
 flux_march_kernel(GV g, const double* __restrict__ P, double* __restrict__ F, double* __restrict__ ctop, int J) {
+  extern __shared__ double ring[];
+  constexpr int H = MarchRing<RECON>::H, R = MarchRing<RECON>::R;
   const int c1 = g.n1 + 2;
   const int cb = (DIR == 2 ? g.n3 : g.n2) + 2;
   const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= (long)c1 * cb) return;
+  if (t >= (long)c1 * cb) return;                     // no barriers below: early exit is safe
   const int i = (int)(t % c1) - 1, b = (int)(t / c1) - 1;
   const int N = (DIR == 2) ? g.n2 : g.n3;
   const int f0 = blockIdx.y * J;
   const int f1 = (f0 + J < N + 1) ? f0 + J : N + 1;
   const long st = (DIR == 2) ? g.s2 : g.s3, nt = g.ntot;
-  long n = (DIR == 2) ? zidx(g, i, f0 - 1, b) : zidx(g, i, b, f0 - 1);
+  double* const col = ring + threadIdx.x;             // this thread's column: col[(slot * 8 + v) * 128]
+  // rows are addressed by the zone index along DIR; the first zone reconstructed is f0 - 1 (for the left state of face f0)
+  const double* src = P + ((DIR == 2) ? zidx(g, i, f0 - 1 - H, b) : zidx(g, i, b, f0 - 1 - H));   // row f0-1-H, variable 0
+  int wslot = 0;                                      // ring slot the next issued row goes to
+  auto issue_row = [&]() {
+#pragma unroll
+    for (int v = 0; v < KH_NP; v++) cp_async8(col + (wslot * KH_NP + v) * 128, src + v * nt);
+    src += st;
+    if (++wslot == R) wslot = 0;
+  };
+#pragma unroll
+  for (int q = 0; q < 2 * H + 1; q++) issue_row();    // rows of zone f0-1
+  cp_async_commit();
+  issue_row();                                        // the one more row zone f0 needs
+  cp_async_commit();
+  cp_async_wait<1>();
+  int s0 = 0;                                         // slot of row z-H of the zone being reconstructed
   double PL[KH_NP];
 #pragma unroll
   for (int v = 0; v < KH_NP; v++) {
     double qm;
-    recon_zone<RECON>(P + v * nt + n, st, qm, PL[v]);
+    recon_ring<RECON>(col + v * 128, s0, qm, PL[v]);
   }
+  long n = (DIR == 2) ? zidx(g, i, f0 - 1, b) : zidx(g, i, b, f0 - 1);
   for (int f = f0; f < f1; f++) {
     n += st;
+    if (++s0 == R) s0 = 0;
+    if (f + 1 < f1) {                                 // row f+1+H for the next face (never beyond the last ghost row)
+      issue_row();
+      if (DIR == 2 && !FLAT) {                        // and that face's geometry towards L1
+        const double* tb = g.geom[2] + pidx(g, i, f + 1);
+#pragma unroll
+        for (int c = 0; c < KH_NGEO; c++)
+          if (c != G02 && c != G23 && c != 10 + G03 && c != 10 + G11 && c != 10 + G12 && c != 10 + G13 && c != 10 + G23 && c != 10 + G33)
+            prefetch_l1(tb + (long)c * g.n2d);
+      }
+    }
+    cp_async_commit();
+    cp_async_wait<1>();                               // everything but the row just issued has landed
     double PR[KH_NP], PLn[KH_NP];
 #pragma unroll
-    for (int v = 0; v < KH_NP; v++) recon_zone<RECON>(P + v * nt + n, st, PR[v], PLn[v]);
+    for (int v = 0; v < KH_NP; v++) recon_ring<RECON>(col + v * 128, s0, PR[v], PLn[v]);
     if (DIR == 2 && polar_face(g, f)) {   // S7 / S10: nothing crosses the axis
 #pragma unroll
       for (int v = 0; v < KH_NP; v++) F[v * nt + n] = 0.0;

@@ -100,6 +100,18 @@ static int fill_ghosts(kh_grid* g, double* P, unsigned char* flag) {
   return KH_OK;
 }
 
+// The marching kernels stage their stencil rows through a shared-memory ring: ask for the large carve-out so that
+// several blocks stay resident (B200: up to 227 KB of shared memory per SM).
+template <int DIR, int RECON, bool FLAT>
+static void setup_march_one() {
+  cudaFuncSetAttribute(flux_march_kernel<DIR, RECON, FLAT>, cudaFuncAttributeMaxDynamicSharedMemorySize, MarchRing<RECON>::BYTES);
+  cudaFuncSetAttribute(flux_march_kernel<DIR, RECON, FLAT>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+}
+static void setup_march_kernels() {
+  setup_march_one<2, 0, true>(); setup_march_one<2, 1, true>(); setup_march_one<2, 0, false>(); setup_march_one<2, 1, false>();
+  setup_march_one<3, 0, true>(); setup_march_one<3, 1, true>(); setup_march_one<3, 0, false>(); setup_march_one<3, 1, false>();
+}
+
 // Chunk length of the marching kernels: long enough that the one extra reconstruction per chunk is
 // small, short enough that the grid fills the SMs in an almost whole number of waves.
 static int march_chunk(const kh_grid* g, long columns, int faces) {
@@ -139,12 +151,13 @@ static void launch_flux(kh_grid* g, const double* Ps) {
     const int J = march_chunk(g, cols, N + 1);
     dim3 grid((unsigned)((cols + 127) / 128), (unsigned)((N + 1 + J - 1) / J));
     constexpr int D = (DIR == 1) ? 2 : DIR;   // (keeps the DIR == 1 instantiation of this branch well-formed)
+    const size_t sm0 = MarchRing<0>::BYTES, sm1 = MarchRing<1>::BYTES;
     if (g->flat) {
-      if (mc) flux_march_kernel<D, 0, true><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct, J);
-      else flux_march_kernel<D, 1, true><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct, J);
+      if (mc) flux_march_kernel<D, 0, true><<<grid, 128, sm0, g->stream>>>(v, Ps, F, ct, J);
+      else flux_march_kernel<D, 1, true><<<grid, 128, sm1, g->stream>>>(v, Ps, F, ct, J);
     } else {
-      if (mc) flux_march_kernel<D, 0, false><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct, J);
-      else flux_march_kernel<D, 1, false><<<grid, 128, 0, g->stream>>>(v, Ps, F, ct, J);
+      if (mc) flux_march_kernel<D, 0, false><<<grid, 128, sm0, g->stream>>>(v, Ps, F, ct, J);
+      else flux_march_kernel<D, 1, false><<<grid, 128, sm1, g->stream>>>(v, Ps, F, ct, J);
     }
   }
   prof_end(g);
@@ -280,10 +293,16 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    setup_march_kernels();
     int nb = 0;
-    cudaError_t eo = g->flat ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, flux_march_kernel<2, 1, true>, 128, 0)
-                             : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, flux_march_kernel<2, 1, false>, 128, 0);
-    g->flux_blocks_per_sm = (eo == cudaSuccess && nb > 0) ? nb : 4;
+    const bool w5 = p->recon == KH_RECON_WENO5;
+    const size_t smem = w5 ? MarchRing<1>::BYTES : MarchRing<0>::BYTES;
+    cudaError_t eo;
+    if (g->flat) eo = w5 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, flux_march_kernel<2, 1, true>, 128, smem)
+                         : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, flux_march_kernel<2, 0, true>, 128, smem);
+    else eo = w5 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, flux_march_kernel<2, 1, false>, 128, smem)
+                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, flux_march_kernel<2, 0, false>, 128, smem);
+    g->flux_blocks_per_sm = (eo == cudaSuccess && nb > 0) ? nb : 3;
     if (g->sm_count < 1) g->sm_count = 148;
   }
   g->use_graph = true;
