@@ -82,18 +82,21 @@ __device__ __forceinline__ void face_flux(const GV& g, const double PL[KH_NP], c
   const double gdd = FLAT ? 1.0 : (DIR == 1 ? G.n11 : (DIR == 2 ? G.n22 : G.n33));
   const double k2 = FLAT ? 1.0 : fma(gtd, gtd, -G.n00 * gdd);
   const double gm1 = g.gam - 1.0;
-  double UL[KH_NP], FL[KH_NP], cL;
-  state_terms<DIR, FLAT>(G, ialpha, gtd, gdd, k2, PL, g.gam, gm1, UL, FL, cL);
-  double UR[KH_NP], FR[KH_NP], cR;
-  state_terms<DIR, FLAT>(G, ialpha, gtd, gdd, k2, PR, g.gam, gm1, UR, FR, cR);
+  StateQ SL, SR;
+  double cL, cR;
+  state_terms<DIR, FLAT>(G, ialpha, gtd, gdd, k2, PL, g.gam, gm1, SL, cL);
+  state_terms<DIR, FLAT>(G, ialpha, gtd, gdd, k2, PR, g.gam, gm1, SR, cR);
   // S14: c_top = max(0, v+L, v+R, -v-L, -v-R) = max over the states of max(|v+|, |v-|)
-  const double c = fmax(cL, cR);
+  const double c = (cL > cR) ? cL : cR;
+  double GL[KH_NP], GR[KH_NP];
+  llf_row<DIR>(SL, c, GL);
+  llf_row<DIR>(SR, -c, GR);
   const double hg = FLAT ? 0.5 : 0.5 * G.gdet;
   const long nt = g.ntot;
 #pragma unroll
   for (int v = 0; v < KH_NP; v++) {
     if (v == B1 + DIR - 1) continue;     // F^d[B^d] = 0, never read
-    F[v * nt + n] = hg * fma(-c, UR[v] - UL[v], FL[v] + FR[v]);
+    F[v * nt + n] = hg * (GL[v] + GR[v]);
   }
   ctop[n] = c;
 }
