@@ -72,10 +72,8 @@ __device__ __forceinline__ bool polar_face(const GV& g, int j) {
 // profiles/ shows dram bytes = algorithmic bytes).
 // ---------------------------------------------------------------------------------------------
 template <int DIR, bool FLAT>
-__device__ __forceinline__ void face_flux(const GV& g, const double PL[KH_NP], const double PR[KH_NP], long p2, long n,
-                                          double* __restrict__ F, double* __restrict__ ctop) {
-  Geo G;
-  load_geo<FLAT, DIR, 0>(G, g.geom[DIR], g.n2d, p2);
+__device__ __forceinline__ void face_flux_geo(const GV& g, const Geo& G, const double PL[KH_NP], const double PR[KH_NP], long n,
+                                              double* __restrict__ F, double* __restrict__ ctop) {
   // per-face quantities shared by the two states
   const double ialpha = FLAT ? 1.0 : -G.n00 * G.alpha;                       // 1/alpha = -g^tt alpha
   const double gtd = FLAT ? 0.0 : (DIR == 1 ? G.n01 : (DIR == 2 ? G.n02 : 0.0));
@@ -99,6 +97,13 @@ __device__ __forceinline__ void face_flux(const GV& g, const double PL[KH_NP], c
     F[v * nt + n] = hg * (GL[v] + GR[v]);
   }
   ctop[n] = c;
+}
+template <int DIR, bool FLAT>
+__device__ __forceinline__ void face_flux(const GV& g, const double PL[KH_NP], const double PR[KH_NP], long p2, long n,
+                                          double* __restrict__ F, double* __restrict__ ctop) {
+  Geo G;
+  load_geo<FLAT, DIR, 0>(G, g.geom[DIR], g.n2d, p2);
+  face_flux_geo<DIR, FLAT>(g, G, PL, PR, n, F, ctop);
 }
 
 template <int RECON, bool FLAT>
@@ -202,6 +207,8 @@ flux_march_kernel(GV g, const double* __restrict__ P, double* __restrict__ F, do
     recon_ring<RECON>(col + v * 128, s0, qm, PL[v]);
   }
   long n = (DIR == 2) ? zidx(g, i, f0 - 1, b) : zidx(g, i, b, f0 - 1);
+  Geo G3;                                             // x3 faces: the metric does not depend on x3 -- one load per thread
+  if (DIR == 3) load_geo<FLAT, 3, 0>(G3, g.geom[3], g.n2d, pidx(g, i, b));
   for (int f = f0; f < f1; f++) {
     n += st;
     if (++s0 == R) s0 = 0;
@@ -225,7 +232,8 @@ flux_march_kernel(GV g, const double* __restrict__ P, double* __restrict__ F, do
       for (int v = 0; v < KH_NP; v++) F[v * nt + n] = 0.0;
       ctop[n] = 0.0;
     } else {
-      face_flux<DIR, FLAT>(g, PL, PR, (DIR == 2) ? pidx(g, i, f) : pidx(g, i, b), n, F, ctop);
+      if (DIR == 3) face_flux_geo<3, FLAT>(g, G3, PL, PR, n, F, ctop);
+      else face_flux<DIR, FLAT>(g, PL, PR, (DIR == 2) ? pidx(g, i, f) : pidx(g, i, b), n, F, ctop);
     }
 #pragma unroll
     for (int v = 0; v < KH_NP; v++) PL[v] = PLn[v];
