@@ -66,6 +66,13 @@ ALG_FLOPS = {
 }
 
 
+# DRAM traffic per launch (bytes) of the default workload's kernels: dram__bytes_read.sum + dram__bytes_write.sum of one
+# `ncu --set full` capture (update = mean of the predictor and the corrector launch).  Source file in profiles/.
+NCU_DRAM_SOURCE = "profiles/r01c_ncu_full.md"
+NCU_DRAM_BYTES_PER_LAUNCH = {"flux1": 394.8e6, "flux2": 401.8e6, "flux3": 402.6e6, "emf": 213.8e6,
+                             "update": 0.5 * (990.2e6 + 199.4e6 + 697.4e6 + 196.2e6)}
+
+
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -219,17 +226,60 @@ def kernel_table(prof, steps, zones, recon, flat, hbm_peak, fp64_peak_tf):
     return rows
 
 
+class Ranks:
+    """Replica plumbing of `--gpus N` (independent replicas, no data-path collective):
+    RANK / LOCAL_RANK / WORLD_SIZE from the launcher's environment, a barrier and the max-over-ranks of a scalar.
+    backend "nccl" on the GPU box; tests drive the same code with "gloo" on CPU (tests/test_bench_ranks.py)."""
+
+    def __init__(self, backend="nccl"):
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        self.backend = backend
+        self.dist = None
+        if self.world > 1:
+            import torch
+            import torch.distributed as dist
+            if backend == "nccl":
+                dist.init_process_group("nccl", device_id=torch.device("cuda", self.local))
+            else:
+                dist.init_process_group(backend)
+            self.dist = dist
+
+    def _device(self):
+        return "cuda" if self.backend == "nccl" else "cpu"
+
+    def barrier(self):
+        if self.dist is not None:
+            self.dist.barrier()
+        if self.backend == "nccl":
+            import torch
+            torch.cuda.synchronize()
+
+    def max(self, x):
+        if self.dist is None:
+            return float(x)
+        import torch
+        t = torch.tensor([x], dtype=torch.float64, device=self._device())
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def whole_job_rate(self, units_per_rank, seconds_local):
+        """Units all ranks processed / the slowest rank's time (every rank holds the same number of units)."""
+        return self.world * units_per_rank / self.max(seconds_local)
+
+    def close(self):
+        if self.dist is not None:
+            self.dist.destroy_process_group()
+            self.dist = None
+
+
 def run_ours(args):
     import torch
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    R = Ranks("nccl")              # world 1: no process group
+    rank, world, local = R.rank, R.world, R.local
     import paper_2408_01361_b200 as kh
 
     cfg, p = workload_params(args.workload)
@@ -238,18 +288,7 @@ def run_ours(args):
     P0 = workload_state(args.workload, p, seed=1 + rank)          # every replica its own seeded block
     stream = torch.cuda.Stream()
     K, W = args.steps, max(args.warmup, 3)
-
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def max_over_ranks(x):
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    barrier, max_over_ranks = R.barrier, R.max
 
     with torch.cuda.stream(stream):
         g = kh.Grid(p, stream=stream.cuda_stream)
@@ -303,6 +342,7 @@ def run_ours(args):
         e2e_s = max_over_ranks(time.perf_counter() - t0)
         state_bytes = 8 * 8 * zones
     if rank != 0:
+        R.close()
         return 0
 
     hbm_peak, hbm_src, peaks = load_peaks()
@@ -320,7 +360,10 @@ def run_ours(args):
     else:
         roof = {"kernel": dom, "bound": "hbm", "achieved": d.get("gbs"), "peak": hbm_peak, "unit": "GB/s",
                 "frac": d.get("frac_hbm"), "peak_source": hbm_src}
-    roof["traffic"] = None      # dram bytes per launch from ncu --set full: see profiles/ (not measurable in-process)
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch of that kernel from the committed ncu --set full capture
+    # (not measurable in-process); only the default workload has one
+    roof["traffic"] = NCU_DRAM_BYTES_PER_LAUNCH.get(dom) if args.workload == DEFAULT_WORKLOAD else None
+    roof["traffic_source"] = NCU_DRAM_SOURCE if roof["traffic"] else None
     roof["ms_per_launch"] = d.get("ms_per_launch")
     prof_ms_step = sum(v["ms_per_step"] for v in kern.values())
     step_gbs = ALG_BYTES_PER_ZONE_STEP * zones / (ms_step * 1e-3) / 1e9
@@ -358,8 +401,7 @@ def run_ours(args):
         "paper_context": "KHARMA: ~21 M ZCPS/V100, ~35 M ZCPS/A100, ~25 M ZCPS/MI250X card (PAPER.md lines 429-433)",
     }
     print(json.dumps(line))
-    if dist is not None:
-        dist.destroy_process_group()
+    R.close()
     return 0
 
 
