@@ -483,6 +483,140 @@ int u2p(const Geom& G, const double U[NP], const double Pg[NP], double gam, doub
 }
 
 // ---------------------------------------------------------------------------------------------
+// C7b. U -> P by the bracketed root find of Kastaun, Kalinani & Ciolfi ("the inverter
+// described in [25] ... greatly improves stability"; reading S24 in DESIGN.md).  Written in the
+// paper's notation.  Inputs seen by the normal observer (same as in u2p above): D, tau = E - D, S_i, B^i;
+//   q = tau/D,  r_i = S_i/D,  b^i = B^i/sqrt(D),  h0 = 1 (ideal gas, eps >= 0),  v0^2 = r^2/(h0^2 + r^2);
+// functions of the unknown mu = 1/(W h):
+//   x = 1/(1 + mu b^2),  rbar^2 = r^2 x^2 + mu x (1 + x) (r.b)^2,  qbar = q - b^2/2 - mu^2 x^2 (b^2 r_perp^2)/2,
+//   b^2 r_perp^2 = b^2 r^2 - (r.b)^2;
+// master function: vhat^2 = min(mu^2 rbar^2, v0^2), What = (1 - vhat^2)^(-1/2), rhohat = D/What,
+//   epshat = What (qbar - mu rbar^2) + vhat^2 What^2/(1 + What), clamped to eps >= 0 inside f only,
+//   ahat = p(rhohat, epshat)/(rhohat (1 + epshat)),  nuA = (1 + ahat)(1 + epshat)/What,
+//   nuB = (1 + ahat)(1 + qbar - mu rbar^2),  f(mu) = mu - 1/(max(nuA, nuB) + rbar^2 mu);
+// bracket (0, mu+], mu+ = 1/h0 if r < h0, else the root of fa(mu) = mu sqrt(h0^2 + rbar^2(mu)) - 1 in (0, 1/h0];
+// velocity v^i = mu x (r^i + mu (r.b) b^i), ut^i = What v^i.
+// Root finder (the paper uses a library bracketing method; S24): Illinois regula falsi on the bracket, stop when the
+// bracket is narrower than 4e-16 of its upper end or f vanishes, at most 100 evaluations (flag 2 otherwise).
+// Flags as for u2p: 1 bad input, 2 not converged, 3 speed limit v0 acted at the root, 5 eps < 0 at the root (the
+// hydro primitives keep the guess), 7 non-finite result.
+// ---------------------------------------------------------------------------------------------
+struct KastaunCtx {
+  double D, q, rsq, bsq, rbsq, brperp, v0sq, gam;
+};
+void kastaun_aux(const KastaunCtx& c, double mu, double& x, double& rbarsq, double& qbar) {
+  x = 1.0 / (1.0 + mu * c.bsq);
+  rbarsq = c.rsq * x * x + mu * x * (1.0 + x) * c.rbsq;
+  qbar = c.q - 0.5 * c.bsq - 0.5 * mu * mu * x * x * c.brperp;
+}
+// the master function; also returns the (unclamped) pieces evaluated at mu
+double kastaun_f(const KastaunCtx& c, double mu, double& vsq_raw, double& W, double& eps_raw) {
+  double x, rbarsq, qbar;
+  kastaun_aux(c, mu, x, rbarsq, qbar);
+  vsq_raw = mu * mu * rbarsq;
+  double vsq = vsq_raw < c.v0sq ? vsq_raw : c.v0sq;
+  W = 1.0 / std::sqrt(1.0 - vsq);
+  eps_raw = W * (qbar - mu * rbarsq) + vsq * W * W / (1.0 + W);
+  double eps = eps_raw > 0.0 ? eps_raw : 0.0;
+  double a = (c.gam - 1.0) * eps / (1.0 + eps);          // p/(rho (1 + eps)), p = (Gamma - 1) rho eps
+  double nuA = (1.0 + a) * (1.0 + eps) / W;
+  double nuB = (1.0 + a) * (1.0 + qbar - mu * rbarsq);
+  double nu = nuA > nuB ? nuA : nuB;
+  return mu - 1.0 / (nu + rbarsq * mu);
+}
+double kastaun_fa(const KastaunCtx& c, double mu) {
+  double x, rbarsq, qbar;
+  kastaun_aux(c, mu, x, rbarsq, qbar);
+  return mu * std::sqrt(1.0 + rbarsq) - 1.0;              // h0 = 1
+}
+// Illinois regula falsi on [a, b] with fn(a) < 0 <= fn(b).  Returns false if 100 evaluations do not converge.
+template <class Fn>
+bool illinois(Fn fn, double a, double fa, double b, double fb, double& lo, double& hi) {
+  int side = 0;
+  for (int it = 0; it < 100; it++) {
+    if (!(b - a > 4e-16 * b)) { lo = a; hi = b; return true; }
+    double m = b - fb * (b - a) / (fb - fa);
+    if (!(m > a && m < b)) m = 0.5 * (a + b);
+    double fm = fn(m);
+    if (fm == 0.0) { lo = hi = m; return true; }
+    if (fm > 0.0) { b = m; fb = fm; if (side == 1) fa *= 0.5; side = 1; }
+    else if (fm < 0.0) { a = m; fa = fm; if (side == -1) fb *= 0.5; side = -1; }
+    else return false;                                      // NaN
+  }
+  return false;
+}
+
+int u2p_kastaun(const Geom& G, const double U[NP], const double Pg[NP], double gam, double Pout[NP]) {
+  for (int v = 0; v < NP; v++) Pout[v] = Pg[v];
+  for (int i = 0; i < 3; i++) Pout[B1 + i] = U[B1 + i] / G.gdet;
+  bool finite = true;
+  for (int v = 0; v < NP; v++) if (!std::isfinite(U[v])) finite = false;
+  if (!finite || !(U[RHO] > 0.0)) return 1;
+
+  // normal-observer quantities, as in u2p
+  double alpha = G.alpha, k = alpha / G.gdet;
+  double D = k * U[RHO];
+  double Bc[4] = {0.0, k * U[B1], k * U[B2], k * U[B3]};
+  double Qcov[4] = {k * (U[UU] - U[RHO]), k * U[U1], k * U[U2], k * U[U3]};
+  double Qcon[4];
+  for (int m = 0; m < 4; m++) { double s = 0.0; for (int n = 0; n < 4; n++) s += G.gcon[m][n] * Qcov[n]; Qcon[m] = s; }
+  double Qdotn = -alpha * Qcon[0];
+  double tau = -Qdotn - D;
+  double Scon[4];                                          // S^i = gamma^{ij} S_j: projection of Q^mu normal to n
+  for (int m = 0; m < 4; m++) Scon[m] = Qcon[m] + Qdotn * (-alpha * G.gcon[m][0]);
+  double Ssq = 0.0, Bsq = 0.0;
+  for (int i = 1; i < 4; i++) for (int j = 1; j < 4; j++) { Ssq += G.gcov[i][j] * Scon[i] * Scon[j]; Bsq += G.gcov[i][j] * Bc[i] * Bc[j]; }
+  double SdotB = Qcov[1] * Bc[1] + Qcov[2] * Bc[2] + Qcov[3] * Bc[3];
+
+  KastaunCtx c;
+  c.gam = gam; c.D = D;
+  c.q = tau / D;
+  c.rsq = Ssq / (D * D);
+  c.bsq = Bsq / D;
+  c.rbsq = SdotB * SdotB / (D * D * D);
+  c.brperp = c.bsq * c.rsq - c.rbsq;
+  if (c.brperp < 0.0) c.brperp = 0.0;                      // Cauchy-Schwarz up to rounding
+  c.v0sq = c.rsq / (1.0 + c.rsq);
+
+  double mu_hi = 1.0;                                      // 1/h0
+  if (!(c.rsq < 1.0)) {
+    double fa1 = kastaun_fa(c, 1.0);
+    if (fa1 > 0.0) {
+      double lo, hi;
+      if (!illinois([&](double m) { return kastaun_fa(c, m); }, 0.0, -1.0, 1.0, fa1, lo, hi)) return 2;
+      mu_hi = hi;
+    }
+  }
+  double vr, W, er;
+  double f0 = kastaun_f(c, 0.0, vr, W, er);
+  double f1 = kastaun_f(c, mu_hi, vr, W, er);
+  double mu;
+  if (!(f0 < 0.0) || !std::isfinite(f1)) return 2;
+  if (f1 <= 0.0) mu = mu_hi;                               // root at the upper end (to rounding)
+  else {
+    double lo, hi;
+    if (!illinois([&](double m) { double a_, b_, c_; return kastaun_f(c, m, a_, b_, c_); }, 0.0, f0, mu_hi, f1, lo, hi)) return 2;
+    mu = 0.5 * (lo + hi);
+  }
+  double vsq_raw, eps_raw;
+  kastaun_f(c, mu, vsq_raw, W, eps_raw);
+  if (!(vsq_raw <= c.v0sq * (1.0 + 1e-12))) return 3;
+  double x, rbarsq, qbar;
+  kastaun_aux(c, mu, x, rbarsq, qbar);
+  double rho = D / W;
+  double u = rho * eps_raw;
+  double rb = SdotB / (D * std::sqrt(D));                  // r.b
+  double ut[3];
+  for (int i = 1; i < 4; i++) ut[i - 1] = W * mu * x * (Scon[i] / D + mu * rb * Bc[i] / std::sqrt(D));
+  if (!std::isfinite(rho) || !std::isfinite(u) || !std::isfinite(ut[0]) || !std::isfinite(ut[1]) || !std::isfinite(ut[2]))
+    return 7;
+  if (eps_raw < 0.0) return 5;
+  Pout[RHO] = rho; Pout[UU] = u;
+  Pout[U1] = ut[0]; Pout[U2] = ut[1]; Pout[U3] = ut[2];
+  return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
 // C8. Floors and ceilings, fluid frame (S18).  Returns the fflag bits.
 // ---------------------------------------------------------------------------------------------
 int floors(const kho_params& p, const Geom& G, double r, double P[NP]) {
@@ -709,7 +843,7 @@ void substep(kho_grid& g, const double* Pi, const double* Ps, double* Pf, double
       for (int d = 0; d < 3; d++) div += (g.F[d][v * nt + n + st[d]] - g.F[d][v * nt + n]) / g.dx[d];
       Uf[v] = Ui[v] + Dt * (-div + S[v]);
     }
-    int pf_flag = u2p(G, Uf, pi, g.p.gamma, pf);
+    int pf_flag = (g.p.inverter == KHO_INV_KASTAUN) ? u2p_kastaun(G, Uf, pi, g.p.gamma, pf) : u2p(G, Uf, pi, g.p.gamma, pf);
     int ff = 0;
     if (pf_flag == 0) ff = floors(g.p, G, g.sfloor_r[n2], pf);
     g.pflag[n] = pf_flag;
@@ -1023,6 +1157,10 @@ void kho_source(const double gcov[16], const double gcon[16], double gdet, const
 int kho_u2p(const double gcov[16], const double gcon[16], double gdet, const double U[8], const double Pguess[8], double gamma, double Pout[8]) {
   Geom G; make_geom(gcov, gcon, gdet, G);
   return u2p(G, U, Pguess, gamma, Pout);
+}
+int kho_u2p_kastaun(const double gcov[16], const double gcon[16], double gdet, const double U[8], const double Pguess[8], double gamma, double Pout[8]) {
+  Geom G; make_geom(gcov, gcon, gdet, G);
+  return u2p_kastaun(G, U, Pguess, gamma, Pout);
 }
 int kho_floors(const kho_params* p, const double gcov[16], const double gcon[16], double x1, double x2, double P[8]) {
   (void)x2;

@@ -24,6 +24,7 @@ extern "C" {
 enum { KHO_MINKOWSKI = 0, KHO_KS = 1, KHO_FMKS = 2 };
 enum { KHO_BC_PERIODIC = 0, KHO_BC_OUTFLOW = 1, KHO_BC_POLAR = 2, KHO_BC_FIXED = 3 };
 enum { KHO_RECON_MC = 0, KHO_RECON_WENO5 = 1 };
+enum { KHO_INV_1DW = 0, KHO_INV_KASTAUN = 1 };
 enum { KHO_LOC_CENT = 0, KHO_LOC_FACE1 = 1, KHO_LOC_FACE2 = 2, KHO_LOC_FACE3 = 3 };
 
 typedef struct {
@@ -37,6 +38,7 @@ typedef struct {
   int recon;
   double rho_min, u_min, r_char, bsq_over_rho_max, bsq_over_u_max, u_over_rho_max, gamma_max;
   double dt_growth_max;
+  int inverter;                                    /* KHO_INV_1DW | KHO_INV_KASTAUN (NEXT-2) */
 } kho_params;
 
 typedef struct kho_grid kho_grid;
@@ -92,6 +94,9 @@ void kho_source(const double gcov[16], const double gcon[16], double gdet, const
 /* U -> P (1D_W); returns the flag (0 = ok). Pout holds guess hydro prims on failure. */
 int kho_u2p(const double gcov[16], const double gcon[16], double gdet, const double U[8],
             const double Pguess[8], double gamma, double Pout[8]);
+/* U -> P by the bracketed root find of Kastaun et al.; same flag convention */
+int kho_u2p_kastaun(const double gcov[16], const double gcon[16], double gdet, const double U[8],
+                    const double Pguess[8], double gamma, double Pout[8]);
 /* floors at a native point; returns fflag bits */
 int kho_floors(const kho_params* p, const double gcov[16], const double gcon[16], double x1,
                double x2, double P[8]);

@@ -27,7 +27,7 @@ class Params(C.Structure):
         ("gamma", C.c_double), ("cfl", C.c_double), ("recon", C.c_int),
         ("rho_min", C.c_double), ("u_min", C.c_double), ("r_char", C.c_double),
         ("bsq_over_rho_max", C.c_double), ("bsq_over_u_max", C.c_double), ("u_over_rho_max", C.c_double),
-        ("gamma_max", C.c_double), ("dt_growth_max", C.c_double),
+        ("gamma_max", C.c_double), ("dt_growth_max", C.c_double), ("inverter", C.c_int),
     ]
 
 
@@ -150,6 +150,12 @@ def source(gcov, gcon, gdet, cn, P, gamma):
 def u2p(gcov, gcon, gdet, U, Pguess, gamma):
     P = np.zeros(8)
     flag = lib().kho_u2p(_ptr(_a(gcov, 16)), _ptr(_a(gcon, 16)), C.c_double(gdet), _ptr(_a(U, 8)), _ptr(_a(Pguess, 8)), C.c_double(gamma), _ptr(P))
+    return P, flag
+
+
+def u2p_kastaun(gcov, gcon, gdet, U, Pguess, gamma):
+    P = np.zeros(8)
+    flag = lib().kho_u2p_kastaun(_ptr(_a(gcov, 16)), _ptr(_a(gcon, 16)), C.c_double(gdet), _ptr(_a(U, 8)), _ptr(_a(Pguess, 8)), C.c_double(gamma), _ptr(P))
     return P, flag
 
 
