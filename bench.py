@@ -40,6 +40,7 @@ WORKLOADS = {
     "torus_sane_192x128x128_weno5": (3, None, None),
     "torus_mad_288x128x128_mc": (4, None, None),
     "torus_sane_192x128x128_mc": (3, None, 0),
+    "torus_sane_192x128x128_weno5_kastaun": (3, None, None),      # same block, kh_params.inverter = KH_INV_KASTAUN
     "minkowski_128_mc": (5, 128, 0), "minkowski_128_weno5": (5, 128, 1),
     "minkowski_256_mc": (5, 256, 0), "minkowski_256_weno5": (5, 256, 1),
     "minkowski_64_mc": (5, 64, 0), "minkowski_192_mc": (5, 192, 0), "minkowski_320_mc": (5, 320, 0),
@@ -85,7 +86,10 @@ def load_peaks():
 def workload_params(name):
     import kharm_inputs as ki
     cfg, n, recon = WORKLOADS[name]
-    return cfg, ki.config_params(cfg, n=n, recon=recon)
+    p = ki.config_params(cfg, n=n, recon=recon)
+    if name.endswith("_kastaun"):
+        p["inverter"] = ki.params.INV_KASTAUN
+    return cfg, p
 
 
 def workload_state(name, p, seed):

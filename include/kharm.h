@@ -37,6 +37,7 @@ enum { KH_OK = 0, KH_EINVAL = -1, KH_ENOMEM = -2, KH_ECUDA = -3, KH_ENAN = -4 };
 enum { KH_MINKOWSKI = 0, KH_KS = 1, KH_FMKS = 2 };                            /* coords          */
 enum { KH_BC_PERIODIC = 0, KH_BC_OUTFLOW = 1, KH_BC_POLAR = 2, KH_BC_FIXED = 3 };
 enum { KH_RECON_MC = 0, KH_RECON_WENO5 = 1 };
+enum { KH_INV_1DW = 0, KH_INV_KASTAUN = 1 };
 enum { KH_MEM_DEVICE = 0, KH_MEM_HOST = 1 };
 enum { KH_LOC_CENT = 0, KH_LOC_FACE1 = 1, KH_LOC_FACE2 = 2, KH_LOC_FACE3 = 3 };
 
@@ -52,6 +53,8 @@ typedef struct {
   int recon;                  /* KH_RECON_MC | KH_RECON_WENO5                                              */
   double rho_min, u_min, r_char, bsq_over_rho_max, bsq_over_u_max, u_over_rho_max, gamma_max; /* floors */
   double dt_growth_max;       /* dt_next <= dt_growth_max * dt                                              */
+  int inverter;               /* KH_INV_1DW (the 1D_W Newton iteration) | KH_INV_KASTAUN (the
+                                 bracketed root find of Kastaun et al.; same pflag codes, no guess needed)   */
 } kh_params;
 
 typedef struct kh_grid kh_grid;   /* opaque */

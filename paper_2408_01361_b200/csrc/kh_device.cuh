@@ -474,4 +474,143 @@ __device__ __forceinline__ int u_to_p_floors(const Geo& G, const double Uh[KH_NP
   return 0;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Second inverter (reading S24): the bracketed root find of Kastaun, Kalinani &
+// Ciolfi in the unknown mu = 1/(W h), fused with the floors like the 1D_W path and behind the same flags.
+// With D, tau, S_i, B^i of the normal observer:  q = tau/D, r^2 = S^2/D^2, b^2 = B^2/D, (r.b)^2 = (S.B)^2/D^3,
+//   x = 1/(1 + mu b^2),  rbar^2 = x (r^2 x + mu (1 + x)(r.b)^2),  qbar = q - b^2/2 - mu^2 x^2 (b^2 r^2 - (r.b)^2)/2,
+//   f(mu) = mu - 1/(nu + rbar^2 mu),  nu = max((1 + Gamma eps)/W, (1 + a)(1 + qbar - mu rbar^2)),  a = (Gamma-1) eps/(1+eps),
+//   v^2 = min(mu^2 rbar^2, v0^2), W = (1 - v^2)^(-1/2), eps = W (qbar - mu rbar^2) + v^2 W^2/(1 + W) (clamped at 0 in f),
+// bracket (0, mu+], mu+ = 1 or the root of mu sqrt(1 + rbar^2) - 1; Illinois regula falsi to a bracket of 4e-16.
+// ---------------------------------------------------------------------------------------------
+struct KastaunC {
+  double q, rsq, bsq, rbsq, brperp, v0sq, gam;
+};
+__device__ __forceinline__ void kastaun_aux(const KastaunC& c, double mu, double& x, double& rbarsq, double& qbar) {
+  x = fast_rcp(fma(mu, c.bsq, 1.0));
+  rbarsq = x * fma(c.rsq, x, mu * ((1.0 + x) * c.rbsq));
+  const double mx = mu * x;
+  qbar = fma(-0.5 * (mx * mx), c.brperp, fma(-0.5, c.bsq, c.q));
+}
+__device__ __forceinline__ double kastaun_f(const KastaunC& c, double mu, double& vsq_raw, double& W, double& eps_raw, double& omv) {
+  double x, rbarsq, qbar;
+  kastaun_aux(c, mu, x, rbarsq, qbar);
+  const double mr = mu * rbarsq;
+  vsq_raw = mu * mr;
+  const double vsq = vsq_raw < c.v0sq ? vsq_raw : c.v0sq;
+  omv = 1.0 - vsq;
+  W = fast_rsqrt(omv);
+  const double e0 = qbar - mr;
+  eps_raw = fma(W, e0, (vsq * (W * W)) * fast_rcp(1.0 + W));
+  const double eps = eps_raw > 0.0 ? eps_raw : 0.0;
+  const double ope = 1.0 + eps;
+  const double nuA = fma(c.gam, eps, 1.0) * (omv * W);               // (1 + a)(1 + eps)/W, 1/W = (1 - v^2) W
+  const double nuB = fma(c.gam, eps, 1.0) * fast_rcp(ope) * (1.0 + e0);
+  const double nu = nuA > nuB ? nuA : nuB;
+  return mu - fast_rcp(fma(rbarsq, mu, nu));
+}
+__device__ __forceinline__ double kastaun_fa(const KastaunC& c, double mu) {
+  double x, rbarsq, qbar;
+  kastaun_aux(c, mu, x, rbarsq, qbar);
+  return fma(mu, fast_sqrt(1.0 + rbarsq), -1.0);
+}
+// Illinois regula falsi on [a, b], fn(a) < 0 <= fn(b); AUX selects the function.  false: no convergence in 100 evaluations.
+template <bool AUX>
+__device__ __forceinline__ bool kastaun_root(const KastaunC& c, double a, double fa, double b, double fb, double& lo, double& hi) {
+  int side = 0;
+#pragma unroll 1
+  for (int it = 0; it < 100; it++) {
+    if (!(b - a > 4e-16 * b)) { lo = a; hi = b; return true; }
+    double m = fma(-fb, (b - a) / (fb - fa), b);
+    if (!(m > a && m < b)) m = 0.5 * (a + b);
+    double t0, t1, t2, t3;
+    const double fm = AUX ? kastaun_fa(c, m) : kastaun_f(c, m, t0, t1, t2, t3);
+    if (fm == 0.0) { lo = hi = m; return true; }
+    if (fm > 0.0) { b = m; fb = fm; if (side == 1) fa *= 0.5; side = 1; }
+    else if (fm < 0.0) { a = m; fa = fm; if (side == -1) fb *= 0.5; side = -1; }
+    else return false;
+  }
+  return false;
+}
+
+template <bool FLAT>
+__device__ __forceinline__ int u_to_p_kastaun_floors(const Geo& G, const double Uh[KH_NP], double gam, const FloorPar& fp, double rho_g,
+                                                     double u_g, double Pout[KH_NP], int& fflag) {
+  fflag = 0;
+  Pout[B1] = Uh[B1]; Pout[B2] = Uh[B2]; Pout[B3] = Uh[B3];
+  bool fin = true;
+#pragma unroll
+  for (int v = 0; v < KH_NP; v++) fin = fin && isfinite(Uh[v]);
+  if (!fin || !(Uh[RHO] > 0.0)) return 1;
+  const double alpha = G.alpha;
+  const double D = alpha * Uh[RHO];
+  const double Bc1 = alpha * Uh[B1], Bc2 = alpha * Uh[B2], Bc3 = alpha * Uh[B3];
+  const double Qc0 = alpha * (Uh[UU] - Uh[RHO]), Qc1 = alpha * Uh[U1], Qc2 = alpha * Uh[U2], Qc3 = alpha * Uh[U3];
+  double Qdotn, S1, S2, S3;                             // S^i = gamma^{ij} S_j
+  if (FLAT) {
+    Qdotn = Qc0; S1 = Qc1; S2 = Qc2; S3 = Qc3;
+  } else {
+    double Q0 = fma(G.n02, Qc2, fma(G.n01, Qc1, G.n00 * Qc0));
+    double Q1 = fma(G.n13, Qc3, fma(G.n12, Qc2, fma(G.n11, Qc1, G.n01 * Qc0)));
+    double Q2 = fma(G.n23, Qc3, fma(G.n22, Qc2, fma(G.n12, Qc1, G.n02 * Qc0)));
+    double Q3 = fma(G.n33, Qc3, fma(G.n23, Qc2, G.n13 * Qc1));
+    Qdotn = -alpha * Q0;
+    double qa = -alpha * Qdotn;
+    S1 = fma(qa, G.n01, Q1); S2 = fma(qa, G.n02, Q2); S3 = Q3;
+  }
+  const double Bsq = spatial_norm2<FLAT>(G, Bc1, Bc2, Bc3);
+  const double SdotB = fma(Qc3, Bc3, fma(Qc2, Bc2, Qc1 * Bc1));
+  const double Ssq = spatial_norm2<FLAT>(G, S1, S2, S3);
+  const double tau = -Qdotn - D;
+  const double iD = 1.0 / D;
+  KastaunC c;
+  c.gam = gam;
+  c.q = tau * iD;
+  c.rsq = Ssq * (iD * iD);
+  c.bsq = Bsq * iD;
+  c.rbsq = (SdotB * SdotB) * (iD * iD * iD);
+  c.brperp = fma(c.bsq, c.rsq, -c.rbsq);
+  if (c.brperp < 0.0) c.brperp = 0.0;
+  c.v0sq = c.rsq / (1.0 + c.rsq);
+
+  double mu_hi = 1.0, lo, hi;
+  if (!(c.rsq < 1.0)) {
+    const double fa1 = kastaun_fa(c, 1.0);
+    if (fa1 > 0.0) {
+      if (!kastaun_root<true>(c, 0.0, -1.0, 1.0, fa1, lo, hi)) return 2;
+      mu_hi = hi;
+    }
+  }
+  double vr, W, er, omv;
+  const double f0 = kastaun_f(c, 0.0, vr, W, er, omv);
+  const double f1 = kastaun_f(c, mu_hi, vr, W, er, omv);
+  double mu;
+  if (!(f0 < 0.0) || !isfinite(f1)) return 2;
+  if (f1 <= 0.0) mu = mu_hi;
+  else {
+    if (!kastaun_root<false>(c, 0.0, f0, mu_hi, f1, lo, hi)) return 2;
+    mu = 0.5 * (lo + hi);
+  }
+  double vsq_raw, eps_raw;
+  kastaun_f(c, mu, vsq_raw, W, eps_raw, omv);
+  if (!(vsq_raw <= c.v0sq * (1.0 + 1e-12))) return 3;
+  const double x = 1.0 / fma(mu, c.bsq, 1.0);
+  double rho = D * (omv * W);                           // D / W
+  double u = rho * eps_raw;
+  const double msb = mu * (SdotB * iD);                 // B_i v^i = mu (S.B)/D
+  const double fac = W * mu * x * iD;
+  double ut1 = fac * fma(msb, Bc1, S1);
+  double ut2 = fac * fma(msb, Bc2, S2);
+  double ut3 = fac * fma(msb, Bc3, S3);
+  if (!isfinite(rho) || !isfinite(u) || !isfinite(ut1) || !isfinite(ut2) || !isfinite(ut3)) return 7;
+  if (eps_raw < 0.0) return 5;
+  // floors (S18): comoving b^2 = B^2 (1 - v^2) + (B_i v^i)^2 and the Lorentz factor W
+  const double bsq = fma(Bsq, omv, msb * msb);
+  double vfac;
+  fflag = floor_limits(fp, rho_g, u_g, bsq, W, rho, u, vfac);
+  if (fflag & 32) { ut1 *= vfac; ut2 *= vfac; ut3 *= vfac; }
+  Pout[RHO] = rho; Pout[UU] = u; Pout[U1] = ut1; Pout[U2] = ut2; Pout[U3] = ut3;
+  return 0;
+}
+
 }  // namespace kh

@@ -277,7 +277,7 @@ emf_kernel(GV g, const double* __restrict__ F1, const double* __restrict__ F2, c
 // ~50 fp64 instructions instead of the 40-entry Gamma table and a 64-term contraction.
 // One thread per interior zone, flattened index (no idle lanes when n1 is not a multiple of the block).
 // ---------------------------------------------------------------------------------------------
-template <bool FLAT, bool CORR>
+template <bool FLAT, bool CORR, int INV>
 __global__ void __launch_bounds__(128, KH_MINB_UPDATE)
 update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps, double* __restrict__ Pf,
               const double* __restrict__ F1, const double* __restrict__ F2, const double* __restrict__ F3,
@@ -381,7 +381,8 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
     {
       const double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2);
       const double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
-      pf_flag = u_to_p_floors<FLAT>(G, Uh, W0, g.gam, g.fp, rho_g, u_g, pf, ff);
+      if (INV == 0) pf_flag = u_to_p_floors<FLAT>(G, Uh, W0, g.gam, g.fp, rho_g, u_g, pf, ff);
+      else pf_flag = u_to_p_kastaun_floors<FLAT>(G, Uh, g.gam, g.fp, rho_g, u_g, pf, ff);
     }
     if (pf_flag != 0) {          // rare: the hydro primitives keep the guess (S16); queue the zone for the fix-up
 #pragma unroll

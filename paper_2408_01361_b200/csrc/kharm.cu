@@ -190,12 +190,17 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
   prof_end(g);
   g->launches++;
   const unsigned grid = (unsigned)(((long)v.n1 * v.n2 * v.n3 + 127) / 128);
-#define UPD(FL, CO)                                                                                                  \
-  update_kernel<FL, CO><<<grid, 128, 0, g->stream>>>(v, Pi, Ps, Pf, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], \
-                                                     g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, g->fflag, g->faillist, g->sc, dt_factor)
+#define UPD(FL, CO, IN)                                                                                                  \
+  update_kernel<FL, CO, IN><<<grid, 128, 0, g->stream>>>(v, Pi, Ps, Pf, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], \
+                                                         g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, g->fflag, g->faillist, g->sc, dt_factor)
   prof_begin(g, KH_K_UPDATE);
-  if (g->flat) { if (corrector) UPD(true, true); else UPD(true, false); }
-  else { if (corrector) UPD(false, true); else UPD(false, false); }
+  if (g->p.inverter == KH_INV_KASTAUN) {
+    if (g->flat) { if (corrector) UPD(true, true, 1); else UPD(true, false, 1); }
+    else { if (corrector) UPD(false, true, 1); else UPD(false, false, 1); }
+  } else {
+    if (g->flat) { if (corrector) UPD(true, true, 0); else UPD(true, false, 0); }
+    else { if (corrector) UPD(false, true, 0); else UPD(false, false, 0); }
+  }
   prof_end(g);
 #undef UPD
   g->launches++;
@@ -261,7 +266,7 @@ int kh_grid_destroy(kh_grid* g) {
 int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   if (!p || !out) return KH_EINVAL;
   if (p->n1 < 1 || p->n2 < 1 || p->n3 < 1) return KH_EINVAL;
-  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1) return KH_EINVAL;
+  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1 || p->inverter < 0 || p->inverter > 1) return KH_EINVAL;
   if (!(p->gamma > 1.0) || !(p->cfl > 0.0) || !(p->dt_growth_max > 0.0)) return KH_EINVAL;
   const int N[3] = {p->n1, p->n2, p->n3};
   for (int d = 0; d < 3; d++) {

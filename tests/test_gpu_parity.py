@@ -275,3 +275,36 @@ def test_full_size_config3_one_step_sampled(kh, kho):
     worst = _assert_step_parity(p, gg.get_prims(), go.get_prims(), pf_g, pf_o, "cfg3 full")
     print("cfg3 full size: worst rel diff per primitive", worst)
     assert gg.divB() < 1e-10
+
+
+# ------------------------------------------------------------------------------------------ second inverter (NEXT-2)
+@pytest.mark.parametrize("case", ["torus_weno5", "mad_mc", "minkowski", "bondi"])
+def test_one_step_kastaun_inverter(kh, kho, case):
+    """Same bars as the 1D_W path with kh_params.inverter = KH_INV_KASTAUN on both sides."""
+    if case == "torus_weno5":
+        p = ki.config_params(3, n=(64, 48, 8)); P0 = torus.torus_state(p, seed=2); gh = False
+    elif case == "mad_mc":
+        p = ki.config_params(4, n=(72, 40, 6)); P0 = torus.torus_state(p, mad=True, seed=2); gh = False
+    elif case == "minkowski":
+        p = ki.config_params(5, n=(37, 13, 5), recon=kp.RECON_WENO5); P0 = modes.config5(p, seed=1, amp=1e-3); gh = False
+    else:
+        p = ki.config_params(2); P0 = bondi.config2(p); gh = True
+    p = dict(p, inverter=kp.INV_KASTAUN)
+    _one_step_case(kh, kho, p, P0, with_ghosts=gh, label="kastaun " + case)
+
+
+def test_kastaun_stress_flags_and_run(kh, kho):
+    """Failures, floors and fix-ups under the second inverter (flags identical), then a short run in L1."""
+    p = dict(ki.config_params(4, n=(72, 40, 8)), inverter=kp.INV_KASTAUN)
+    P0 = torus.torus_state(p, mad=True, seed=3, stress=True, stress_fraction=0.02)
+    worst, gg, go = _one_step_case(kh, kho, p, P0, label="kastaun cfg4-stress")
+    pf, ff = go.get_flags()
+    assert gg.count_flags()[0] == (pf != 0).sum()
+    p = dict(ki.config_params(3, n=(48, 32, 8)), inverter=kp.INV_KASTAUN)
+    gg, go = _both(kh, kho, p, torus.torus_state(p, seed=1))
+    dt = go.estimate_dt()
+    for _ in range(10):
+        dg, dt = gg.step(dt), go.step(dt)
+        assert abs(dg / dt - 1) < 1e-9
+    l1 = l1_diff(p, gg.get_prims(), go.get_prims())
+    assert l1.max() <= TOL_RUN_L1, l1
