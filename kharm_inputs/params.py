@@ -20,7 +20,7 @@ FLOOR_DEFAULTS = dict(rho_min=1e-6, u_min=1e-8, r_char=10.0, bsq_over_rho_max=10
 def base_params(**kw):
     p = dict(coords=MINKOWSKI, a=0.0, hslope=0.3, poly_xt=0.82, poly_alpha=14.0, mks_smooth=0.5,
              n1=16, n2=16, n3=16, xmin=[0.0, 0.0, 0.0], xmax=[1.0, 1.0, 1.0], bc=[BC_PERIODIC] * 6,
-             gamma=4.0 / 3.0, cfl=0.9, recon=RECON_MC, inverter=INV_1DW)
+             gamma=4.0 / 3.0, cfl=0.9, recon=RECON_MC, inverter=INV_1DW, fofc=0)
     p.update(FLOOR_DEFAULTS)
     p.update(kw)
     return p

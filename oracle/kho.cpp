@@ -817,12 +817,10 @@ void fixup(kho_grid& g, double* Pf) {
 }
 
 // One sub-step (S22): fluxes from Ps, update of U(Pi) by Dt, U->P with guess Pi, floors, fill, fix-up, fill.
-void substep(kho_grid& g, const double* Pi, const double* Ps, double* Pf, double Dt) {
-  for (int d = 0; d < 3; d++) compute_flux(g, Ps, d);
-  flux_ct(g, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data());
+// C6 + C7 + C8 on the interior zones: U_f = U(P_i) + Dt [-div F + S(P_s)], inversion with guess P_i, floors.
+void update_zones(kho_grid& g, const double* Pi, const double* Ps, double* Pf, double Dt) {
   const long nt = g.ntot;
   const long st[3] = {1, g.nt[0], (long)g.nt[0] * g.nt[1]};
-  if (Pf != Pi) std::memcpy(Pf, Pi, sizeof(double) * NP * nt);   // ghosts of Pf start from Pi (matters for FIXED)
   std::fill(g.pflag.begin(), g.pflag.end(), 0);
   std::fill(g.fflag.begin(), g.fflag.end(), 0);
 #ifdef _OPENMP
@@ -850,6 +848,48 @@ void substep(kho_grid& g, const double* Pi, const double* Ps, double* Pf, double
     g.fflag[n] = ff;
     for (int v = 0; v < NP; v++) Pf[v * nt + n] = pf[v];
   }
+}
+
+// First-order flux correction (reading S25 in DESIGN.md): the faces of
+// every zone of `mask` (ghost images included) get the Local Lax-Friedrichs flux of the donor-cell states, i.e.
+// P_L = P_s(zone below the face), P_R = P_s(zone above it).  Same face ranges as compute_flux; axis faces stay zero.
+void fofc_reflux(kho_grid& g, const double* Ps, const std::vector<int>& mask) {
+  for (int d = 0; d < 3; d++) {
+    int lo[3], hi[3];
+    for (int e = 0; e < 3; e++) { lo[e] = (e == d) ? 0 : -1; hi[e] = g.n[e] + 1; }
+    long stride = (d == 0) ? 1 : (d == 1 ? g.nt[0] : (long)g.nt[0] * g.nt[1]);
+    for (int k = lo[2]; k < hi[2]; k++) for (int j = lo[1]; j < hi[1]; j++) for (int i = lo[0]; i < hi[0]; i++) {
+      long n = g.idx(i, j, k);
+      if (!(mask[n - stride] || mask[n])) continue;
+      if (d == 1 && polar_face(g, j)) continue;
+      double PL[NP], PR[NP], Fl[NP], c;
+      get_prim(g, Ps, n - stride, PL);
+      get_prim(g, Ps, n, PR);
+      llf(g.G[1 + d][g.idx2(i, j)], PL, PR, g.p.gamma, d + 1, Fl, c);
+      for (int v = 0; v < NP; v++) g.F[d][v * g.ntot + n] = Fl[v];
+      g.ctop[d][n] = c;
+    }
+  }
+}
+
+void substep(kho_grid& g, const double* Pi, const double* Ps, double* Pf, double Dt) {
+  for (int d = 0; d < 3; d++) compute_flux(g, Ps, d);
+  const long nt = g.ntot;
+  if (g.p.fofc) {
+    // speculative update with the high-order fluxes: which zones would fail the inversion or hit a floor?
+    std::vector<double> raw[3] = {g.F[0], g.F[1], g.F[2]};                      // flux_ct rewrites the B components in place
+    flux_ct(g, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data());
+    if (Pf != Pi) std::memcpy(Pf, Pi, sizeof(double) * NP * nt);
+    update_zones(g, Pi, Ps, Pf, Dt);
+    std::vector<int> mask(nt, 0);
+    for (long n = 0; n < nt; n++) mask[n] = (g.pflag[n] != 0 || g.fflag[n] != 0) ? 1 : 0;   // ghosts are 0 here
+    fill_ghosts_flag(g, mask.data());                                              // ghost images of troubled zones
+    for (int d = 0; d < 3; d++) g.F[d] = raw[d];
+    fofc_reflux(g, Ps, mask);
+  }
+  flux_ct(g, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data());
+  if (Pf != Pi) std::memcpy(Pf, Pi, sizeof(double) * NP * nt);   // ghosts of Pf start from Pi (matters for FIXED)
+  update_zones(g, Pi, Ps, Pf, Dt);
   fill_ghosts_prims(g, Pf);
   fill_ghosts_flag(g, g.pflag.data());
   fixup(g, Pf);
@@ -1090,6 +1130,15 @@ int kho_debug_fixup(kho_grid* g, const int* pflag_with_ghosts) {
   if (!g || !pflag_with_ghosts) return KHO_EINVAL;
   for (long n = 0; n < g->ntot; n++) { g->pflag[n] = pflag_with_ghosts[n]; g->fflag[n] = 0; }
   fixup(*g, g->P.data());
+  return KHO_OK;
+}
+int kho_debug_fofc(kho_grid* g, const int* mask_with_ghosts) {
+  if (!g || !mask_with_ghosts) return KHO_EINVAL;
+  const double* P = g->P.data();
+  for (int d = 0; d < 3; d++) compute_flux(*g, P, d);
+  std::vector<int> mask(mask_with_ghosts, mask_with_ghosts + g->ntot);
+  fill_ghosts_flag(*g, mask.data());
+  fofc_reflux(*g, P, mask);
   return KHO_OK;
 }
 int kho_fill_ghosts(kho_grid* g) {

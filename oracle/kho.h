@@ -39,6 +39,7 @@ typedef struct {
   double rho_min, u_min, r_char, bsq_over_rho_max, bsq_over_u_max, u_over_rho_max, gamma_max;
   double dt_growth_max;
   int inverter;                                    /* KHO_INV_1DW | KHO_INV_KASTAUN (NEXT-2) */
+  int fofc;                                        /* 1: first-order flux correction (NEXT-3) */
 } kho_params;
 
 typedef struct kho_grid kho_grid;
@@ -62,6 +63,9 @@ int kho_get_conn(kho_grid* g, double* conn64);            /* [(n2+6)(n1+6)][lam]
 int kho_fill_ghosts(kho_grid* g);
 /* test hook: C9 fix-up (+ floors) of the current primitives for a caller-supplied pflag array [nt] */
 int kho_debug_fixup(kho_grid* g, const int* pflag_with_ghosts);
+/* test hook (NEXT-3): high-order fluxes of the current primitives, then the first-order flux correction for a caller-
+ * supplied zone mask [nt] (its ghosts are filled like pflag); leaves the RAW fluxes (no Flux-CT) for kho_get_flux */
+int kho_debug_fofc(kho_grid* g, const int* mask_with_ghosts);
 /* test hook: predictor sub-step only; P* becomes the current state */
 int kho_debug_predictor(kho_grid* g, double dt);
 

@@ -27,7 +27,7 @@ class Params(C.Structure):
         ("gamma", C.c_double), ("cfl", C.c_double), ("recon", C.c_int),
         ("rho_min", C.c_double), ("u_min", C.c_double), ("r_char", C.c_double),
         ("bsq_over_rho_max", C.c_double), ("bsq_over_u_max", C.c_double), ("u_over_rho_max", C.c_double),
-        ("gamma_max", C.c_double), ("dt_growth_max", C.c_double), ("inverter", C.c_int),
+        ("gamma_max", C.c_double), ("dt_growth_max", C.c_double), ("inverter", C.c_int), ("fofc", C.c_int),
     ]
 
 
@@ -262,6 +262,11 @@ class Grid:
         pf = np.ascontiguousarray(pflag_with_ghosts, dtype=np.int32)
         assert pf.shape == self.shape_gh[1:]
         _chk(self.L.kho_debug_fixup(self.h, pf.ctypes.data_as(_ip)))
+
+    def debug_fofc(self, mask_with_ghosts):
+        m = np.ascontiguousarray(mask_with_ghosts, dtype=np.int32)
+        assert m.shape == self.shape_gh[1:]
+        _chk(self.L.kho_debug_fofc(self.h, m.ctypes.data_as(_ip)))
 
     def fill_ghosts(self):
         _chk(self.L.kho_fill_ghosts(self.h))
