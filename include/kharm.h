@@ -55,6 +55,8 @@ typedef struct {
   double dt_growth_max;       /* dt_next <= dt_growth_max * dt                                              */
   int inverter;               /* KH_INV_1DW (the 1D_W Newton iteration) | KH_INV_KASTAUN (the
                                  bracketed root find of Kastaun et al.; same pflag codes, no guess needed)   */
+  int fofc;                   /* 1: first-order flux correction: a speculative update finds the zones
+                                 that would fail the inversion or hit a floor; their faces get donor-cell LLF fluxes */
 } kh_params;
 
 typedef struct kh_grid kh_grid;   /* opaque */
@@ -130,7 +132,7 @@ int kh_set_graph(kh_grid* g, int enable);
  * per-kernel roofline; the bracketing serialises nothing (one stream) but adds two event records per launch,
  * so headline throughput is always measured with profiling off. */
 enum { KH_K_FLUX1 = 0, KH_K_FLUX2 = 1, KH_K_FLUX3 = 2, KH_K_EMF = 3, KH_K_UPDATE = 4, KH_K_FILL = 5, KH_K_FIXUP = 6,
-       KH_K_COUNT = 7 };
+       KH_K_FOFC = 7 /* mask + re-flux of the first-order flux correction */, KH_K_COUNT = 8 };
 int kh_set_profile(kh_grid* g, int enable);
 int kh_get_profile(kh_grid* g, double* ms, long long* count);
 /* Stand-alone DFMA-chain micro-benchmark: returns achieved fp64 TFLOP/s on the current device

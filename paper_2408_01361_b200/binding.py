@@ -13,7 +13,7 @@ BC_PERIODIC, BC_OUTFLOW, BC_POLAR, BC_FIXED = 0, 1, 2, 3
 RECON_MC, RECON_WENO5 = 0, 1
 INV_1DW, INV_KASTAUN = 0, 1
 LOC_CENT, LOC_FACE1, LOC_FACE2, LOC_FACE3 = 0, 1, 2, 3
-KERNEL_KINDS = ("flux1", "flux2", "flux3", "emf", "update", "fill", "fixup")     # KH_K_* of include/kharm.h
+KERNEL_KINDS = ("flux1", "flux2", "flux3", "emf", "update", "fill", "fixup", "fofc")     # KH_K_* of include/kharm.h
 MEM_DEVICE, MEM_HOST = 0, 1
 NG = 3
 
@@ -40,7 +40,7 @@ class Params(C.Structure):
         ("gamma", C.c_double), ("cfl", C.c_double), ("recon", C.c_int),
         ("rho_min", C.c_double), ("u_min", C.c_double), ("r_char", C.c_double),
         ("bsq_over_rho_max", C.c_double), ("bsq_over_u_max", C.c_double), ("u_over_rho_max", C.c_double),
-        ("gamma_max", C.c_double), ("dt_growth_max", C.c_double), ("inverter", C.c_int),
+        ("gamma_max", C.c_double), ("dt_growth_max", C.c_double), ("inverter", C.c_int), ("fofc", C.c_int),
     ]
 
 

@@ -423,7 +423,10 @@ __global__ void finalize_dt_kernel(StepScalars* sc, double cfl, double growth) {
   sc->rate_bits = 0ULL;
 }
 __global__ void set_dt_kernel(StepScalars* sc, double dt, int from_next) { sc->dt = from_next ? sc->dt_next : dt; }
-__global__ void reset_counters_kernel(StepScalars* sc) { sc->n_pflag = 0; sc->n_fflag = 0; }
+__global__ void reset_counters_kernel(StepScalars* sc, int also_rate) {
+  sc->n_pflag = 0; sc->n_fflag = 0;
+  if (also_rate) sc->rate_bits = 0ULL;      // FOFC: the speculative corrector update has written its CFL maximum
+}
 
 // ---------------------------------------------------------------------------------------------
 // K7: ghost fill (S20).  The scheme's definition is three sequential passes x1 -> x2 -> x3, each spanning the
@@ -590,6 +593,57 @@ fixup_apply_kernel(GV g, double* __restrict__ Pf, const unsigned* __restrict__ l
           for (int v = 0; v < 5; v++) Pf[v * nt + m] = (v == U2) ? sgn * P[v] : P[v];
         }
       }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// First-order flux correction (S25).  After a speculative update with the
+// high-order fluxes, every zone whose inversion failed or that hit a floor is "troubled"; the faces of the troubled
+// zones and of their ghost images get the LLF flux of the donor-cell states (the two adjacent zones' primitives).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+fofc_mask_kernel(GV g, const unsigned char* __restrict__ pflag, const unsigned char* __restrict__ fflag, unsigned char* __restrict__ mask) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  if (i >= g.n1) return;
+  const long n = zidx(g, i, j, k);
+  mask[n] = (pflag[n] | fflag[n]) != 0;
+}
+
+template <bool FLAT>
+__global__ void __launch_bounds__(128)
+fofc_reflux_kernel(GV g, const double* __restrict__ P, const unsigned char* __restrict__ mask, double* __restrict__ F1,
+                   double* __restrict__ F2, double* __restrict__ F3, double* __restrict__ ct1, double* __restrict__ ct2,
+                   double* __restrict__ ct3) {
+  // zones (i, j, k) in [-1, N]^3: each owns its three lower faces (same face ranges as the flux kernels)
+  const int i = blockIdx.x * blockDim.x + threadIdx.x - 1, j = (int)blockIdx.y - 1, k = (int)blockIdx.z - 1;
+  if (i > g.n1) return;
+  const long n = zidx(g, i, j, k), nt = g.ntot;
+  const bool me = mask[n] != 0;
+  double PR[KH_NP], PL[KH_NP];
+  bool loaded = false;
+  auto load_own = [&]() {
+    if (loaded) return;
+#pragma unroll
+    for (int v = 0; v < KH_NP; v++) PR[v] = P[v * nt + n];
+    loaded = true;
+  };
+  if (i >= 0 && (me || mask[n - 1])) {
+    load_own();
+#pragma unroll
+    for (int v = 0; v < KH_NP; v++) PL[v] = P[v * nt + n - 1];
+    face_flux<1, FLAT>(g, PL, PR, pidx(g, i, j), n, F1, ct1);
+  }
+  if (j >= 0 && (me || mask[n - g.s2]) && !polar_face(g, j)) {
+    load_own();
+#pragma unroll
+    for (int v = 0; v < KH_NP; v++) PL[v] = P[v * nt + n - g.s2];
+    face_flux<2, FLAT>(g, PL, PR, pidx(g, i, j), n, F2, ct2);
+  }
+  if (k >= 0 && (me || mask[n - g.s3])) {
+    load_own();
+#pragma unroll
+    for (int v = 0; v < KH_NP; v++) PL[v] = P[v * nt + n - g.s3];
+    face_flux<3, FLAT>(g, PL, PR, pidx(g, i, j), n, F3, ct3);
   }
 }
 

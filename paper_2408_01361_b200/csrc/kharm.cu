@@ -39,6 +39,7 @@ struct kh_grid {
   double* ctop[3];
   double* emf[3];
   unsigned char *pflag, *fflag;
+  unsigned char* mask;   // FOFC: troubled zones of the speculative update (with ghost images)
   unsigned* faillist;    // zones (device-layout index) whose inversion failed in the current sub-step
   double* fix;           // [5][ntot] scratch of the fix-up (pre-fix-up snapshot semantics)
   double* stage;         // lazily allocated [8][ntot] staging buffer for host transfers / debug copies
@@ -180,31 +181,50 @@ static int do_fixup(kh_grid* g, double* Pf) {
 // One sub-step (S22): fluxes from Ps, update of U(Pi), inversion with guess Pi, floors, fill, fix-up, fill.
 static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, double dt_factor, bool corrector) {
   const GV& v = g->gv;
-  reset_counters_kernel<<<1, 1, 0, g->stream>>>(g->sc);
+  reset_counters_kernel<<<1, 1, 0, g->stream>>>(g->sc, 0);
   g->launches++;
   launch_flux<1>(g, Ps);
   launch_flux<2>(g, Ps);
   launch_flux<3>(g, Ps);
-  prof_begin(g, KH_K_EMF);
-  emf_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], g->emf[2]);
-  prof_end(g);
-  g->launches++;
-  const unsigned grid = (unsigned)(((long)v.n1 * v.n2 * v.n3 + 127) / 128);
+  const int passes = g->p.fofc ? 2 : 1;       // FOFC: a speculative update first, then the re-flux, then the real one
+  for (int pass = 0; pass < passes; pass++) {
+    prof_begin(g, KH_K_EMF);
+    emf_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], g->emf[2]);
+    prof_end(g);
+    g->launches++;
+    const unsigned grid = (unsigned)(((long)v.n1 * v.n2 * v.n3 + 127) / 128);
 #define UPD(FL, CO, IN)                                                                                                  \
   update_kernel<FL, CO, IN><<<grid, 128, 0, g->stream>>>(v, Pi, Ps, Pf, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], \
                                                          g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, g->fflag, g->faillist, g->sc, dt_factor)
-  prof_begin(g, KH_K_UPDATE);
-  if (g->p.inverter == KH_INV_KASTAUN) {
-    if (g->flat) { if (corrector) UPD(true, true, 1); else UPD(true, false, 1); }
-    else { if (corrector) UPD(false, true, 1); else UPD(false, false, 1); }
-  } else {
-    if (g->flat) { if (corrector) UPD(true, true, 0); else UPD(true, false, 0); }
-    else { if (corrector) UPD(false, true, 0); else UPD(false, false, 0); }
-  }
-  prof_end(g);
+    prof_begin(g, KH_K_UPDATE);
+    if (g->p.inverter == KH_INV_KASTAUN) {
+      if (g->flat) { if (corrector) UPD(true, true, 1); else UPD(true, false, 1); }
+      else { if (corrector) UPD(false, true, 1); else UPD(false, false, 1); }
+    } else {
+      if (g->flat) { if (corrector) UPD(true, true, 0); else UPD(true, false, 0); }
+      else { if (corrector) UPD(false, true, 0); else UPD(false, false, 0); }
+    }
+    prof_end(g);
 #undef UPD
-  g->launches++;
-  CK(cudaGetLastError());
+    g->launches++;
+    CK(cudaGetLastError());
+    if (pass + 1 < passes) {
+      // troubled zones of the speculative update -> mask (+ ghost images) -> donor-cell LLF on their faces
+      prof_begin(g, KH_K_FOFC);
+      CK(cudaMemsetAsync(g->mask, 0, v.ntot, g->stream));
+      fofc_mask_kernel<<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, g->pflag, g->fflag, g->mask);
+      prof_end(g);
+      int rc = fill_ghosts(g, nullptr, g->mask);
+      if (rc) return rc;
+      prof_begin(g, KH_K_FOFC);
+      if (g->flat) fofc_reflux_kernel<true><<<zone_grid(v.n1 + 2, v.n2 + 2, v.n3 + 2), 128, 0, g->stream>>>(v, Ps, g->mask, g->F[0], g->F[1], g->F[2], g->ctop[0], g->ctop[1], g->ctop[2]);
+      else fofc_reflux_kernel<false><<<zone_grid(v.n1 + 2, v.n2 + 2, v.n3 + 2), 128, 0, g->stream>>>(v, Ps, g->mask, g->F[0], g->F[1], g->F[2], g->ctop[0], g->ctop[1], g->ctop[2]);
+      reset_counters_kernel<<<1, 1, 0, g->stream>>>(g->sc, 1);
+      prof_end(g);
+      g->launches += 3;
+      CK(cudaGetLastError());
+    }
+  }
   int rc = fill_ghosts(g, Pf, g->pflag);
   if (rc) return rc;
   return do_fixup(g, Pf);      // also refreshes the ghost images of the fixed zones (the second fill of S22)
@@ -254,7 +274,7 @@ int kh_grid_destroy(kh_grid* g) {
   for (int l = 0; l < 4; l++) cudaFree(g->geom[l]);
   cudaFree(g->conn); cudaFree(g->dg); cudaFree(g->floorp);
   for (int b = 0; b < 3; b++) { cudaFree(g->P[b]); cudaFree(g->F[b]); cudaFree(g->ctop[b]); cudaFree(g->emf[b]); }
-  cudaFree(g->pflag); cudaFree(g->fflag); cudaFree(g->faillist); cudaFree(g->sc); cudaFree(g->fix); cudaFree(g->stage);
+  cudaFree(g->pflag); cudaFree(g->fflag); cudaFree(g->mask); cudaFree(g->faillist); cudaFree(g->sc); cudaFree(g->fix); cudaFree(g->stage);
   if (g->sc_host) cudaFreeHost(g->sc_host);
   if (g->pev) { for (int e = 0; e < 2 * KH_PROF_POOL; e++) if (g->pev[e]) cudaEventDestroy(g->pev[e]); delete[] g->pev; }
   delete[] g->pkind;
@@ -266,7 +286,7 @@ int kh_grid_destroy(kh_grid* g) {
 int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   if (!p || !out) return KH_EINVAL;
   if (p->n1 < 1 || p->n2 < 1 || p->n3 < 1) return KH_EINVAL;
-  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1 || p->inverter < 0 || p->inverter > 1) return KH_EINVAL;
+  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1 || p->inverter < 0 || p->inverter > 1 || p->fofc < 0 || p->fofc > 1) return KH_EINVAL;
   if (!(p->gamma > 1.0) || !(p->cfl > 0.0) || !(p->dt_growth_max > 0.0)) return KH_EINVAL;
   const int N[3] = {p->n1, p->n2, p->n3};
   for (int d = 0; d < 3; d++) {
@@ -345,6 +365,7 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   ALLOC(g->fix, 5 * fb);
   ALLOC(g->pflag, v.ntot);
   ALLOC(g->fflag, v.ntot);
+  if (p->fofc) ALLOC(g->mask, v.ntot);
   ALLOC(g->faillist, sizeof(unsigned) * (size_t)v.n1 * v.n2 * v.n3);
   ALLOC(g->sc, sizeof(StepScalars));
 #undef ALLOC
@@ -624,7 +645,7 @@ int kh_debug_fixup(kh_grid* g, const int* pflag_with_ghosts, int mem) {
   int_to_flags_kernel<<<(unsigned)((v.ntot + 127) / 128), 128, 0, g->stream>>>(v.ntot, src, g->pflag);
   g->launches++;
   CK(cudaMemsetAsync(g->fflag, 0, v.ntot, g->stream));
-  reset_counters_kernel<<<1, 1, 0, g->stream>>>(g->sc);
+  reset_counters_kernel<<<1, 1, 0, g->stream>>>(g->sc, 0);
   build_faillist_kernel<<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, g->pflag, g->faillist, g->sc);
   g->launches += 2;
   int rc = do_fixup(g, g->P[g->cur]);

@@ -308,3 +308,55 @@ def test_kastaun_stress_flags_and_run(kh, kho):
         assert abs(dg / dt - 1) < 1e-9
     l1 = l1_diff(p, gg.get_prims(), go.get_prims())
     assert l1.max() <= TOL_RUN_L1, l1
+
+
+# ------------------------------------------------------------------------------------------ first-order flux correction (NEXT-3)
+@pytest.mark.parametrize("case", ["torus_weno5", "mad_stress_mc", "minkowski", "bondi", "torus_kastaun"])
+def test_one_step_fofc(kh, kho, case):
+    """kh_params.fofc = 1 on both sides: same bars; the troubled-zone selection goes through
+    the flags, which must be identical for the corrected fluxes to be."""
+    if case == "torus_weno5":
+        p = ki.config_params(3, n=(64, 48, 8)); P0 = torus.torus_state(p, seed=2); gh = False
+    elif case == "mad_stress_mc":
+        p = ki.config_params(4, n=(72, 40, 8)); P0 = torus.torus_state(p, mad=True, seed=3, stress=True, stress_fraction=0.02); gh = False
+    elif case == "minkowski":
+        p = ki.config_params(5, n=(37, 13, 5), recon=kp.RECON_WENO5); P0 = modes.config5(p, seed=1, amp=1e-3); gh = False
+    elif case == "bondi":
+        p = ki.config_params(2); P0 = bondi.config2(p); gh = True
+    else:
+        p = dict(ki.config_params(3, n=(33, 17, 3)), inverter=kp.INV_KASTAUN); P0 = torus.torus_state(p, seed=2); gh = False
+    p = dict(p, fofc=1)
+    worst, gg, go = _one_step_case(kh, kho, p, P0, with_ghosts=gh, label="fofc " + case)
+    if case == "mad_stress_mc":
+        assert gg.count_flags()[0] == (go.get_flags()[0] != 0).sum()
+        # stage parity of the corrected fluxes, EMFs and c_top (the corrector's)
+        I = (slice(3, -3), slice(3, -3), slice(3, -3))
+        for d in (1, 2, 3):
+            Fg, cg = gg.get_flux(d)
+            Fo, co = go.get_flux(d)
+            assert np.allclose(cg[I], co[I], rtol=1e-11, atol=1e-14), d
+            for v in range(8):
+                assert np.abs(Fg[v][I] - Fo[v][I]).max() <= 1e-11 * (np.abs(Fo[v][I]).max() + 1e-300), (d, v)
+
+
+def test_fofc_run_l1_and_untroubled_bit_identity(kh, kho):
+    p = dict(ki.config_params(3, n=(48, 32, 8)), fofc=1)
+    gg, go = _both(kh, kho, p, torus.torus_state(p, seed=1))
+    dt = go.estimate_dt()
+    for _ in range(10):
+        dg, dt = gg.step(dt), go.step(dt)
+        assert abs(dg / dt - 1) < 1e-9
+    l1 = l1_diff(p, gg.get_prims(), go.get_prims())
+    assert l1.max() <= TOL_RUN_L1, l1
+    # a problem on which nothing is troubled: the FOFC step is bit-identical to the plain step on the GPU too
+    q = ki.config_params(5, n=(24, 16, 8), recon=kp.RECON_WENO5)
+    P0 = modes.config5(q, seed=1, amp=1e-3)
+    res = []
+    for fofc in (0, 1):
+        g = kh.Grid(dict(q, fofc=fofc))
+        g.set_prims(P0)
+        d = g.estimate_dt()
+        for _ in range(3):
+            d = g.step(d)
+        res.append((g.get_prims(), d))
+    assert np.array_equal(res[0][0], res[1][0]) and res[0][1] == res[1][1]
