@@ -617,8 +617,40 @@ int u2p_kastaun(const Geom& G, const double U[NP], const double Pg[NP], double g
 }
 
 // ---------------------------------------------------------------------------------------------
-// C8. Floors and ceilings, fluid frame (S18).  Returns the fflag bits.
+// C8. Floors and ceilings (S18).  Returns the fflag bits.
+// p.floor_frame = KHO_FRAME_FLUID: rho, u overwritten in place, velocity and field untouched.
+// p.floor_frame = KHO_FRAME_DRIFT ("the most common of which is the drift frame"; SURVEY 8(f)
+// NEXT-4; reading S26): the material is added in the frame that moves with the E x B drift, so that with the normal
+// observer's velocity v^i = ut^i/gamma split along the field, v = v_perp + v_par B/|B|,
+//   * the drift velocity v_perp is unchanged, and
+//   * the momentum along the field, S_i B^i/|B| = w gamma^2 v_par (w = rho + Gamma u), is conserved:
+//       A = w gamma^2 v_par / w',   v_par' / (1 - v_perp^2 - v_par'^2) = A
+//       =>  v_par' = 2 A (1 - v_perp^2) / (1 + sqrt(1 + 4 A^2 (1 - v_perp^2))).
+// (b^2 = B^2 (1 - v_perp^2) is then unchanged too, so the magnetisation limits stay consistent.)  B = 0: no direction,
+// the velocity is kept.  The Lorentz-factor ceiling acts on the adjusted velocity.
 // ---------------------------------------------------------------------------------------------
+void drift_frame_velocity(const Geom& G, double gam, double rho_old, double u_old, double rho_new, double u_new, double P[NP]) {
+  double Bcov[4] = {0, 0, 0, 0}, qsq = 0.0, Bsq = 0.0, uB = 0.0;
+  for (int i = 1; i < 4; i++) for (int j = 1; j < 4; j++) {
+    qsq += G.gcov[i][j] * P[U1 + i - 1] * P[U1 + j - 1];
+    Bcov[i] += G.gcov[i][j] * P[B1 + j - 1];
+  }
+  for (int i = 1; i < 4; i++) { Bsq += Bcov[i] * P[B1 + i - 1]; uB += Bcov[i] * P[U1 + i - 1]; }
+  if (!(Bsq > 0.0)) return;
+  double gamma = std::sqrt(1.0 + qsq), B = std::sqrt(Bsq);
+  double vpar = uB / (gamma * B);                          // v^i B_i / |B|
+  double vsq = qsq / (gamma * gamma);
+  double omp = 1.0 - (vsq - vpar * vpar);                  // 1 - v_perp^2
+  if (omp > 1.0) omp = 1.0;
+  double vperp[3];
+  for (int i = 0; i < 3; i++) vperp[i] = P[U1 + i] / gamma - vpar * P[B1 + i] / B;
+  double w_old = rho_old + gam * u_old, w_new = rho_new + gam * u_new;
+  double A = w_old * gamma * gamma * vpar / w_new;
+  double vpar_new = 2.0 * A * omp / (1.0 + std::sqrt(1.0 + 4.0 * A * A * omp));
+  double gamma_new = 1.0 / std::sqrt(omp - vpar_new * vpar_new);
+  for (int i = 0; i < 3; i++) P[U1 + i] = gamma_new * (vperp[i] + vpar_new * P[B1 + i] / B);
+}
+
 int floors(const kho_params& p, const Geom& G, double r, double P[NP]) {
   int flag = 0;
   double s = (p.coords == KHO_MINKOWSKI) ? 1.0 : 1.0 / (r * r) / (1.0 + r / p.r_char);
@@ -628,9 +660,11 @@ int floors(const kho_params& p, const Geom& G, double r, double P[NP]) {
   double u_g = p.u_min * std::pow(s, p.gamma), u_b = D.bsq / p.bsq_over_u_max;
   double rho_fl = rho_b > rho_g ? rho_b : rho_g;
   double u_fl = u_b > u_g ? u_b : u_g;
+  const double rho_old = P[RHO], u_old = P[UU];
   if (P[RHO] < rho_fl) { P[RHO] = rho_fl; flag |= (rho_b > rho_g) ? 2 : 1; }
   if (P[UU] < u_fl) { P[UU] = u_fl; flag |= (u_b > u_g) ? 8 : 4; }
   if (P[UU] > p.u_over_rho_max * P[RHO]) { P[UU] = p.u_over_rho_max * P[RHO]; flag |= 16; }
+  if (p.floor_frame == KHO_FRAME_DRIFT && flag != 0) drift_frame_velocity(G, p.gamma, rho_old, u_old, P[RHO], P[UU], P);
   double qsq = 0.0;
   for (int i = 1; i < 4; i++) for (int j = 1; j < 4; j++) qsq += G.gcov[i][j] * P[U1 + i - 1] * P[U1 + j - 1];
   double gamma = std::sqrt(1.0 + qsq);

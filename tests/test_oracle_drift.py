@@ -1,0 +1,122 @@
+"""Pins of the oracle's drift-frame floors (S26).
+
+The frame is defined by two physical statements, and the tests check exactly those on the oracle's output with
+quantities computed here from the primitives alone (numpy) or by the separately pinned P -> U map:
+  * the velocity component perpendicular to the field seen by the normal observer (the E x B drift) is unchanged;
+  * the conserved momentum along the field, S_i B^i, is unchanged although rho and u were raised;
+plus the consequences / limits: comoving b^2 unchanged, v perpendicular to B or B = 0 -> velocity unchanged, no floor
+hit -> identity, and the same (rho, u, flags) as the fluid-frame floors.
+"""
+import numpy as np
+
+import kharm_inputs as ki
+from kharm_inputs import params as kp
+
+ETA = np.diag([-1.0, 1, 1, 1])
+
+
+def _geoms(kho):
+    out = [(ETA, ETA, 1.0, 0.5, 0.5)]
+    Pf = kho.make_params(ki.config_params(3))
+    for x1, x2 in ((0.26, 0.004), (2.5, 0.5), (6.5, 0.8)):
+        gcov, gcon, gdet, _ = kho.metric(Pf, x1, x2)
+        out.append((gcov, gcon, gdet, x1, x2))
+    return out
+
+
+def _split(gcov, P):
+    """normal-observer velocity, its part along B and the perpendicular rest (contravariant components)"""
+    g3 = gcov[1:, 1:]
+    ut, B = P[2:5], P[5:8]
+    gamma = np.sqrt(1 + ut @ g3 @ ut)
+    v = ut / gamma
+    Bn = np.sqrt(B @ g3 @ B)
+    vpar = (v @ g3 @ B) / Bn
+    return v, vpar, v - vpar * B / Bn, gamma
+
+
+def _params(kho, cfg_coords, frame, **kw):
+    d = ki.config_params(3) if cfg_coords else ki.config_params(5)
+    d = dict(d, floor_frame=frame, **kw)
+    return kho.make_params(d)
+
+
+def test_drift_frame_keeps_the_drift_velocity_and_the_momentum_along_the_field(kho):
+    rng = np.random.default_rng(11)
+    n = 0
+    for gi, (gcov, gcon, gdet, x1, x2) in enumerate(_geoms(kho)):
+        pd, pf = _params(kho, gi > 0, kp.FRAME_DRIFT), _params(kho, gi > 0, kp.FRAME_FLUID)
+        gam = pd.gamma
+        for _ in range(40):
+            P = np.zeros(8)
+            P[0] = 10 ** rng.uniform(-24, -20)                     # below the floors at every radius
+            P[1] = P[0] * 10 ** rng.uniform(-4, 0)
+            for i in range(3):
+                P[2 + i] = rng.normal() * 10 ** rng.uniform(-1, 0.5) / np.sqrt(gcov[i + 1, i + 1])
+                P[5 + i] = rng.normal() * 1e-3 / np.sqrt(gcov[i + 1, i + 1])
+            Pd, fd = kho.floors(pd, gcov, gcon, x1, x2, P)
+            Pf_, ff = kho.floors(pf, gcov, gcon, x1, x2, P)
+            assert fd == ff and fd != 0 and Pd[0] == Pf_[0] and Pd[1] == Pf_[1]        # same limits as the fluid frame
+            assert np.array_equal(Pd[5:], P[5:])
+            v0, vp0, vperp0, g0 = _split(gcov, P)
+            v1, vp1, vperp1, g1 = _split(gcov, Pd)
+            assert np.abs(vperp1 - vperp0).max() <= 1e-13 * np.abs(v0).max()
+            # S_i B^i from the (separately pinned) conserved variables
+            U0 = kho.prim_to_flux(gcov, gcon, gdet, P, gam, 0)
+            U1 = kho.prim_to_flux(gcov, gcon, gdet, Pd, gam, 0)
+            sb0, sb1 = U0[2:5] @ P[5:8], U1[2:5] @ P[5:8]
+            scale = np.abs(U1[2:5] * P[5:8]).sum() + 1e-300
+            assert abs(sb1 - sb0) <= 1e-10 * scale, (sb0, sb1)
+            assert abs(vp1) <= abs(vp0) * (1 + 1e-12)                                 # heavier fluid moves slower along B
+            b0, b1 = kho.fourvec(gcov, gcon, P)["bsq"], kho.fourvec(gcov, gcon, Pd)["bsq"]
+            assert abs(b1 - b0) <= 1e-12 * b0
+            n += 1
+    assert n == 160
+
+
+def test_drift_frame_limits(kho):
+    gcov, gcon, gdet, x1, x2 = _geoms(kho)[2]
+    pd = _params(kho, True, kp.FRAME_DRIFT)
+    g3 = gcov[1:, 1:]
+    # no floor hit: identity
+    P = np.array([1.0, 0.1, 0.2, -0.1, 0.05, 1e-3, 2e-3, -1e-3])
+    Pd, f = kho.floors(pd, gcov, gcon, x1, x2, P)
+    assert f == 0 and np.array_equal(Pd, P)
+    # B = 0: velocity kept
+    P = np.array([1e-22, 1e-24, 0.2, -0.1, 0.05, 0, 0, 0.0])
+    Pd, f = kho.floors(pd, gcov, gcon, x1, x2, P)
+    assert f != 0 and np.array_equal(Pd[2:5], P[2:5])
+    # velocity perpendicular to B: nothing moves along the field, velocity kept
+    B = np.array([1e-3, 2e-3, -1e-3])
+    ut = np.array([0.3, -0.2, 0.1])
+    ut = ut - (ut @ g3 @ B) / (B @ g3 @ B) * B
+    P = np.concatenate([[1e-22, 1e-24], ut, B])
+    Pd, f = kho.floors(pd, gcov, gcon, x1, x2, P)
+    assert f != 0 and np.allclose(Pd[2:5], P[2:5], rtol=1e-12, atol=1e-16)
+    # velocity along B, mildly relativistic: w gamma^2 v conserved in closed form
+    ut = 0.5 * B / np.sqrt(B @ g3 @ B)
+    P = np.concatenate([[1e-22, 1e-24], ut, B])
+    Pd, f = kho.floors(pd, gcov, gcon, x1, x2, P)
+    gam = pd.gamma
+    w0, w1 = P[0] + gam * P[1], Pd[0] + gam * Pd[1]
+    q0, q1 = np.sqrt(P[2:5] @ g3 @ P[2:5]), np.sqrt(Pd[2:5] @ g3 @ Pd[2:5])
+    # w gamma^2 v = w gamma * q with q = gamma v
+    assert abs(w1 * np.sqrt(1 + q1 ** 2) * q1 - w0 * np.sqrt(1 + q0 ** 2) * q0) <= 1e-12 * w0 * q0
+
+
+def test_step_with_drift_frame_floors_runs_and_differs_only_where_floors_act(kho):
+    from kharm_inputs import torus
+    p = ki.config_params(3, n=(24, 16, 4))
+    P0 = torus.torus_state(p, seed=2)
+    out = []
+    for frame in (kp.FRAME_FLUID, kp.FRAME_DRIFT):
+        g = kho.Grid(dict(p, floor_frame=frame))
+        g.set_prims(P0)
+        g.debug_predictor(g.estimate_dt())            # one sub-step: zones without a floor hit are untouched by the frame
+        out.append((g.get_prims(), g.get_flags()))
+    (a, (pfa, ffa)), (b, (pfb, ffb)) = out
+    assert np.array_equal(pfa, pfb) and np.array_equal(ffa, ffb) and (ffa != 0).any() and (ffa == 0).any()
+    clean = (ffa == 0) & (pfa == 0)
+    assert np.array_equal(a[:, clean], b[:, clean])
+    assert np.array_equal(a[[0, 1, 5, 6, 7]], b[[0, 1, 5, 6, 7]])     # only the velocities differ
+    assert np.isfinite(b).all()
