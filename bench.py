@@ -42,6 +42,7 @@ WORKLOADS = {
     "torus_sane_192x128x128_mc": (3, None, 0),
     "torus_sane_192x128x128_weno5_kastaun": (3, None, None),      # same block, kh_params.inverter = KH_INV_KASTAUN
     "torus_sane_192x128x128_weno5_fofc": (3, None, None),         # same block, kh_params.fofc = 1
+    "torus_sane_192x128x128_weno5_drift": (3, None, None),        # same block, kh_params.floor_frame = KH_FRAME_DRIFT
     "minkowski_128_mc": (5, 128, 0), "minkowski_128_weno5": (5, 128, 1),
     "minkowski_256_mc": (5, 256, 0), "minkowski_256_weno5": (5, 256, 1),
     "minkowski_64_mc": (5, 64, 0), "minkowski_192_mc": (5, 192, 0), "minkowski_320_mc": (5, 320, 0),
@@ -92,6 +93,8 @@ def workload_params(name):
         p["inverter"] = ki.params.INV_KASTAUN
     if name.endswith("_fofc"):
         p["fofc"] = 1
+    if name.endswith("_drift"):
+        p["floor_frame"] = ki.params.FRAME_DRIFT
     return cfg, p
 
 

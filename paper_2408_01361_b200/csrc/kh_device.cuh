@@ -349,19 +349,69 @@ __device__ __forceinline__ int floor_limits(const FloorPar& fp, double rho_g, do
   return flag;
 }
 
+// Drift-frame injection (S26): after (rho, u) were moved to (rho', u'), the
+// normal observer's velocity v = ut/gamma keeps its part perpendicular to B (the E x B drift) and changes its part
+// along B so that the momentum along the field w gamma^2 v_par (w = rho + Gamma u) is conserved:
+//   A = w gamma^2 v_par / w',  v_par' = 2 A (1 - v_perp^2) / (1 + sqrt(1 + 4 A^2 (1 - v_perp^2))),  gamma'^2 = 1/(1 - v_perp^2 - v_par'^2).
+// B = 0: the velocity is kept.  Acts on the primitive velocities ut^i in place.
+template <bool FLAT>
+__device__ __forceinline__ void drift_frame_velocity(const Geo& G, double gam, double rho_old, double u_old, double rho_new, double u_new,
+                                                     double& ut1, double& ut2, double& ut3, double b1, double b2, double b3) {
+  double l1, l2, l3;
+  lower3<FLAT>(G, b1, b2, b3, l1, l2, l3);                               // B_i
+  const double Bsq = fma(b3, l3, fma(b2, l2, b1 * l1));
+  if (!(Bsq > 0.0)) return;
+  const double uB = fma(ut3, l3, fma(ut2, l2, ut1 * l1));                // ut^i B_i
+  const double qsq = spatial_norm2<FLAT>(G, ut1, ut2, ut3);
+  const double gsq = 1.0 + qsq, gamma = sqrt(gsq), iB = 1.0 / sqrt(Bsq), ig = 1.0 / gamma;
+  const double vpar = uB * ig * iB;
+  double omp = 1.0 - (qsq / gsq - vpar * vpar);                          // 1 - v_perp^2
+  if (omp > 1.0) omp = 1.0;
+  const double A = (fma(gam, u_old, rho_old) * gsq * vpar) / fma(gam, u_new, rho_new);
+  const double vpn = 2.0 * A * omp / (1.0 + sqrt(fma(4.0 * A * A, omp, 1.0)));
+  const double gn = 1.0 / sqrt(fma(-vpn, vpn, omp));
+  const double dv = (vpn - vpar) * iB;                                   // v' = v + (v_par' - v_par) B/|B|
+  ut1 = gn * fma(dv, b1, ut1 * ig);
+  ut2 = gn * fma(dv, b2, ut2 * ig);
+  ut3 = gn * fma(dv, b3, ut3 * ig);
+}
+
+// Limits, injection frame and Lorentz-factor ceiling on a state whose b^2 and gamma are known.  frame 0: fluid frame
+// (velocity untouched), 1: drift frame (the ceiling then acts on the adjusted velocity).
+template <bool FLAT>
+__device__ __forceinline__ int floors_in_frame(const Geo& G, const FloorPar& fp, int frame, double gam, double rho_g, double u_g, double bsq,
+                                               double gamma, double& rho, double& u, double& ut1, double& ut2, double& ut3, double b1,
+                                               double b2, double b3) {
+  double vfac;
+  if (frame == 0) {
+    const int flag = floor_limits(fp, rho_g, u_g, bsq, gamma, rho, u, vfac);
+    if (flag & 32) { ut1 *= vfac; ut2 *= vfac; ut3 *= vfac; }
+    return flag;
+  }
+  const double rho_old = rho, u_old = u;
+  int flag = floor_limits(fp, rho_g, u_g, bsq, 1.0, rho, u, vfac);       // limits only (gamma = 1 never trips the ceiling)
+  if (flag != 0) {
+    drift_frame_velocity<FLAT>(G, gam, rho_old, u_old, rho, u, ut1, ut2, ut3, b1, b2, b3);
+    gamma = sqrt(1.0 + spatial_norm2<FLAT>(G, ut1, ut2, ut3));
+  }
+  if (gamma > fp.gamma_max) {
+    vfac = sqrt((fp.gamma_max * fp.gamma_max - 1.0) / (gamma * gamma - 1.0));
+    ut1 *= vfac; ut2 *= vfac; ut3 *= vfac;
+    flag |= 32;
+  }
+  return flag;
+}
+
 // Floors of a primitive state (fix-up path): b^2 = (g_ij B^i B^j + (b^t)^2)/(u^t)^2 with b^t = B^i u_i.
 template <bool FLAT>
-__device__ __forceinline__ int apply_floors(const Geo& G, const FloorPar& fp, double rho_g, double u_g, double P[KH_NP]) {
+__device__ __forceinline__ int apply_floors(const Geo& G, const FloorPar& fp, int frame, double gam, double rho_g, double u_g, double P[KH_NP]) {
   double c1, c2, c3;
   lower3<FLAT>(G, P[U1], P[U2], P[U3], c1, c2, c3);
   double qsq = fma(P[U3], c3, fma(P[U2], c2, P[U1] * c1));
   double bt = fma(P[B3], c3, fma(P[B2], c2, P[B1] * c1));
   double BB = spatial_norm2<FLAT>(G, P[B1], P[B2], P[B3]);
   double bsq = fma(bt, bt, BB) / (-(1.0 + qsq) * G.n00);      // 1/(u^t)^2 = alpha^2/gamma^2 = -1/(gamma^2 g^tt)
-  double vfac;
-  int flag = floor_limits(fp, rho_g, u_g, bsq, sqrt(1.0 + qsq), P[RHO], P[UU], vfac);
-  if (flag & 32) { P[U1] *= vfac; P[U2] *= vfac; P[U3] *= vfac; }
-  return flag;
+  return floors_in_frame<FLAT>(G, fp, frame, gam, rho_g, u_g, bsq, sqrt(1.0 + qsq), P[RHO], P[UU], P[U1], P[U2], P[U3], P[B1], P[B2], P[B3]);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -374,7 +424,7 @@ __device__ __forceinline__ int apply_floors(const Geo& G, const FloorPar& fp, do
 // floors need no second pass through the four-vectors.
 // ---------------------------------------------------------------------------------------------
 template <bool FLAT>
-__device__ __forceinline__ int u_to_p_floors(const Geo& G, const double Uh[KH_NP], double W0, double gam, const FloorPar& fp,
+__device__ __forceinline__ int u_to_p_floors(const Geo& G, const double Uh[KH_NP], double W0, double gam, const FloorPar& fp, int frame,
                                              double rho_g, double u_g, double Pout[KH_NP], int& fflag) {
   fflag = 0;
   Pout[B1] = Uh[B1]; Pout[B2] = Uh[B2]; Pout[B3] = Uh[B3];
@@ -467,9 +517,7 @@ __device__ __forceinline__ int u_to_p_floors(const Geo& G, const double Uh[KH_NP
   if (badu) return 5;
   // floors (S18): b^2 and gamma of the recovered state from the conserved side
   double bsq = fma(Bsq, omv, QdotBsq * (iW * iW));
-  double vfac;
-  fflag = floor_limits(fp, rho_g, u_g, bsq, g, rho, u, vfac);
-  if (fflag & 32) { ut1 *= vfac; ut2 *= vfac; ut3 *= vfac; }
+  fflag = floors_in_frame<FLAT>(G, fp, frame, gam, rho_g, u_g, bsq, g, rho, u, ut1, ut2, ut3, Uh[B1], Uh[B2], Uh[B3]);
   Pout[RHO] = rho; Pout[UU] = u; Pout[U1] = ut1; Pout[U2] = ut2; Pout[U3] = ut3;
   return 0;
 }
@@ -534,8 +582,8 @@ __device__ __forceinline__ bool kastaun_root(const KastaunC& c, double a, double
 }
 
 template <bool FLAT>
-__device__ __forceinline__ int u_to_p_kastaun_floors(const Geo& G, const double Uh[KH_NP], double gam, const FloorPar& fp, double rho_g,
-                                                     double u_g, double Pout[KH_NP], int& fflag) {
+__device__ __forceinline__ int u_to_p_kastaun_floors(const Geo& G, const double Uh[KH_NP], double gam, const FloorPar& fp, int frame,
+                                                     double rho_g, double u_g, double Pout[KH_NP], int& fflag) {
   fflag = 0;
   Pout[B1] = Uh[B1]; Pout[B2] = Uh[B2]; Pout[B3] = Uh[B3];
   bool fin = true;
@@ -606,9 +654,7 @@ __device__ __forceinline__ int u_to_p_kastaun_floors(const Geo& G, const double 
   if (eps_raw < 0.0) return 5;
   // floors (S18): comoving b^2 = B^2 (1 - v^2) + (B_i v^i)^2 and the Lorentz factor W
   const double bsq = fma(Bsq, omv, msb * msb);
-  double vfac;
-  fflag = floor_limits(fp, rho_g, u_g, bsq, W, rho, u, vfac);
-  if (fflag & 32) { ut1 *= vfac; ut2 *= vfac; ut3 *= vfac; }
+  fflag = floors_in_frame<FLAT>(G, fp, frame, gam, rho_g, u_g, bsq, W, rho, u, ut1, ut2, ut3, Uh[B1], Uh[B2], Uh[B3]);
   Pout[RHO] = rho; Pout[UU] = u; Pout[U1] = ut1; Pout[U2] = ut2; Pout[U3] = ut3;
   return 0;
 }

@@ -36,6 +36,7 @@ struct GV {                 // grid view, passed by value
   const double* dg;         // source table, KH_NDG x n2d
   const double* floorp;
   FloorPar fp;
+  int floor_frame;          // 0 fluid, 1 drift (fix-up path; the update kernel has it as a template parameter)
 };
 
 struct StepScalars {        // device-resident scalars of the time stepping
@@ -277,7 +278,8 @@ emf_kernel(GV g, const double* __restrict__ F1, const double* __restrict__ F2, c
 // ~50 fp64 instructions instead of the 40-entry Gamma table and a 64-term contraction.
 // One thread per interior zone, flattened index (no idle lanes when n1 is not a multiple of the block).
 // ---------------------------------------------------------------------------------------------
-template <bool FLAT, bool CORR, int INV>
+// MODE = inverter (bit 0: 0 1D_W, 1 Kastaun) + 2 * floor frame (0 fluid, 1 drift)
+template <bool FLAT, bool CORR, int MODE>
 __global__ void __launch_bounds__(128, KH_MINB_UPDATE)
 update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps, double* __restrict__ Pf,
               const double* __restrict__ F1, const double* __restrict__ F2, const double* __restrict__ F3,
@@ -381,8 +383,8 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
     {
       const double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2);
       const double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
-      if (INV == 0) pf_flag = u_to_p_floors<FLAT>(G, Uh, W0, g.gam, g.fp, rho_g, u_g, pf, ff);
-      else pf_flag = u_to_p_kastaun_floors<FLAT>(G, Uh, g.gam, g.fp, rho_g, u_g, pf, ff);
+      if ((MODE & 1) == 0) pf_flag = u_to_p_floors<FLAT>(G, Uh, W0, g.gam, g.fp, MODE >> 1, rho_g, u_g, pf, ff);
+      else pf_flag = u_to_p_kastaun_floors<FLAT>(G, Uh, g.gam, g.fp, MODE >> 1, rho_g, u_g, pf, ff);
     }
     if (pf_flag != 0) {          // rare: the hydro primitives keep the guess (S16); queue the zone for the fix-up
 #pragma unroll
@@ -575,7 +577,7 @@ fixup_apply_kernel(GV g, double* __restrict__ Pf, const unsigned* __restrict__ l
     load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, p2);
     double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2);
     double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
-    int ff = apply_floors<FLAT>(G, g.fp, rho_g, u_g, P);
+    int ff = apply_floors<FLAT>(G, g.fp, g.floor_frame, g.gam, rho_g, u_g, P);
     fflag[n] |= (unsigned char)ff;
     // the zone and its ghost images (S20: copies; polar images flip ut^2)
     int i1[2 * KH_NGH + 1], i2[2 * KH_NGH + 1], i3[2 * KH_NGH + 1];

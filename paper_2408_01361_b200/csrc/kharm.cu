@@ -197,13 +197,14 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
   update_kernel<FL, CO, IN><<<grid, 128, 0, g->stream>>>(v, Pi, Ps, Pf, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], \
                                                          g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, g->fflag, g->faillist, g->sc, dt_factor)
     prof_begin(g, KH_K_UPDATE);
-    if (g->p.inverter == KH_INV_KASTAUN) {
-      if (g->flat) { if (corrector) UPD(true, true, 1); else UPD(true, false, 1); }
-      else { if (corrector) UPD(false, true, 1); else UPD(false, false, 1); }
-    } else {
-      if (g->flat) { if (corrector) UPD(true, true, 0); else UPD(true, false, 0); }
-      else { if (corrector) UPD(false, true, 0); else UPD(false, false, 0); }
+#define UPD2(FL, CO)                                                                 \
+    switch (g->p.inverter + 2 * g->p.floor_frame) {                                  \
+      case 0: UPD(FL, CO, 0); break; case 1: UPD(FL, CO, 1); break;                  \
+      case 2: UPD(FL, CO, 2); break; default: UPD(FL, CO, 3); break;                 \
     }
+    if (g->flat) { if (corrector) { UPD2(true, true) } else { UPD2(true, false) } }
+    else { if (corrector) { UPD2(false, true) } else { UPD2(false, false) } }
+#undef UPD2
     prof_end(g);
 #undef UPD
     g->launches++;
@@ -286,7 +287,7 @@ int kh_grid_destroy(kh_grid* g) {
 int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   if (!p || !out) return KH_EINVAL;
   if (p->n1 < 1 || p->n2 < 1 || p->n3 < 1) return KH_EINVAL;
-  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1 || p->inverter < 0 || p->inverter > 1 || p->fofc < 0 || p->fofc > 1) return KH_EINVAL;
+  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1 || p->inverter < 0 || p->inverter > 1 || p->fofc < 0 || p->fofc > 1 || p->floor_frame < 0 || p->floor_frame > 1) return KH_EINVAL;
   if (!(p->gamma > 1.0) || !(p->cfl > 0.0) || !(p->dt_growth_max > 0.0)) return KH_EINVAL;
   const int N[3] = {p->n1, p->n2, p->n3};
   for (int d = 0; d < 3; d++) {
@@ -343,6 +344,7 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   v.ndim_mask = (v.n1 > 1 ? 1 : 0) | (v.n2 > 1 ? 2 : 0) | (v.n3 > 1 ? 4 : 0);
   v.fp.inv_bsq_over_rho_max = 1.0 / p->bsq_over_rho_max; v.fp.inv_bsq_over_u_max = 1.0 / p->bsq_over_u_max;
   v.fp.u_over_rho_max = p->u_over_rho_max; v.fp.gamma_max = p->gamma_max;
+  v.floor_frame = p->floor_frame;
 
 #define ALLOC(ptr, bytes)                                                       \
   do {                                                                          \

@@ -360,3 +360,43 @@ def test_fofc_run_l1_and_untroubled_bit_identity(kh, kho):
             d = g.step(d)
         res.append((g.get_prims(), d))
     assert np.array_equal(res[0][0], res[1][0]) and res[0][1] == res[1][1]
+
+
+# ------------------------------------------------------------------------------------------ drift-frame floors (NEXT-4)
+@pytest.mark.parametrize("case", ["torus_weno5", "mad_stress_mc", "bondi", "torus_kastaun_fofc"])
+def test_one_step_drift_frame_floors(kh, kho, case):
+    """kh_params.floor_frame = KH_FRAME_DRIFT on both sides: same bars."""
+    if case == "torus_weno5":
+        p = ki.config_params(3, n=(64, 48, 8)); P0 = torus.torus_state(p, seed=2); gh = False
+    elif case == "mad_stress_mc":
+        p = ki.config_params(4, n=(72, 40, 8)); P0 = torus.torus_state(p, mad=True, seed=3, stress=True, stress_fraction=0.02); gh = False
+    elif case == "bondi":
+        p = ki.config_params(2); P0 = bondi.config2(p); gh = True
+    else:
+        p = dict(ki.config_params(3, n=(33, 17, 3)), inverter=kp.INV_KASTAUN, fofc=1); P0 = torus.torus_state(p, seed=2); gh = False
+    p = dict(p, floor_frame=kp.FRAME_DRIFT)
+    worst, gg, go = _one_step_case(kh, kho, p, P0, with_ghosts=gh, label="drift " + case)
+    if case != "bondi":
+        assert (go.get_flags()[1] != 0).any()          # floors really acted
+
+
+def test_drift_frame_run_l1_and_fixup_hook(kh, kho):
+    p = dict(ki.config_params(3, n=(48, 32, 8)), floor_frame=kp.FRAME_DRIFT)
+    gg, go = _both(kh, kho, p, torus.torus_state(p, seed=1))
+    dt = go.estimate_dt()
+    for _ in range(10):
+        dg, dt = gg.step(dt), go.step(dt)
+        assert abs(dg / dt - 1) < 1e-9
+    l1 = l1_diff(p, gg.get_prims(), go.get_prims())
+    assert l1.max() <= TOL_RUN_L1, l1
+    # fix-up hook: the floors after the repair also run in the drift frame
+    p = dict(ki.config_params(3, n=(20, 16, 6)), floor_frame=kp.FRAME_DRIFT)
+    P0 = torus.torus_state(p, seed=1)
+    gg, go = _both(kh, kho, p, P0)
+    rng = np.random.default_rng(0)
+    pf = np.zeros((p["n3"] + 6, p["n2"] + 6, p["n1"] + 6), dtype=np.int32)
+    pf[3:-3, 3:-3, 3:-3] = (rng.uniform(size=(p["n3"], p["n2"], p["n1"])) < 0.1) * 3
+    gg.debug_fixup(pf); go.debug_fixup(pf)
+    a, b = gg.get_prims(), go.get_prims()          # interior (the oracle's hook stops before the ghost refresh)
+    assert np.allclose(a, b, rtol=1e-11, atol=1e-300)
+    assert np.array_equal(gg.get_flags()[1], go.get_flags()[1])
