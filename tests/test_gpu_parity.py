@@ -400,3 +400,30 @@ def test_drift_frame_run_l1_and_fixup_hook(kh, kho):
     a, b = gg.get_prims(), go.get_prims()          # interior (the oracle's hook stops before the ghost refresh)
     assert np.allclose(a, b, rtol=1e-11, atol=1e-300)
     assert np.array_equal(gg.get_flags()[1], go.get_flags()[1])
+
+
+# ------------------------------------------------------------------------------------------ the configs' own step counts
+@pytest.mark.parametrize("cfg,n", [(3, (96, 64, 32)), (4, (96, 48, 24)), (2, None)])
+def test_hundred_step_runs_l1(kh, kho, cfg, n):
+    """BASELINE configs 3 and 4 ask for 100 steps (config 2: the first 100 steps of the Bondi run): L1 difference per
+    primitive <= 1e-8 at the end, flags identical, div B at round-off -- at reduced resolution, device-resident dt.
+    (Bondi: the zones at the inner edge, inside the horizon, are not steady in this scheme -- both sides show the same 30 %
+    density excursion there -- and amplify a round-off difference by ~100 every 20 steps from step ~120 on, so a longer
+    run compares two valid realisations of an unstable boundary layer, not two implementations.)"""
+    if cfg == 2:
+        p = ki.config_params(2); P0 = bondi.config2(p); gh, nsteps = True, 100
+    else:
+        p = ki.config_params(cfg, n=n); P0 = torus.torus_state(p, mad=(cfg == 4), seed=1); gh, nsteps = False, 100
+    gg, go = _both(kh, kho, p, P0, with_ghosts=gh)
+    dt = go.estimate_dt()
+    gg.step(dt, sync=False)
+    for _ in range(nsteps - 1):
+        gg.step(-1.0, sync=False)               # CUDA-graph replay, dt stays on the device
+    for _ in range(nsteps):
+        dt = go.step(dt)
+    a, b = gg.get_prims(), go.get_prims()
+    l1 = l1_diff(p, a, b)
+    assert (l1 <= TOL_RUN_L1).all(), l1
+    assert np.array_equal(gg.get_flags()[0], go.get_flags()[0])
+    d_g, d_o = gg.divB(), go.divB()
+    assert d_g <= 4 * d_o + 1e-12
