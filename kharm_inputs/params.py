@@ -12,7 +12,7 @@ MINKOWSKI, KS, FMKS = 0, 1, 2
 BC_PERIODIC, BC_OUTFLOW, BC_POLAR, BC_FIXED = 0, 1, 2, 3
 RECON_MC, RECON_WENO5 = 0, 1
 INV_1DW, INV_KASTAUN = 0, 1
-FRAME_FLUID, FRAME_DRIFT = 0, 1
+FRAME_FLUID, FRAME_DRIFT, FRAME_NORMAL = 0, 1, 2
 
 FLOOR_DEFAULTS = dict(rho_min=1e-6, u_min=1e-8, r_char=10.0, bsq_over_rho_max=100.0, bsq_over_u_max=1e4,
                       u_over_rho_max=100.0, gamma_max=50.0, dt_growth_max=1.3)

@@ -651,7 +651,45 @@ void drift_frame_velocity(const Geom& G, double gam, double rho_old, double u_ol
   for (int i = 0; i < 3; i++) P[U1 + i] = gamma_new * (vperp[i] + vpar_new * P[B1 + i] / B);
 }
 
+int floors(const kho_params& p, const Geom& G, double r, double P[NP]);
+
+// p.floor_frame = KHO_FRAME_NORMAL ("any of a number of different frames"; SURVEY 8(f) NEXT-4;
+// reading S27): the floor material (rho_inj, u_inj) = (max(rho_fl - rho, 0), max(u_fl - u, 0)) is added AT REST IN THE
+// NORMAL OBSERVER'S FRAME, i.e. as conserved variables: with u^mu = n^mu the added gas has T^t_i = 0 and
+//   U_add = sqrt(-g) ( rho_inj/alpha,  -(rho_inj + u_inj) + rho_inj/alpha,  0, 0, 0,  0, 0, 0 ),
+// so the momentum density is untouched; the primitives follow from inverting U(P) + U_add (guess: the fluid-frame
+// result), and the fluid-frame limits and ceilings then act once more on them.  If that inversion fails the fluid-frame
+// result is kept (fflag bit 64).
+int floors_normal_frame(const kho_params& p, const Geom& G, double r, double P[NP]) {
+  kho_params pf = p;
+  pf.floor_frame = KHO_FRAME_FLUID;
+  double P0[NP];
+  for (int v = 0; v < NP; v++) P0[v] = P[v];
+  // the limits, as in the fluid frame
+  double s = (p.coords == KHO_MINKOWSKI) ? 1.0 : 1.0 / (r * r) / (1.0 + r / p.r_char);
+  FourVec D;
+  four_vectors(G.gcov, G.gcon, P0, D);
+  double rho_g = p.rho_min * s, rho_b = D.bsq / p.bsq_over_rho_max;
+  double u_g = p.u_min * std::pow(s, p.gamma), u_b = D.bsq / p.bsq_over_u_max;
+  double rho_fl = rho_b > rho_g ? rho_b : rho_g, u_fl = u_b > u_g ? u_b : u_g;
+  double rho_inj = rho_fl > P0[RHO] ? rho_fl - P0[RHO] : 0.0;
+  double u_inj = u_fl > P0[UU] ? u_fl - P0[UU] : 0.0;
+  int flag = floors(pf, G, r, P);                       // provisional: the fluid-frame result
+  if (!(rho_inj > 0.0) && !(u_inj > 0.0)) return flag;
+  double U[NP];
+  prim_to_flux(G, P0, D, p.gamma, 0, U);
+  U[RHO] += G.gdet * (rho_inj / G.alpha);
+  U[UU] += G.gdet * (-(rho_inj + u_inj) + rho_inj / G.alpha);
+  double Pn[NP];
+  int pfl = (p.inverter == KHO_INV_KASTAUN) ? u2p_kastaun(G, U, P, p.gamma, Pn) : u2p(G, U, P, p.gamma, Pn);
+  if (pfl != 0) return flag | 64;
+  int flag2 = floors(pf, G, r, Pn);
+  for (int v = 0; v < NP; v++) P[v] = Pn[v];
+  return (flag & 15) | flag2;
+}
+
 int floors(const kho_params& p, const Geom& G, double r, double P[NP]) {
+  if (p.floor_frame == KHO_FRAME_NORMAL) return floors_normal_frame(p, G, r, P);
   int flag = 0;
   double s = (p.coords == KHO_MINKOWSKI) ? 1.0 : 1.0 / (r * r) / (1.0 + r / p.r_char);
   FourVec D;

@@ -25,7 +25,7 @@ enum { KHO_MINKOWSKI = 0, KHO_KS = 1, KHO_FMKS = 2 };
 enum { KHO_BC_PERIODIC = 0, KHO_BC_OUTFLOW = 1, KHO_BC_POLAR = 2, KHO_BC_FIXED = 3 };
 enum { KHO_RECON_MC = 0, KHO_RECON_WENO5 = 1 };
 enum { KHO_INV_1DW = 0, KHO_INV_KASTAUN = 1 };
-enum { KHO_FRAME_FLUID = 0, KHO_FRAME_DRIFT = 1 };
+enum { KHO_FRAME_FLUID = 0, KHO_FRAME_DRIFT = 1, KHO_FRAME_NORMAL = 2 };
 enum { KHO_LOC_CENT = 0, KHO_LOC_FACE1 = 1, KHO_LOC_FACE2 = 2, KHO_LOC_FACE3 = 3 };
 
 typedef struct {
@@ -41,7 +41,7 @@ typedef struct {
   double dt_growth_max;
   int inverter;                                    /* KHO_INV_1DW | KHO_INV_KASTAUN (NEXT-2) */
   int fofc;                                        /* 1: first-order flux correction (NEXT-3) */
-  int floor_frame;                                 /* KHO_FRAME_FLUID | KHO_FRAME_DRIFT (NEXT-4) */
+  int floor_frame;                                 /* KHO_FRAME_FLUID | _DRIFT | _NORMAL (NEXT-4) */
 } kho_params;
 
 typedef struct kho_grid kho_grid;

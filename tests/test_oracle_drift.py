@@ -120,3 +120,51 @@ def test_step_with_drift_frame_floors_runs_and_differs_only_where_floors_act(kho
     assert np.array_equal(a[:, clean], b[:, clean])
     assert np.array_equal(a[[0, 1, 5, 6, 7]], b[[0, 1, 5, 6, 7]])     # only the velocities differ
     assert np.isfinite(b).all()
+
+
+# ------------------------------------------------------------------------------------------ normal-observer frame (S27)
+def test_normal_frame_injection_conserves_momentum_and_adds_exactly_the_floor_material(kho):
+    """The added gas is at rest for the normal observer: T^t_i of it vanishes, so S_i is unchanged, the conserved
+    density grows by sqrt(-g) rho_inj/alpha and the energy slot by sqrt(-g)(-(rho_inj + u_inj) + rho_inj/alpha)."""
+    rng = np.random.default_rng(13)
+    n = 0
+    for gi, (gcov, gcon, gdet, x1, x2) in enumerate(_geoms(kho)):
+        pn, pf = _params(kho, gi > 0, kp.FRAME_NORMAL), _params(kho, gi > 0, kp.FRAME_FLUID)
+        gam = pn.gamma
+        alpha = 1.0 / np.sqrt(-gcon[0, 0])
+        for _ in range(30):
+            P = np.zeros(8)
+            Pfl, _ = kho.floors(pf, gcov, gcon, x1, x2, np.array([1e-30, 1e-32, 0, 0, 0, 0, 0, 0.0]))   # the geometric floors here
+            P[0] = Pfl[0] * 10 ** rng.uniform(-2, -0.3)            # below the floor by a modest factor
+            P[1] = Pfl[1] * 10 ** rng.uniform(-2, -0.3)
+            for i in range(3):
+                P[2 + i] = rng.normal() * 0.3 / np.sqrt(gcov[i + 1, i + 1])
+                P[5 + i] = rng.normal() * 1e-3 * np.sqrt(P[0]) / np.sqrt(gcov[i + 1, i + 1])
+            Pn, fn = kho.floors(pn, gcov, gcon, x1, x2, P)
+            Pf_, ff = kho.floors(pf, gcov, gcon, x1, x2, P)
+            assert fn != 0 and not (fn & 64)
+            if (fn & ~15) or (fn != ff):
+                continue                                           # a second-pass limit acted: conservation is not exact then
+            U0 = kho.prim_to_flux(gcov, gcon, 1.0, P, gam, 0)      # the pointwise floors call uses sqrt(-g) = 1
+            U1 = kho.prim_to_flux(gcov, gcon, 1.0, Pn, gam, 0)
+            rho_inj, u_inj = Pf_[0] - P[0], Pf_[1] - P[1]
+            assert rho_inj > 0 and u_inj > 0
+            scale = np.abs(U1[:5]).max()
+            assert np.abs(U1[2:5] - U0[2:5]).max() <= 1e-11 * scale                      # momentum density untouched
+            assert abs((U1[0] - U0[0]) - rho_inj / alpha) <= 1e-11 * scale
+            assert abs((U1[1] - U0[1]) - (-(rho_inj + u_inj) + rho_inj / alpha)) <= 1e-11 * scale
+            assert np.array_equal(Pn[5:], P[5:])
+            n += 1
+    assert n > 60
+
+
+def test_normal_frame_static_fluid_equals_fluid_frame_in_flat_space(kho):
+    pn, pf = _params(kho, False, kp.FRAME_NORMAL), _params(kho, False, kp.FRAME_FLUID)
+    P = np.array([1e-9, 1e-12, 0, 0, 0, 1e-6, 0, 0.0])
+    a, fa = kho.floors(pn, ETA, ETA, 0.5, 0.5, P)
+    b, fb = kho.floors(pf, ETA, ETA, 0.5, 0.5, P)
+    assert fa == fb and np.allclose(a, b, rtol=1e-12, atol=1e-300)
+    # moving fluid: the injected gas carries no momentum, so the velocity drops by about w_old/w_new
+    P = np.array([1e-9, 1e-12, 0.1, 0, 0, 0, 0, 0.0])
+    a, fa = kho.floors(pn, ETA, ETA, 0.5, 0.5, P)
+    assert 0 < a[2] < 0.1 * 2e-3 and a[0] >= 1e-6
