@@ -38,7 +38,7 @@ enum { KH_MINKOWSKI = 0, KH_KS = 1, KH_FMKS = 2 };                            /*
 enum { KH_BC_PERIODIC = 0, KH_BC_OUTFLOW = 1, KH_BC_POLAR = 2, KH_BC_FIXED = 3 };
 enum { KH_RECON_MC = 0, KH_RECON_WENO5 = 1 };                                 /* P:253           */
 enum { KH_INV_1DW = 0, KH_INV_KASTAUN = 1 };
-enum { KH_FRAME_FLUID = 0, KH_FRAME_DRIFT = 1 };
+enum { KH_FRAME_FLUID = 0, KH_FRAME_DRIFT = 1, KH_FRAME_NORMAL = 2 };
 enum { KH_MEM_DEVICE = 0, KH_MEM_HOST = 1 };
 enum { KH_LOC_CENT = 0, KH_LOC_FACE1 = 1, KH_LOC_FACE2 = 2, KH_LOC_FACE3 = 3 };
 
@@ -59,7 +59,8 @@ typedef struct {
   int fofc;                   /* 1: first-order flux correction: a speculative update finds the zones
                                  that would fail the inversion or hit a floor; their faces get donor-cell LLF fluxes */
   int floor_frame;            /* frame the floor material is injected in: KH_FRAME_FLUID (velocity
-                                 untouched) | KH_FRAME_DRIFT (E x B drift velocity kept, momentum along B conserved) */
+                                 untouched) | KH_FRAME_DRIFT (E x B drift velocity kept, momentum along B conserved) |
+                                 KH_FRAME_NORMAL (added as gas at rest for the normal observer, then re-inverted)   */
 } kh_params;
 
 typedef struct kh_grid kh_grid;   /* opaque */

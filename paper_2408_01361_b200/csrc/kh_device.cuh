@@ -332,13 +332,14 @@ struct FloorPar {
 // Limits on (rho, u) and the Lorentz-factor ceiling given b^2 and gamma of the state; returns the fflag bits and
 // the factor (1 = none) by which the caller scales ut^i.
 __device__ __forceinline__ int floor_limits(const FloorPar& fp, double rho_g, double u_g, double bsq, double gamma, double& rho,
-                                            double& u, double& vfac) {
+                                            double& u, double& vfac, double inj[2]) {
   int flag = 0;
   double rho_b = bsq * fp.inv_bsq_over_rho_max, u_b = bsq * fp.inv_bsq_over_u_max;
   double rho_fl = rho_b > rho_g ? rho_b : rho_g;
   double u_fl = u_b > u_g ? u_b : u_g;
-  if (rho < rho_fl) { rho = rho_fl; flag |= (rho_b > rho_g) ? 2 : 1; }
-  if (u < u_fl) { u = u_fl; flag |= (u_b > u_g) ? 8 : 4; }
+  inj[0] = inj[1] = 0.0;                      // floor material (rho_inj, u_inj): used by the normal-frame injection only
+  if (rho < rho_fl) { inj[0] = rho_fl - rho; rho = rho_fl; flag |= (rho_b > rho_g) ? 2 : 1; }
+  if (u < u_fl) { inj[1] = u_fl - u; u = u_fl; flag |= (u_b > u_g) ? 8 : 4; }
   double ucap = fp.u_over_rho_max * rho;
   if (u > ucap) { u = ucap; flag |= 16; }
   vfac = 1.0;
@@ -381,15 +382,15 @@ __device__ __forceinline__ void drift_frame_velocity(const Geo& G, double gam, d
 template <bool FLAT>
 __device__ __forceinline__ int floors_in_frame(const Geo& G, const FloorPar& fp, int frame, double gam, double rho_g, double u_g, double bsq,
                                                double gamma, double& rho, double& u, double& ut1, double& ut2, double& ut3, double b1,
-                                               double b2, double b3) {
+                                               double b2, double b3, double inj[2]) {
   double vfac;
-  if (frame == 0) {
-    const int flag = floor_limits(fp, rho_g, u_g, bsq, gamma, rho, u, vfac);
+  if (frame != 1) {                            // fluid frame; the normal frame starts from the same provisional result
+    const int flag = floor_limits(fp, rho_g, u_g, bsq, gamma, rho, u, vfac, inj);
     if (flag & 32) { ut1 *= vfac; ut2 *= vfac; ut3 *= vfac; }
     return flag;
   }
   const double rho_old = rho, u_old = u;
-  int flag = floor_limits(fp, rho_g, u_g, bsq, 1.0, rho, u, vfac);       // limits only (gamma = 1 never trips the ceiling)
+  int flag = floor_limits(fp, rho_g, u_g, bsq, 1.0, rho, u, vfac, inj);  // limits only (gamma = 1 never trips the ceiling)
   if (flag != 0) {
     drift_frame_velocity<FLAT>(G, gam, rho_old, u_old, rho, u, ut1, ut2, ut3, b1, b2, b3);
     gamma = sqrt(1.0 + spatial_norm2<FLAT>(G, ut1, ut2, ut3));
@@ -404,14 +405,15 @@ __device__ __forceinline__ int floors_in_frame(const Geo& G, const FloorPar& fp,
 
 // Floors of a primitive state (fix-up path): b^2 = (g_ij B^i B^j + (b^t)^2)/(u^t)^2 with b^t = B^i u_i.
 template <bool FLAT>
-__device__ __forceinline__ int apply_floors(const Geo& G, const FloorPar& fp, int frame, double gam, double rho_g, double u_g, double P[KH_NP]) {
+__device__ __forceinline__ int apply_floors(const Geo& G, const FloorPar& fp, int frame, double gam, double rho_g, double u_g, double P[KH_NP],
+                                            double inj[2]) {
   double c1, c2, c3;
   lower3<FLAT>(G, P[U1], P[U2], P[U3], c1, c2, c3);
   double qsq = fma(P[U3], c3, fma(P[U2], c2, P[U1] * c1));
   double bt = fma(P[B3], c3, fma(P[B2], c2, P[B1] * c1));
   double BB = spatial_norm2<FLAT>(G, P[B1], P[B2], P[B3]);
   double bsq = fma(bt, bt, BB) / (-(1.0 + qsq) * G.n00);      // 1/(u^t)^2 = alpha^2/gamma^2 = -1/(gamma^2 g^tt)
-  return floors_in_frame<FLAT>(G, fp, frame, gam, rho_g, u_g, bsq, sqrt(1.0 + qsq), P[RHO], P[UU], P[U1], P[U2], P[U3], P[B1], P[B2], P[B3]);
+  return floors_in_frame<FLAT>(G, fp, frame, gam, rho_g, u_g, bsq, sqrt(1.0 + qsq), P[RHO], P[UU], P[U1], P[U2], P[U3], P[B1], P[B2], P[B3], inj);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -425,7 +427,7 @@ __device__ __forceinline__ int apply_floors(const Geo& G, const FloorPar& fp, in
 // ---------------------------------------------------------------------------------------------
 template <bool FLAT>
 __device__ __forceinline__ int u_to_p_floors(const Geo& G, const double Uh[KH_NP], double W0, double gam, const FloorPar& fp, int frame,
-                                             double rho_g, double u_g, double Pout[KH_NP], int& fflag) {
+                                             double rho_g, double u_g, double Pout[KH_NP], int& fflag, double inj[2]) {
   fflag = 0;
   Pout[B1] = Uh[B1]; Pout[B2] = Uh[B2]; Pout[B3] = Uh[B3];
   bool fin = true;
@@ -517,7 +519,7 @@ __device__ __forceinline__ int u_to_p_floors(const Geo& G, const double Uh[KH_NP
   if (badu) return 5;
   // floors (S18): b^2 and gamma of the recovered state from the conserved side
   double bsq = fma(Bsq, omv, QdotBsq * (iW * iW));
-  fflag = floors_in_frame<FLAT>(G, fp, frame, gam, rho_g, u_g, bsq, g, rho, u, ut1, ut2, ut3, Uh[B1], Uh[B2], Uh[B3]);
+  fflag = floors_in_frame<FLAT>(G, fp, frame, gam, rho_g, u_g, bsq, g, rho, u, ut1, ut2, ut3, Uh[B1], Uh[B2], Uh[B3], inj);
   Pout[RHO] = rho; Pout[UU] = u; Pout[U1] = ut1; Pout[U2] = ut2; Pout[U3] = ut3;
   return 0;
 }
@@ -583,7 +585,7 @@ __device__ __forceinline__ bool kastaun_root(const KastaunC& c, double a, double
 
 template <bool FLAT>
 __device__ __forceinline__ int u_to_p_kastaun_floors(const Geo& G, const double Uh[KH_NP], double gam, const FloorPar& fp, int frame,
-                                                     double rho_g, double u_g, double Pout[KH_NP], int& fflag) {
+                                                     double rho_g, double u_g, double Pout[KH_NP], int& fflag, double inj[2]) {
   fflag = 0;
   Pout[B1] = Uh[B1]; Pout[B2] = Uh[B2]; Pout[B3] = Uh[B3];
   bool fin = true;
@@ -654,8 +656,44 @@ __device__ __forceinline__ int u_to_p_kastaun_floors(const Geo& G, const double 
   if (eps_raw < 0.0) return 5;
   // floors (S18): comoving b^2 = B^2 (1 - v^2) + (B_i v^i)^2 and the Lorentz factor W
   const double bsq = fma(Bsq, omv, msb * msb);
-  fflag = floors_in_frame<FLAT>(G, fp, frame, gam, rho_g, u_g, bsq, W, rho, u, ut1, ut2, ut3, Uh[B1], Uh[B2], Uh[B3]);
+  fflag = floors_in_frame<FLAT>(G, fp, frame, gam, rho_g, u_g, bsq, W, rho, u, ut1, ut2, ut3, Uh[B1], Uh[B2], Uh[B3], inj);
   Pout[RHO] = rho; Pout[UU] = u; Pout[U1] = ut1; Pout[U2] = ut2; Pout[U3] = ut3;
+  return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Inversion + floors with the injection frame resolved.  INVERTER: 0 1D_W, 1 Kastaun.  Frame 2 (normal observer, S27):
+// the floor material enters as conserved variables of a gas at rest for the normal observer,
+//   U_add/sqrt(-g) = (rho_inj/alpha, -(rho_inj + u_inj) + rho_inj/alpha, 0, 0, 0), and the sum is inverted again (guess: the
+// fluid-frame result; the fluid-frame limits and ceilings act on the new state).  A failed re-inversion keeps the
+// fluid-frame result and sets fflag bit 64.
+// ---------------------------------------------------------------------------------------------
+template <bool FLAT, int INVERTER>
+__device__ __forceinline__ int invert_any(const Geo& G, const double Uh[KH_NP], double W0, double gam, const FloorPar& fp, int frame,
+                                          double rho_g, double u_g, double Pout[KH_NP], int& fflag, double inj[2]) {
+  if (INVERTER == 0) return u_to_p_floors<FLAT>(G, Uh, W0, gam, fp, frame, rho_g, u_g, Pout, fflag, inj);
+  return u_to_p_kastaun_floors<FLAT>(G, Uh, gam, fp, frame, rho_g, u_g, Pout, fflag, inj);
+}
+
+template <bool FLAT, int INVERTER>
+__device__ __forceinline__ int invert_with_floors(const Geo& G, const double Uh[KH_NP], double W0, double gam, const FloorPar& fp, int frame,
+                                                  double rho_g, double u_g, double Pout[KH_NP], int& fflag) {
+  double inj[2];
+  const int pflag = invert_any<FLAT, INVERTER>(G, Uh, W0, gam, fp, frame, rho_g, u_g, Pout, fflag, inj);
+  if (frame != 2 || pflag != 0 || !(inj[0] > 0.0 || inj[1] > 0.0)) return pflag;
+  const double ialpha = FLAT ? 1.0 : -G.n00 * G.alpha;
+  double Ub[KH_NP], Pb[KH_NP], inj2[2];
+#pragma unroll
+  for (int v = 0; v < KH_NP; v++) Ub[v] = Uh[v];
+  Ub[RHO] = fma(inj[0], ialpha, Ub[RHO]);
+  Ub[UU] += fma(inj[0], ialpha, -(inj[0] + inj[1]));
+  const double W0b = fma(gam, Pout[UU], Pout[RHO]) * (1.0 + spatial_norm2<FLAT>(G, Pout[U1], Pout[U2], Pout[U3]));
+  int ff2;
+  const int p2 = invert_any<FLAT, INVERTER>(G, Ub, W0b, gam, fp, 0, rho_g, u_g, Pb, ff2, inj2);
+  if (p2 != 0) { fflag |= 64; return 0; }
+#pragma unroll
+  for (int v = 0; v < 5; v++) Pout[v] = Pb[v];
+  fflag = (fflag & 15) | ff2;
   return 0;
 }
 

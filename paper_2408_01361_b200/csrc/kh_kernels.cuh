@@ -36,7 +36,8 @@ struct GV {                 // grid view, passed by value
   const double* dg;         // source table, KH_NDG x n2d
   const double* floorp;
   FloorPar fp;
-  int floor_frame;          // 0 fluid, 1 drift (fix-up path; the update kernel has it as a template parameter)
+  int floor_frame;          // 0 fluid, 1 drift, 2 normal observer (fix-up path; the update kernel has it as a template parameter)
+  int inverter;             // 0 1D_W, 1 Kastaun (fix-up path with normal-frame floors)
 };
 
 struct StepScalars {        // device-resident scalars of the time stepping
@@ -278,7 +279,7 @@ emf_kernel(GV g, const double* __restrict__ F1, const double* __restrict__ F2, c
 // ~50 fp64 instructions instead of the 40-entry Gamma table and a 64-term contraction.
 // One thread per interior zone, flattened index (no idle lanes when n1 is not a multiple of the block).
 // ---------------------------------------------------------------------------------------------
-// MODE = inverter (bit 0: 0 1D_W, 1 Kastaun) + 2 * floor frame (0 fluid, 1 drift)
+// MODE = inverter (bit 0: 0 1D_W, 1 Kastaun) + 2 * floor frame (0 fluid, 1 drift, 2 normal observer)
 template <bool FLAT, bool CORR, int MODE>
 __global__ void __launch_bounds__(128, KH_MINB_UPDATE)
 update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps, double* __restrict__ Pf,
@@ -383,8 +384,7 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
     {
       const double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2);
       const double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
-      if ((MODE & 1) == 0) pf_flag = u_to_p_floors<FLAT>(G, Uh, W0, g.gam, g.fp, MODE >> 1, rho_g, u_g, pf, ff);
-      else pf_flag = u_to_p_kastaun_floors<FLAT>(G, Uh, g.gam, g.fp, MODE >> 1, rho_g, u_g, pf, ff);
+      pf_flag = invert_with_floors<FLAT, MODE & 1>(G, Uh, W0, g.gam, g.fp, MODE >> 1, rho_g, u_g, pf, ff);
     }
     if (pf_flag != 0) {          // rare: the hydro primitives keep the guess (S16); queue the zone for the fix-up
 #pragma unroll
@@ -577,7 +577,32 @@ fixup_apply_kernel(GV g, double* __restrict__ Pf, const unsigned* __restrict__ l
     load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, p2);
     double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2);
     double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
-    int ff = apply_floors<FLAT>(G, g.fp, g.floor_frame, g.gam, rho_g, u_g, P);
+    double inj[2];
+    double P0[KH_NP];
+#pragma unroll
+    for (int v = 0; v < KH_NP; v++) P0[v] = P[v];
+    int ff = apply_floors<FLAT>(G, g.fp, g.floor_frame, g.gam, rho_g, u_g, P, inj);
+    if (g.floor_frame == 2 && (inj[0] > 0.0 || inj[1] > 0.0)) {      // normal-frame injection (S27): conserved variables of P0 + floor material
+      const double ialpha = FLAT ? 1.0 : -G.n00 * G.alpha;
+      FourVec D;
+      four_vectors<FLAT>(G, ialpha, P0, D);
+      const double ee = fma(g.gam, P0[UU], P0[RHO]) + D.bsq, ptot = fma(0.5, D.bsq, (g.gam - 1.0) * P0[UU]);
+      const double eu[4] = {ee * D.ucov[0], ee * D.ucov[1], ee * D.ucov[2], ee * D.ucov[3]};
+      double Uh[KH_NP], Pb[KH_NP], inj2[2];
+      flux_row(P0, D, eu, ptot, 0, Uh);
+      Uh[RHO] = fma(inj[0], ialpha, Uh[RHO]);
+      Uh[UU] += fma(inj[0], ialpha, -(inj[0] + inj[1]));
+      const double W0b = fma(g.gam, P[UU], P[RHO]) * (1.0 + spatial_norm2<FLAT>(G, P[U1], P[U2], P[U3]));
+      int ff2;
+      const int p2 = g.inverter ? invert_any<FLAT, 1>(G, Uh, W0b, g.gam, g.fp, 0, rho_g, u_g, Pb, ff2, inj2)
+                                : invert_any<FLAT, 0>(G, Uh, W0b, g.gam, g.fp, 0, rho_g, u_g, Pb, ff2, inj2);
+      if (p2 != 0) ff |= 64;
+      else {
+#pragma unroll
+        for (int v = 0; v < 5; v++) P[v] = Pb[v];
+        ff = (ff & 15) | ff2;
+      }
+    }
     fflag[n] |= (unsigned char)ff;
     // the zone and its ghost images (S20: copies; polar images flip ut^2)
     int i1[2 * KH_NGH + 1], i2[2 * KH_NGH + 1], i3[2 * KH_NGH + 1];

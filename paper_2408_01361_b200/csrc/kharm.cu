@@ -200,7 +200,8 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
 #define UPD2(FL, CO)                                                                 \
     switch (g->p.inverter + 2 * g->p.floor_frame) {                                  \
       case 0: UPD(FL, CO, 0); break; case 1: UPD(FL, CO, 1); break;                  \
-      case 2: UPD(FL, CO, 2); break; default: UPD(FL, CO, 3); break;                 \
+      case 2: UPD(FL, CO, 2); break; case 3: UPD(FL, CO, 3); break;                  \
+      case 4: UPD(FL, CO, 4); break; default: UPD(FL, CO, 5); break;                 \
     }
     if (g->flat) { if (corrector) { UPD2(true, true) } else { UPD2(true, false) } }
     else { if (corrector) { UPD2(false, true) } else { UPD2(false, false) } }
@@ -287,7 +288,7 @@ int kh_grid_destroy(kh_grid* g) {
 int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   if (!p || !out) return KH_EINVAL;
   if (p->n1 < 1 || p->n2 < 1 || p->n3 < 1) return KH_EINVAL;
-  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1 || p->inverter < 0 || p->inverter > 1 || p->fofc < 0 || p->fofc > 1 || p->floor_frame < 0 || p->floor_frame > 1) return KH_EINVAL;
+  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1 || p->inverter < 0 || p->inverter > 1 || p->fofc < 0 || p->fofc > 1 || p->floor_frame < 0 || p->floor_frame > 2) return KH_EINVAL;
   if (!(p->gamma > 1.0) || !(p->cfl > 0.0) || !(p->dt_growth_max > 0.0)) return KH_EINVAL;
   const int N[3] = {p->n1, p->n2, p->n3};
   for (int d = 0; d < 3; d++) {
@@ -344,7 +345,7 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   v.ndim_mask = (v.n1 > 1 ? 1 : 0) | (v.n2 > 1 ? 2 : 0) | (v.n3 > 1 ? 4 : 0);
   v.fp.inv_bsq_over_rho_max = 1.0 / p->bsq_over_rho_max; v.fp.inv_bsq_over_u_max = 1.0 / p->bsq_over_u_max;
   v.fp.u_over_rho_max = p->u_over_rho_max; v.fp.gamma_max = p->gamma_max;
-  v.floor_frame = p->floor_frame;
+  v.floor_frame = p->floor_frame; v.inverter = p->inverter;
 
 #define ALLOC(ptr, bytes)                                                       \
   do {                                                                          \

@@ -427,3 +427,30 @@ def test_hundred_step_runs_l1(kh, kho, cfg, n):
     assert np.array_equal(gg.get_flags()[0], go.get_flags()[0])
     d_g, d_o = gg.divB(), go.divB()
     assert d_g <= 4 * d_o + 1e-12
+
+
+# ------------------------------------------------------------------------------------------ normal-frame floors (NEXT-4)
+@pytest.mark.parametrize("case", ["torus_weno5", "mad_stress_mc", "torus_kastaun", "minkowski"])
+def test_one_step_normal_frame_floors(kh, kho, case):
+    """kh_params.floor_frame = KH_FRAME_NORMAL on both sides: same bars (floor flags may carry bit 64)."""
+    if case == "torus_weno5":
+        p = ki.config_params(3, n=(64, 48, 8)); P0 = torus.torus_state(p, seed=2)
+    elif case == "mad_stress_mc":
+        p = ki.config_params(4, n=(72, 40, 8)); P0 = torus.torus_state(p, mad=True, seed=3, stress=True, stress_fraction=0.02)
+    elif case == "torus_kastaun":
+        p = dict(ki.config_params(3, n=(33, 17, 3)), inverter=kp.INV_KASTAUN); P0 = torus.torus_state(p, seed=2)
+    else:
+        p = ki.config_params(5, n=(16, 12, 8)); P0 = modes.config5(p, seed=1, amp=1e-3)
+    p = dict(p, floor_frame=kp.FRAME_NORMAL)
+    worst, gg, go = _one_step_case(kh, kho, p, P0, label="normal " + case)
+    if case != "minkowski":
+        assert (go.get_flags()[1] != 0).any()
+    # fix-up hook under the same frame
+    if case == "torus_weno5":
+        rng = np.random.default_rng(0)
+        pf = np.zeros((p["n3"] + 6, p["n2"] + 6, p["n1"] + 6), dtype=np.int32)
+        pf[3:-3, 3:-3, 3:-3] = (rng.uniform(size=(p["n3"], p["n2"], p["n1"])) < 0.1) * 3
+        gg.debug_fixup(pf); go.debug_fixup(pf)
+        z = np.zeros_like(gg.get_flags()[0])
+        _assert_step_parity(p, gg.get_prims(), go.get_prims(), z, z, "normal-frame fix-up")     # the S23 metric
+        assert (gg.get_flags()[1] != go.get_flags()[1]).mean() < 1e-3
