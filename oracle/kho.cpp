@@ -733,6 +733,7 @@ struct kho_grid {
   std::vector<double> ctop[3];   // [ntot]
   std::vector<double> emf[3];    // [ntot]
   std::vector<int> pflag, fflag; // [ntot]
+  std::vector<double> Bf[3], Bfs[3], Bff[3];   // face-centred CT (S28): sqrt(-g) B^d on the lower d-face of each zone, [ntot]; n / * / n+1
   long idx(int i, int j, int k) const { return ((long)(k + NG) * nt[1] + (j + NG)) * nt[0] + (i + NG); }
   long idx2(int i, int j) const { return (long)(j + NG) * nt[0] + (i + NG); }
   double xc(int d, int i) const { return p.xmin[d] + (i + 0.5) * dx[d]; }
@@ -890,7 +891,7 @@ void fixup(kho_grid& g, double* Pf) {
 
 // One sub-step (S22): fluxes from Ps, update of U(Pi) by Dt, U->P with guess Pi, floors, fill, fix-up, fill.
 // C6 + C7 + C8 on the interior zones: U_f = U(P_i) + Dt [-div F + S(P_s)], inversion with guess P_i, floors.
-void update_zones(kho_grid& g, const double* Pi, const double* Ps, double* Pf, double Dt) {
+void update_zones(kho_grid& g, const double* Pi, const double* Ps, double* Pf, double Dt, const std::vector<double>* Bface = nullptr) {
   const long nt = g.ntot;
   const long st[3] = {1, g.nt[0], (long)g.nt[0] * g.nt[1]};
   std::fill(g.pflag.begin(), g.pflag.end(), 0);
@@ -913,6 +914,8 @@ void update_zones(kho_grid& g, const double* Pi, const double* Ps, double* Pf, d
       for (int d = 0; d < 3; d++) div += (g.F[d][v * nt + n + st[d]] - g.F[d][v * nt + n]) / g.dx[d];
       Uf[v] = Ui[v] + Dt * (-div + S[v]);
     }
+    // face-centred CT (S28): the zone's conserved field is the mean of its two face values
+    if (Bface) for (int d = 0; d < 3; d++) Uf[B1 + d] = 0.5 * (Bface[d][n] + Bface[d][n + st[d]]);
     int pf_flag = (g.p.inverter == KHO_INV_KASTAUN) ? u2p_kastaun(G, Uf, pi, g.p.gamma, pf) : u2p(G, Uf, pi, g.p.gamma, pf);
     int ff = 0;
     if (pf_flag == 0) ff = floors(g.p, G, g.sfloor_r[n2], pf);
@@ -944,7 +947,27 @@ void fofc_reflux(kho_grid& g, const double* Ps, const std::vector<int>& mask) {
   }
 }
 
-void substep(kho_grid& g, const double* Pi, const double* Ps, double* Pf, double Dt) {
+// Face-centred constrained transport ("the face-centered constrained transport scheme outlined in [50],
+// including a number of schemes for determining the EMFs along zone edges"; reading S28).  The
+// magnetic field lives on the faces as Phi^d = sqrt(-g) B^d; it is advanced by the circulation of the edge EMFs around
+// each face, so the face-centred divergence sum_d (Phi^d(+1) - Phi^d)/dx_d is constant to round-off:
+//   Phi^1_f = Phi^1_i + Dt [ (E3(i,j+1,k) - E3(i,j,k))/dx2 - (E2(i,j,k+1) - E2(i,j,k))/dx3 ]   and cyclic (E = this file's
+// emf arrays, lower edge of the zone).  EMF option built: the arithmetic four-point average of the face fluxes (the one
+// Flux-CT uses, C5), for which the zone-centred mean of the face field evolves exactly as under Flux-CT (Toth 2000).
+// Zone-centred B (primitive) = mean of the zone's two face values / sqrt(-g); ghosts by the ordinary fill.
+void face_ct_update(const kho_grid& g, const std::vector<double>* Bi, std::vector<double>* Bf, double Dt) {
+  const long s1 = 1, s2 = g.nt[0], s3 = (long)g.nt[0] * g.nt[1];
+  const double* e1 = g.emf[0].data(); const double* e2 = g.emf[1].data(); const double* e3 = g.emf[2].data();
+  for (int k = 0; k <= g.n[2]; k++) for (int j = 0; j <= g.n[1]; j++) for (int i = 0; i <= g.n[0]; i++) {
+    long n = g.idx(i, j, k);
+    if (j < g.n[1] && k < g.n[2]) Bf[0][n] = Bi[0][n] + Dt * ((e3[n + s2] - e3[n]) / g.dx[1] - (e2[n + s3] - e2[n]) / g.dx[2]);
+    if (i < g.n[0] && k < g.n[2]) Bf[1][n] = Bi[1][n] + Dt * ((e1[n + s3] - e1[n]) / g.dx[2] - (e3[n + s1] - e3[n]) / g.dx[0]);
+    if (i < g.n[0] && j < g.n[1]) Bf[2][n] = Bi[2][n] + Dt * ((e2[n + s1] - e2[n]) / g.dx[0] - (e1[n + s2] - e1[n]) / g.dx[1]);
+  }
+}
+
+void substep(kho_grid& g, const double* Pi, const double* Ps, double* Pf, double Dt, const std::vector<double>* Bfi = nullptr,
+             std::vector<double>* Bff = nullptr) {
   for (int d = 0; d < 3; d++) compute_flux(g, Ps, d);
   const long nt = g.ntot;
   if (g.p.fofc) {
@@ -961,7 +984,8 @@ void substep(kho_grid& g, const double* Pi, const double* Ps, double* Pf, double
   }
   flux_ct(g, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data());
   if (Pf != Pi) std::memcpy(Pf, Pi, sizeof(double) * NP * nt);   // ghosts of Pf start from Pi (matters for FIXED)
-  update_zones(g, Pi, Ps, Pf, Dt);
+  if (Bfi) face_ct_update(g, Bfi, Bff, Dt);
+  update_zones(g, Pi, Ps, Pf, Dt, Bfi ? Bff : nullptr);
   fill_ghosts_prims(g, Pf);
   fill_ghosts_flag(g, g.pflag.data());
   fixup(g, Pf);
@@ -1040,6 +1064,7 @@ int kho_grid_create(const kho_params* p, kho_grid** out) {
     g->P.assign(NP * g->ntot, 0.0); g->Ps.assign(NP * g->ntot, 0.0); g->Pf.assign(NP * g->ntot, 0.0);
     for (int d = 0; d < 3; d++) { g->F[d].assign(NP * g->ntot, 0.0); g->ctop[d].assign(g->ntot, 0.0); g->emf[d].assign(g->ntot, 0.0); }
     g->pflag.assign(g->ntot, 0); g->fflag.assign(g->ntot, 0);
+    if (g->p.transport == KHO_B_FACE_CT) for (int d = 0; d < 3; d++) { g->Bf[d].assign(g->ntot, 0.0); g->Bfs[d].assign(g->ntot, 0.0); g->Bff[d].assign(g->ntot, 0.0); }
   } catch (...) { delete g; return KHO_ENOMEM; }
   *out = g;
   return KHO_OK;
@@ -1121,8 +1146,14 @@ int kho_estimate_dt(kho_grid* g, double* dt) {
 // C11 (S22): P* = substep(P^n, P^n, dt/2);  P^{n+1} = substep(P^n, P*, dt);  dt_next from the corrector's face speeds.
 int kho_step(kho_grid* g, double dt, double* dt_next) {
   if (!g || !(dt > 0.0)) return KHO_EINVAL;
-  substep(*g, g->P.data(), g->P.data(), g->Ps.data(), 0.5 * dt);
-  substep(*g, g->P.data(), g->Ps.data(), g->Pf.data(), dt);
+  if (g->p.transport == KHO_B_FACE_CT) {
+    substep(*g, g->P.data(), g->P.data(), g->Ps.data(), 0.5 * dt, g->Bf, g->Bfs);
+    substep(*g, g->P.data(), g->Ps.data(), g->Pf.data(), dt, g->Bf, g->Bff);
+    for (int d = 0; d < 3; d++) g->Bf[d].swap(g->Bff[d]);
+  } else {
+    substep(*g, g->P.data(), g->P.data(), g->Ps.data(), 0.5 * dt);
+    substep(*g, g->P.data(), g->Ps.data(), g->Pf.data(), dt);
+  }
   g->P.swap(g->Pf);
   if (dt_next) {
     double d = g->p.cfl * dt_from_ctop(*g);
@@ -1194,7 +1225,12 @@ int kho_get_conn(kho_grid* g, double* conn64) {
 // test hook: predictor sub-step only; P* becomes the current state
 int kho_debug_predictor(kho_grid* g, double dt) {
   if (!g || !(dt > 0.0)) return KHO_EINVAL;
-  substep(*g, g->P.data(), g->P.data(), g->Ps.data(), 0.5 * dt);
+  if (g->p.transport == KHO_B_FACE_CT) {
+    substep(*g, g->P.data(), g->P.data(), g->Ps.data(), 0.5 * dt, g->Bf, g->Bfs);
+    for (int d = 0; d < 3; d++) g->Bf[d].swap(g->Bfs[d]);
+  } else {
+    substep(*g, g->P.data(), g->P.data(), g->Ps.data(), 0.5 * dt);
+  }
   g->P.swap(g->Ps);
   return KHO_OK;
 }
@@ -1202,6 +1238,37 @@ int kho_debug_fixup(kho_grid* g, const int* pflag_with_ghosts) {
   if (!g || !pflag_with_ghosts) return KHO_EINVAL;
   for (long n = 0; n < g->ntot; n++) { g->pflag[n] = pflag_with_ghosts[n]; g->fflag[n] = 0; }
   fixup(*g, g->P.data());
+  return KHO_OK;
+}
+int kho_set_face_B(kho_grid* g, const double* f1, const double* f2, const double* f3) {
+  if (!g || !f1 || !f2 || !f3 || g->p.transport != KHO_B_FACE_CT) return KHO_EINVAL;
+  const double* f[3] = {f1, f2, f3};
+  for (int d = 0; d < 3; d++) g->Bf[d].assign(f[d], f[d] + g->ntot);
+  const long st[3] = {1, g->nt[0], (long)g->nt[0] * g->nt[1]};
+  for (int k = 0; k < g->n[2]; k++) for (int j = 0; j < g->n[1]; j++) for (int i = 0; i < g->n[0]; i++) {
+    long n = g->idx(i, j, k);
+    for (int d = 0; d < 3; d++) g->P[(B1 + d) * g->ntot + n] = 0.5 * (g->Bf[d][n] + g->Bf[d][n + st[d]]) / g->G[0][g->idx2(i, j)].gdet;
+  }
+  fill_ghosts_prims(*g, g->P.data());
+  return KHO_OK;
+}
+int kho_get_face_B(kho_grid* g, double* f1, double* f2, double* f3) {
+  if (!g || !f1 || !f2 || !f3 || g->p.transport != KHO_B_FACE_CT) return KHO_EINVAL;
+  double* f[3] = {f1, f2, f3};
+  for (int d = 0; d < 3; d++) std::memcpy(f[d], g->Bf[d].data(), sizeof(double) * g->ntot);
+  return KHO_OK;
+}
+int kho_divB_face(kho_grid* g, double* max_abs) {
+  if (!g || !max_abs || g->p.transport != KHO_B_FACE_CT) return KHO_EINVAL;
+  const long st[3] = {1, g->nt[0], (long)g->nt[0] * g->nt[1]};
+  double m = 0.0;
+  for (int k = 0; k < g->n[2]; k++) for (int j = 0; j < g->n[1]; j++) for (int i = 0; i < g->n[0]; i++) {
+    long n = g->idx(i, j, k);
+    double div = 0.0;
+    for (int d = 0; d < 3; d++) div += (g->Bf[d][n + st[d]] - g->Bf[d][n]) / g->dx[d];
+    if (std::fabs(div) > m) m = std::fabs(div);
+  }
+  *max_abs = m;
   return KHO_OK;
 }
 int kho_debug_fofc(kho_grid* g, const int* mask_with_ghosts) {

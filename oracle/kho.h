@@ -26,6 +26,7 @@ enum { KHO_BC_PERIODIC = 0, KHO_BC_OUTFLOW = 1, KHO_BC_POLAR = 2, KHO_BC_FIXED =
 enum { KHO_RECON_MC = 0, KHO_RECON_WENO5 = 1 };
 enum { KHO_INV_1DW = 0, KHO_INV_KASTAUN = 1 };
 enum { KHO_FRAME_FLUID = 0, KHO_FRAME_DRIFT = 1, KHO_FRAME_NORMAL = 2 };
+enum { KHO_B_FLUX_CT = 0, KHO_B_FACE_CT = 1 };
 enum { KHO_LOC_CENT = 0, KHO_LOC_FACE1 = 1, KHO_LOC_FACE2 = 2, KHO_LOC_FACE3 = 3 };
 
 typedef struct {
@@ -42,6 +43,7 @@ typedef struct {
   int inverter;                                    /* KHO_INV_1DW | KHO_INV_KASTAUN (NEXT-2) */
   int fofc;                                        /* 1: first-order flux correction (NEXT-3) */
   int floor_frame;                                 /* KHO_FRAME_FLUID | _DRIFT | _NORMAL (NEXT-4) */
+  int transport;                                   /* KHO_B_FLUX_CT | KHO_B_FACE_CT (NEXT-1) */
 } kho_params;
 
 typedef struct kho_grid kho_grid;
@@ -56,6 +58,11 @@ int kho_get_flags(kho_grid* g, int* pflag, int* fflag);   /* interior, last sub-
 int kho_estimate_dt(kho_grid* g, double* dt);
 int kho_step(kho_grid* g, double dt, double* dt_next);
 int kho_divB(kho_grid* g, double* max_abs);
+/* face-centred CT (NEXT-1): Phi^d = sqrt(-g) B^d on the lower d-face of each zone, with ghosts [nt] each (faces
+ * i_d in [0, N_d], transverse interior are used); setting it also sets the zone-centred B of the current state */
+int kho_set_face_B(kho_grid* g, const double* f1, const double* f2, const double* f3);
+int kho_get_face_B(kho_grid* g, double* f1, double* f2, double* f3);
+int kho_divB_face(kho_grid* g, double* max_abs);   /* max |sum_d (Phi^d(+1) - Phi^d)/dx_d| over interior zones */
 /* stage access for tests: fluxes after Flux-CT of the LAST sub-step, with ghosts [8][nt]; ctop [nt] */
 int kho_get_flux(kho_grid* g, int dir, double* F, double* ctop);
 int kho_get_emf(kho_grid* g, int dir, double* emf);

@@ -27,7 +27,7 @@ class Params(C.Structure):
         ("gamma", C.c_double), ("cfl", C.c_double), ("recon", C.c_int),
         ("rho_min", C.c_double), ("u_min", C.c_double), ("r_char", C.c_double),
         ("bsq_over_rho_max", C.c_double), ("bsq_over_u_max", C.c_double), ("u_over_rho_max", C.c_double),
-        ("gamma_max", C.c_double), ("dt_growth_max", C.c_double), ("inverter", C.c_int), ("fofc", C.c_int), ("floor_frame", C.c_int),
+        ("gamma_max", C.c_double), ("dt_growth_max", C.c_double), ("inverter", C.c_int), ("fofc", C.c_int), ("floor_frame", C.c_int), ("transport", C.c_int),
     ]
 
 
@@ -262,6 +262,21 @@ class Grid:
         pf = np.ascontiguousarray(pflag_with_ghosts, dtype=np.int32)
         assert pf.shape == self.shape_gh[1:]
         _chk(self.L.kho_debug_fixup(self.h, pf.ctypes.data_as(_ip)))
+
+    def set_face_B(self, f1, f2, f3):
+        a = [np.ascontiguousarray(f, dtype=np.float64) for f in (f1, f2, f3)]
+        assert all(x.shape == self.shape_gh[1:] for x in a)
+        _chk(self.L.kho_set_face_B(self.h, *[x.ctypes.data_as(_dp) for x in a]))
+
+    def get_face_B(self):
+        a = [np.empty(self.shape_gh[1:]) for _ in range(3)]
+        _chk(self.L.kho_get_face_B(self.h, *[x.ctypes.data_as(_dp) for x in a]))
+        return a
+
+    def divB_face(self):
+        m = C.c_double()
+        _chk(self.L.kho_divB_face(self.h, C.byref(m)))
+        return m.value
 
     def debug_fofc(self, mask_with_ghosts):
         m = np.ascontiguousarray(mask_with_ghosts, dtype=np.int32)
