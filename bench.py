@@ -43,6 +43,7 @@ WORKLOADS = {
     "torus_sane_192x128x128_weno5_kastaun": (3, None, None),      # same block, kh_params.inverter = KH_INV_KASTAUN
     "torus_sane_192x128x128_weno5_fofc": (3, None, None),         # same block, kh_params.fofc = 1
     "torus_sane_192x128x128_weno5_drift": (3, None, None),        # same block, kh_params.floor_frame = KH_FRAME_DRIFT
+    "torus_sane_192x128x128_weno5_facect": (3, None, None),       # same block, kh_params.transport = KH_B_FACE_CT
     "minkowski_128_mc": (5, 128, 0), "minkowski_128_weno5": (5, 128, 1),
     "minkowski_256_mc": (5, 256, 0), "minkowski_256_weno5": (5, 256, 1),
     "minkowski_64_mc": (5, 64, 0), "minkowski_192_mc": (5, 192, 0), "minkowski_320_mc": (5, 320, 0),
@@ -95,6 +96,8 @@ def workload_params(name):
         p["fofc"] = 1
     if name.endswith("_drift"):
         p["floor_frame"] = ki.params.FRAME_DRIFT
+    if name.endswith("_facect"):
+        p["transport"] = ki.params.B_FACE_CT
     return cfg, p
 
 
@@ -303,6 +306,9 @@ def run_ours(args):
     with torch.cuda.stream(stream):
         g = kh.Grid(p, stream=stream.cuda_stream)
         g.set_prims(P0)
+        if p.get("transport", 0) == 1:       # face-centred CT: a divergence-free poloidal loop on the faces (Stokes)
+            from kharm_inputs import facefield
+            g.set_face_B(*facefield.face_from_potential(p, *facefield.axisymmetric_loop_potential(p, amp=2e-3, x1c=2.5)))
         dt0 = g.estimate_dt()
         # ---- device-resident timing: W warm-up steps, then exactly K steps between two events on the grid's stream
         g.step(dt0, sync=False)

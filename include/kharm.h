@@ -39,6 +39,7 @@ enum { KH_BC_PERIODIC = 0, KH_BC_OUTFLOW = 1, KH_BC_POLAR = 2, KH_BC_FIXED = 3 }
 enum { KH_RECON_MC = 0, KH_RECON_WENO5 = 1 };                                 /* P:253           */
 enum { KH_INV_1DW = 0, KH_INV_KASTAUN = 1 };
 enum { KH_FRAME_FLUID = 0, KH_FRAME_DRIFT = 1, KH_FRAME_NORMAL = 2 };
+enum { KH_B_FLUX_CT = 0, KH_B_FACE_CT = 1 };
 enum { KH_MEM_DEVICE = 0, KH_MEM_HOST = 1 };
 enum { KH_LOC_CENT = 0, KH_LOC_FACE1 = 1, KH_LOC_FACE2 = 2, KH_LOC_FACE3 = 3 };
 
@@ -61,6 +62,9 @@ typedef struct {
   int floor_frame;            /* frame the floor material is injected in: KH_FRAME_FLUID (velocity
                                  untouched) | KH_FRAME_DRIFT (E x B drift velocity kept, momentum along B conserved) |
                                  KH_FRAME_NORMAL (added as gas at rest for the normal observer, then re-inverted)   */
+  int transport;              /* magnetic field transport: KH_B_FLUX_CT (zone-centred field, Toth's Flux-CT) |
+                                 KH_B_FACE_CT (face-centred field advanced by the circulation of the edge EMFs;
+                                 EMF = arithmetic four-point average; needs kh_set_face_B)                     */
 } kh_params;
 
 typedef struct kh_grid kh_grid;   /* opaque */
@@ -117,6 +121,14 @@ int kh_get_conn(kh_grid* g, double* conn64, int mem);
  * face of the zone; hydro components as used by the update, B components replaced by their Flux-CT
  * values (computed from the edge EMFs); ctop [nt].  Entries outside the computed face range are 0. */
 int kh_get_flux(kh_grid* g, int dir, double* F, double* ctop, int mem);
+/* Face-centred CT (kh_params.transport = KH_B_FACE_CT).  Phi^d = sqrt(-g) B^d on the lower d-face of each zone, three
+ * arrays with ghosts [nt] (faces i_d in [0, N_d] with interior transverse indices are used, the rest ignored).
+ * kh_set_face_B also sets the zone-centred field of the current state to the mean of each zone's two face values over
+ * sqrt(-g) and fills its ghosts: call it AFTER kh_set_prims.  kh_divB_face: max over interior zones of
+ * |sum_d (Phi^d(upper) - Phi^d(lower))/dx_d|, which the transport keeps at its initial value to round-off. */
+int kh_set_face_B(kh_grid* g, const double* f1, const double* f2, const double* f3, int mem);
+int kh_get_face_B(kh_grid* g, double* f1, double* f2, double* f3, int mem);
+int kh_divB_face(kh_grid* g, double* max_abs);
 /* Edge EMFs of the last sub-step, with ghosts [nt], index = lower edge of the zone. */
 int kh_get_emf(kh_grid* g, int dir, double* emf, int mem);
 /* Run the fix-up (K5b) + floors + refresh of the fixed zones' ghost images on the current primitives for a caller-supplied flag array

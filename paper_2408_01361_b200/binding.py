@@ -19,7 +19,7 @@ NG = 3
 
 EXPORTED_SYMBOLS = (
     "kh_grid_create", "kh_grid_destroy", "kh_set_prims", "kh_get_prims", "kh_get_cons", "kh_get_flags",
-    "kh_estimate_dt", "kh_step", "kh_divB", "kh_count_flags", "kh_get_geom", "kh_get_conn", "kh_get_flux",
+    "kh_estimate_dt", "kh_step", "kh_divB", "kh_set_face_B", "kh_get_face_B", "kh_divB_face", "kh_count_flags", "kh_get_geom", "kh_get_conn", "kh_get_flux",
     "kh_get_emf", "kh_debug_fixup", "kh_debug_predictor", "kh_launch_count", "kh_set_graph", "kh_set_profile", "kh_get_profile", "kh_measure_fp64_peak", "kh_strerror",
     "kh_last_cuda_error",
 )
@@ -40,7 +40,7 @@ class Params(C.Structure):
         ("gamma", C.c_double), ("cfl", C.c_double), ("recon", C.c_int),
         ("rho_min", C.c_double), ("u_min", C.c_double), ("r_char", C.c_double),
         ("bsq_over_rho_max", C.c_double), ("bsq_over_u_max", C.c_double), ("u_over_rho_max", C.c_double),
-        ("gamma_max", C.c_double), ("dt_growth_max", C.c_double), ("inverter", C.c_int), ("fofc", C.c_int), ("floor_frame", C.c_int),
+        ("gamma_max", C.c_double), ("dt_growth_max", C.c_double), ("inverter", C.c_int), ("fofc", C.c_int), ("floor_frame", C.c_int), ("transport", C.c_int),
     ]
 
 
@@ -81,6 +81,9 @@ def lib():
         L.kh_estimate_dt.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.kh_step.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         L.kh_divB.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+        L.kh_divB_face.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+        L.kh_set_face_B.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
+        L.kh_get_face_B.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         L.kh_count_flags.argtypes = [C.c_void_p, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
         L.kh_get_geom.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         L.kh_get_conn.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
@@ -208,6 +211,22 @@ class Grid:
     def divB(self):
         m = C.c_double()
         _chk(self.L.kh_divB(self.h, C.byref(m)))
+        return m.value
+
+    def set_face_B(self, f1, f2, f3):
+        """Face field of the face-centred CT transport (three arrays with ghosts); also sets the zone-centred field."""
+        a = [np.ascontiguousarray(f, dtype=np.float64) for f in (f1, f2, f3)]
+        assert all(x.shape == self.shape_gh[1:] for x in a)
+        _chk(self.L.kh_set_face_B(self.h, _np_ptr(a[0]), _np_ptr(a[1]), _np_ptr(a[2]), MEM_HOST))
+
+    def get_face_B(self):
+        a = [np.empty(self.shape_gh[1:]) for _ in range(3)]
+        _chk(self.L.kh_get_face_B(self.h, _np_ptr(a[0]), _np_ptr(a[1]), _np_ptr(a[2]), MEM_HOST))
+        return a
+
+    def divB_face(self):
+        m = C.c_double()
+        _chk(self.L.kh_divB_face(self.h, C.byref(m)))
         return m.value
 
     def count_flags(self):

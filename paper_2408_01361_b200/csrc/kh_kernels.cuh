@@ -674,6 +674,50 @@ fofc_reflux_kernel(GV g, const double* __restrict__ P, const unsigned char* __re
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Face-centred constrained transport (S28).  Phi^d = sqrt(-g) B^d lives on the lower
+// d-face of each zone and is advanced by the circulation of the edge EMFs around the face (arithmetic four-point EMF, the
+// emf_kernel's), so the face-centred divergence is constant to round-off.  The zone-centred field is the mean of the two
+// face values over sqrt(-g).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+face_ct_kernel(GV g, const double* __restrict__ i1, const double* __restrict__ i2, const double* __restrict__ i3, double* __restrict__ o1,
+               double* __restrict__ o2, double* __restrict__ o3, const double* __restrict__ e1, const double* __restrict__ e2,
+               const double* __restrict__ e3, const StepScalars* __restrict__ sc, double dt_factor) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  if (i > g.n1) return;
+  const long n = zidx(g, i, j, k), s2 = g.s2, s3 = g.s3;
+  const double Dt = dt_factor * sc->dt;
+  if (j < g.n2 && k < g.n3) o1[n] = fma(Dt, (e3[n + s2] - e3[n]) * g.idx2 - (e2[n + s3] - e2[n]) * g.idx3, i1[n]);
+  if (i < g.n1 && k < g.n3) o2[n] = fma(Dt, (e1[n + s3] - e1[n]) * g.idx3 - (e3[n + 1] - e3[n]) * g.idx1, i2[n]);
+  if (i < g.n1 && j < g.n2) o3[n] = fma(Dt, (e2[n + 1] - e2[n]) * g.idx1 - (e1[n + s2] - e1[n]) * g.idx2, i3[n]);
+}
+
+// zone-centred primitive field from the face field: B^d = (Phi^d(lower) + Phi^d(upper)) / (2 sqrt(-g))
+__global__ void __launch_bounds__(128)
+face_to_cent_kernel(GV g, const double* __restrict__ f1, const double* __restrict__ f2, const double* __restrict__ f3, double* __restrict__ P,
+                    int flat) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  if (i >= g.n1) return;
+  const long n = zidx(g, i, j, k), nt = g.ntot;
+  const double h = flat ? 0.5 : 0.5 / __ldg(g.geom[0] + 20 * g.n2d + pidx(g, i, j));
+  P[B1 * nt + n] = h * (f1[n] + f1[n + 1]);
+  P[B2 * nt + n] = h * (f2[n] + f2[n + g.s2]);
+  P[B3 * nt + n] = h * (f3[n] + f3[n + g.s3]);
+}
+
+__global__ void divb_face_kernel(GV g, const double* __restrict__ f1, const double* __restrict__ f2, const double* __restrict__ f3,
+                                 StepScalars* __restrict__ sc) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  double a = 0.0;
+  if (i < g.n1) {
+    const long n = zidx(g, i, j, k);
+    a = fabs((f1[n + 1] - f1[n]) * g.idx1 + (f2[n + g.s2] - f2[n]) * g.idx2 + (f3[n + g.s3] - f3[n]) * g.idx3);
+  }
+  for (int o = 16; o > 0; o >>= 1) a = fmax(a, __shfl_xor_sync(0xffffffffu, a, o));
+  if ((threadIdx.x & 31) == 0) atomicMax(&sc->max_bits, (unsigned long long)__double_as_longlong(a));
+}
+
 // debug hook support: failure list from a caller-supplied flag array (interior zones, any order)
 __global__ void build_faillist_kernel(GV g, const unsigned char* __restrict__ pflag, unsigned* __restrict__ list, StepScalars* __restrict__ sc) {
   int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;

@@ -39,6 +39,7 @@ struct kh_grid {
   double* ctop[3];
   double* emf[3];
   unsigned char *pflag, *fflag;
+  double* Bf[3][3];      // face-centred CT: Phi^d per rotation state [state][d], [ntot] each (allocated on demand)
   unsigned char* mask;   // FOFC: troubled zones of the speculative update (with ghost images)
   unsigned* faillist;    // zones (device-layout index) whose inversion failed in the current sub-step
   double* fix;           // [5][ntot] scratch of the fix-up (pre-fix-up snapshot semantics)
@@ -179,7 +180,8 @@ static int do_fixup(kh_grid* g, double* Pf) {
 }
 
 // One sub-step (S22): fluxes from Ps, update of U(Pi), inversion with guess Pi, floors, fill, fix-up, fill.
-static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, double dt_factor, bool corrector) {
+static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, double dt_factor, bool corrector,
+                   double* const* Bfi = nullptr, double* const* Bff = nullptr) {
   const GV& v = g->gv;
   reset_counters_kernel<<<1, 1, 0, g->stream>>>(g->sc, 0);
   g->launches++;
@@ -210,6 +212,17 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
 #undef UPD
     g->launches++;
     CK(cudaGetLastError());
+    if (Bfi && pass + 1 == passes) {
+      // face-centred CT: advance the face field by the EMF circulation and slave the zone-centred field to it (the
+      // update kernel's own induction update equals the face mean to round-off for the arithmetic EMF: Toth 2000)
+      prof_begin(g, KH_K_EMF);
+      face_ct_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, Bfi[0], Bfi[1], Bfi[2], Bff[0], Bff[1], Bff[2], g->emf[0],
+                                                                                       g->emf[1], g->emf[2], g->sc, dt_factor);
+      face_to_cent_kernel<<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, Bff[0], Bff[1], Bff[2], Pf, g->flat ? 1 : 0);
+      prof_end(g);
+      g->launches += 2;
+      CK(cudaGetLastError());
+    }
     if (pass + 1 < passes) {
       // troubled zones of the speculative update -> mask (+ ghost images) -> donor-cell LLF on their faces
       prof_begin(g, KH_K_FOFC);
@@ -234,9 +247,10 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
 
 static int enqueue_step(kh_grid* g, int cur) {
   double *Pn = g->P[cur], *Pstar = g->P[(cur + 1) % 3], *Pnew = g->P[(cur + 2) % 3];
-  int rc = substep(g, Pn, Pn, Pstar, 0.5, false);
+  const bool face = g->p.transport == KH_B_FACE_CT;
+  int rc = substep(g, Pn, Pn, Pstar, 0.5, false, face ? g->Bf[cur] : nullptr, face ? g->Bf[(cur + 1) % 3] : nullptr);
   if (rc) return rc;
-  rc = substep(g, Pn, Pstar, Pnew, 1.0, true);
+  rc = substep(g, Pn, Pstar, Pnew, 1.0, true, face ? g->Bf[cur] : nullptr, face ? g->Bf[(cur + 2) % 3] : nullptr);
   if (rc) return rc;
   finalize_dt_kernel<<<1, 1, 0, g->stream>>>(g->sc, g->p.cfl, g->p.dt_growth_max);
   g->launches++;
@@ -276,7 +290,8 @@ int kh_grid_destroy(kh_grid* g) {
   for (int l = 0; l < 4; l++) cudaFree(g->geom[l]);
   cudaFree(g->conn); cudaFree(g->dg); cudaFree(g->floorp);
   for (int b = 0; b < 3; b++) { cudaFree(g->P[b]); cudaFree(g->F[b]); cudaFree(g->ctop[b]); cudaFree(g->emf[b]); }
-  cudaFree(g->pflag); cudaFree(g->fflag); cudaFree(g->mask); cudaFree(g->faillist); cudaFree(g->sc); cudaFree(g->fix); cudaFree(g->stage);
+  cudaFree(g->pflag); cudaFree(g->fflag); cudaFree(g->mask);
+  for (int b = 0; b < 3; b++) for (int d = 0; d < 3; d++) cudaFree(g->Bf[b][d]); cudaFree(g->faillist); cudaFree(g->sc); cudaFree(g->fix); cudaFree(g->stage);
   if (g->sc_host) cudaFreeHost(g->sc_host);
   if (g->pev) { for (int e = 0; e < 2 * KH_PROF_POOL; e++) if (g->pev[e]) cudaEventDestroy(g->pev[e]); delete[] g->pev; }
   delete[] g->pkind;
@@ -288,7 +303,7 @@ int kh_grid_destroy(kh_grid* g) {
 int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   if (!p || !out) return KH_EINVAL;
   if (p->n1 < 1 || p->n2 < 1 || p->n3 < 1) return KH_EINVAL;
-  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1 || p->inverter < 0 || p->inverter > 1 || p->fofc < 0 || p->fofc > 1 || p->floor_frame < 0 || p->floor_frame > 2) return KH_EINVAL;
+  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1 || p->inverter < 0 || p->inverter > 1 || p->fofc < 0 || p->fofc > 1 || p->floor_frame < 0 || p->floor_frame > 2 || p->transport < 0 || p->transport > 1) return KH_EINVAL;
   if (!(p->gamma > 1.0) || !(p->cfl > 0.0) || !(p->dt_growth_max > 0.0)) return KH_EINVAL;
   const int N[3] = {p->n1, p->n2, p->n3};
   for (int d = 0; d < 3; d++) {
@@ -369,6 +384,7 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   ALLOC(g->pflag, v.ntot);
   ALLOC(g->fflag, v.ntot);
   if (p->fofc) ALLOC(g->mask, v.ntot);
+  if (p->transport == KH_B_FACE_CT) for (int b = 0; b < 3; b++) for (int d = 0; d < 3; d++) ALLOC(g->Bf[b][d], fb);
   ALLOC(g->faillist, sizeof(unsigned) * (size_t)v.n1 * v.n2 * v.n3);
   ALLOC(g->sc, sizeof(StepScalars));
 #undef ALLOC
@@ -556,6 +572,52 @@ int kh_divB(kh_grid* g, double* max_abs) {
   return KH_OK;
 }
 
+int kh_set_face_B(kh_grid* g, const double* f1, const double* f2, const double* f3, int mem) {
+  if (!g || !f1 || !f2 || !f3 || g->p.transport != KH_B_FACE_CT || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  const GV& v = g->gv;
+  const double* f[3] = {f1, f2, f3};
+  for (int d = 0; d < 3; d++) {
+    int rc = xfer(g, g->Bf[g->cur][d], f[d], sizeof(double) * v.ntot, mem, false);
+    if (rc) return rc;
+  }
+  double* const* B = g->Bf[g->cur];
+  face_to_cent_kernel<<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, B[0], B[1], B[2], g->P[g->cur], g->flat ? 1 : 0);
+  g->launches++;
+  CK(cudaGetLastError());
+  int rc = fill_ghosts(g, g->P[g->cur], nullptr);
+  if (rc) return rc;
+  CK(cudaStreamSynchronize(g->stream));
+  return KH_OK;
+}
+
+int kh_get_face_B(kh_grid* g, double* f1, double* f2, double* f3, int mem) {
+  if (!g || !f1 || !f2 || !f3 || g->p.transport != KH_B_FACE_CT || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  double* f[3] = {f1, f2, f3};
+  for (int d = 0; d < 3; d++) {
+    int rc = xfer(g, f[d], g->Bf[g->cur][d], sizeof(double) * g->gv.ntot, mem, true);
+    if (rc) return rc;
+  }
+  return KH_OK;
+}
+
+int kh_divB_face(kh_grid* g, double* max_abs) {
+  if (!g || !max_abs || g->p.transport != KH_B_FACE_CT) return KH_EINVAL;
+  const GV& v = g->gv;
+  unsigned long long zero = 0;
+  CK(cudaMemcpyAsync(&g->sc->max_bits, &zero, sizeof(zero), cudaMemcpyHostToDevice, g->stream));
+  double* const* B = g->Bf[g->cur];
+  divb_face_kernel<<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, B[0], B[1], B[2], g->sc);
+  g->launches++;
+  CK(cudaGetLastError());
+  int rc = read_scalars(g);
+  if (rc) return rc;
+  long long bits = (long long)g->sc_host->max_bits;
+  double val;
+  memcpy(&val, &bits, sizeof(val));
+  *max_abs = val;
+  return KH_OK;
+}
+
 int kh_count_flags(kh_grid* g, long long* n_pflag, long long* n_fflag) {
   if (!g) return KH_EINVAL;
   int rc = read_scalars(g);
@@ -627,7 +689,9 @@ int kh_debug_predictor(kh_grid* g, double dt) {
   if (!g || !(dt > 0.0)) return KH_EINVAL;
   set_dt_kernel<<<1, 1, 0, g->stream>>>(g->sc, dt, 0);
   g->launches++;
-  int rc = substep(g, g->P[g->cur], g->P[g->cur], g->P[(g->cur + 1) % 3], 0.5, false);
+  const bool face = g->p.transport == KH_B_FACE_CT;
+  int rc = substep(g, g->P[g->cur], g->P[g->cur], g->P[(g->cur + 1) % 3], 0.5, false, face ? g->Bf[g->cur] : nullptr,
+                   face ? g->Bf[(g->cur + 1) % 3] : nullptr);
   if (rc) return rc;
   g->cur = (g->cur + 1) % 3;
   CK(cudaStreamSynchronize(g->stream));

@@ -454,3 +454,50 @@ def test_one_step_normal_frame_floors(kh, kho, case):
         z = np.zeros_like(gg.get_flags()[0])
         _assert_step_parity(p, gg.get_prims(), go.get_prims(), z, z, "normal-frame fix-up")     # the S23 metric
         assert (gg.get_flags()[1] != go.get_flags()[1]).mean() < 1e-3
+
+
+# ------------------------------------------------------------------------------------------ face-centred CT (NEXT-1)
+def _face_pair(kh, kho, p, P0, faces):
+    p = dict(p, transport=kp.B_FACE_CT)
+    gg, go = kh.Grid(p), kho.Grid(p, omp=True)
+    for g in (gg, go):
+        g.set_prims(P0)
+        g.set_face_B(*faces)
+    return p, gg, go
+
+
+@pytest.mark.parametrize("case", ["minkowski_weno5", "torus_mc", "torus_weno5_kastaun_fofc"])
+def test_face_centred_ct_parity(kh, kho, case):
+    """kh_params.transport = KH_B_FACE_CT on both sides: the face field agrees to round-off, its
+    divergence stays at round-off on both sides, the primitives meet the one-step and run bars."""
+    from kharm_inputs import facefield
+    if case == "minkowski_weno5":
+        p = ki.config_params(5, n=(24, 18, 10), recon=kp.RECON_WENO5)
+        P0 = modes.config5(p, seed=2, amp=1e-2)
+        faces = facefield.face_from_potential(p, *facefield.periodic_potential(p, seed=3, amp=5e-2))
+    else:
+        p = ki.config_params(3, n=(48, 32, 8), recon=kp.RECON_MC if case == "torus_mc" else kp.RECON_WENO5)
+        if case != "torus_mc":
+            p = dict(p, inverter=kp.INV_KASTAUN, fofc=1)
+        P0 = torus.torus_state(p, seed=2)
+        faces = facefield.face_from_potential(p, *facefield.axisymmetric_loop_potential(p, amp=2e-3, x1c=2.3))
+    p, gg, go = _face_pair(kh, kho, p, P0, faces)
+    assert np.array_equal(gg.get_prims(with_ghosts=True)[:5], go.get_prims(with_ghosts=True)[:5])
+    assert np.allclose(gg.get_prims(with_ghosts=True)[5:], go.get_prims(with_ghosts=True)[5:], rtol=1e-13, atol=1e-300)
+    d0 = go.divB_face()
+    assert gg.divB_face() <= 2 * d0 + 1e-16
+    dt = go.estimate_dt()
+    assert abs(gg.estimate_dt() / dt - 1) < 1e-12
+    n_g, n_o = gg.step(dt), go.step(dt)
+    assert abs(n_g / n_o - 1) < 1e-11
+    _assert_step_parity(p, gg.get_prims(), go.get_prims(), gg.get_flags()[0], go.get_flags()[0], "face-CT " + case)
+    for _ in range(9):
+        n_g, n_o = gg.step(n_g), go.step(n_o)
+    l1 = l1_diff(p, gg.get_prims(), go.get_prims())
+    assert l1.max() <= TOL_RUN_L1, l1
+    fg, fo = gg.get_face_B(), go.get_face_B()
+    I = (slice(3, -3), slice(3, -3), slice(3, -3))
+    for d in range(3):
+        sc = max(np.abs(fo[d][I]).max(), 1e-300)
+        assert np.abs(fg[d][I] - fo[d][I]).max() <= 1e-9 * max(sc, np.abs(fo[0][I]).max()), d
+    assert gg.divB_face() <= 1e-11 * max(np.abs(fo[0]).max(), np.abs(fo[1]).max()) * max(p["n1"], p["n2"]) + 4 * d0
