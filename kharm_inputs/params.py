@@ -14,6 +14,7 @@ RECON_MC, RECON_WENO5 = 0, 1
 INV_1DW, INV_KASTAUN = 0, 1
 FRAME_FLUID, FRAME_DRIFT, FRAME_NORMAL = 0, 1, 2
 B_FLUX_CT, B_FACE_CT = 0, 1
+EMF_ARITHMETIC, EMF_UPWIND = 0, 1
 
 FLOOR_DEFAULTS = dict(rho_min=1e-6, u_min=1e-8, r_char=10.0, bsq_over_rho_max=100.0, bsq_over_u_max=1e4,
                       u_over_rho_max=100.0, gamma_max=50.0, dt_growth_max=1.3)
@@ -22,7 +23,7 @@ FLOOR_DEFAULTS = dict(rho_min=1e-6, u_min=1e-8, r_char=10.0, bsq_over_rho_max=10
 def base_params(**kw):
     p = dict(coords=MINKOWSKI, a=0.0, hslope=0.3, poly_xt=0.82, poly_alpha=14.0, mks_smooth=0.5,
              n1=16, n2=16, n3=16, xmin=[0.0, 0.0, 0.0], xmax=[1.0, 1.0, 1.0], bc=[BC_PERIODIC] * 6,
-             gamma=4.0 / 3.0, cfl=0.9, recon=RECON_MC, inverter=INV_1DW, fofc=0, floor_frame=FRAME_FLUID, transport=B_FLUX_CT)
+             gamma=4.0 / 3.0, cfl=0.9, recon=RECON_MC, inverter=INV_1DW, fofc=0, floor_frame=FRAME_FLUID, transport=B_FLUX_CT, emf=EMF_ARITHMETIC)
     p.update(FLOOR_DEFAULTS)
     p.update(kw)
     return p

@@ -828,10 +828,11 @@ void compute_flux(kho_grid& g, const double* Ps, int d) {
 }
 
 // C5. Flux-CT (S15a).  Works on raw face-flux arrays so the invariant can be tested on arbitrary fluxes.
-void flux_ct(const kho_grid& g, double* F1, double* F2, double* F3, double* e1, double* e2, double* e3) {
+void flux_ct(const kho_grid& g, double* F1, double* F2, double* F3, double* e1, double* e2, double* e3, bool have_emf = false) {
   const long nt = g.ntot;
   const int N1 = g.n[0], N2 = g.n[1], N3 = g.n[2];
   auto X = [&](int i, int j, int k) { return g.idx(i, j, k); };
+  if (!have_emf)
   for (int k = 0; k <= N3; k++) for (int j = 0; j <= N2; j++) for (int i = 0; i <= N1; i++) {
     long n = X(i, j, k);
     if (k < N3)
@@ -858,6 +859,62 @@ void flux_ct(const kho_grid& g, double* F1, double* F2, double* F3, double* e1, 
       F3[B3 * nt + n] = 0.0;
       F3[B1 * nt + n] = 0.5 * (e2[n] + e2[X(i + 1, j, k)]);
       F3[B2 * nt + n] = -0.5 * (e1[n] + e1[X(i, j + 1, k)]);
+    }
+  }
+}
+
+// Upwinded edge EMFs (EMFs "along zone edges with and without upwinding"; reading
+// S29): the contact-upwind construction of Gardiner & Stone (2005), restated for the three components.  For component c
+// with (a, b) cyclic, eps_c = F^a[B^b] = -F^b[B^a]; per zone n (lower faces / lower edge):
+//   efa(n) = F^a[B^b](n),  efb(n) = -F^b[B^a](n),  ec(n) = sqrt(-g) (B^b u^a - B^a u^b)/u^t at the zone centre,
+//   gradients across half zones:  da_m(n) = 2 (efa(n) - ec(n - s_a)),  da_p(n) = 2 (ec(n) - efa(n))   (and b likewise),
+//   each upwinded in the OTHER direction by the sign of the mass flux through the face between the two candidates,
+//   eps_edge = 1/4 (efa(n) + efa(n - s_b) + efb(n) + efb(n - s_a))
+//            + 1/8 [ up_a(db_m; M_a(n - s_b)) - up_a(db_p; M_a(n)) ] + 1/8 [ up_b(da_m; M_b(n - s_a)) - up_b(da_p; M_b(n)) ],
+//   up_a(d; M) = d(n - s_a) if M > 0, d(n) if M < 0, their mean if M = 0.
+// For plane-parallel, grid-aligned flow this reduces to the one-dimensional face value (the design condition of that
+// paper; pinned in tests/test_oracle_facect.py).  Writes the same emf arrays as flux_ct's first loop.
+void emf_upwind(const kho_grid& g, const double* Ps, const double* F1, const double* F2, const double* F3, double* e1, double* e2, double* e3) {
+  const long nt = g.ntot;
+  const long st[3] = {1, g.nt[0], (long)g.nt[0] * g.nt[1]};
+  const double* F[3] = {F1, F2, F3};
+  double* E[3] = {e1, e2, e3};
+  // zone-centred reference values, zones -1 .. N in every direction
+  std::vector<double> ec[3];
+  for (int c = 0; c < 3; c++) ec[c].assign(nt, 0.0);
+  for (int k = -1; k <= g.n[2]; k++) for (int j = -1; j <= g.n[1]; j++) for (int i = -1; i <= g.n[0]; i++) {
+    long n = g.idx(i, j, k);
+    const Geom& G = g.G[0][g.idx2(i, j)];
+    double P[NP];
+    get_prim(g, Ps, n, P);
+    FourVec D;
+    four_vectors(G.gcov, G.gcon, P, D);
+    for (int c = 0; c < 3; c++) {
+      int a = (c + 1) % 3, b = (c + 2) % 3;
+      ec[c][n] = G.gdet * (P[B1 + b] * D.ucon[1 + a] - P[B1 + a] * D.ucon[1 + b]) / D.ucon[0];
+    }
+  }
+  for (int c = 0; c < 3; c++) {
+    const int a = (c + 1) % 3, b = (c + 2) % 3;
+    const long sa = st[a], sb = st[b];
+    const double* Fa = F[a]; const double* Fb = F[b];
+    auto efa = [&](long n) { return Fa[(B1 + b) * nt + n]; };
+    auto efb = [&](long n) { return -Fb[(B1 + a) * nt + n]; };
+    auto da_m = [&](long n) { return 2.0 * (efa(n) - ec[c][n - sa]); };
+    auto da_p = [&](long n) { return 2.0 * (ec[c][n] - efa(n)); };
+    auto db_m = [&](long n) { return 2.0 * (efb(n) - ec[c][n - sb]); };
+    auto db_p = [&](long n) { return 2.0 * (ec[c][n] - efb(n)); };
+    auto up = [&](double lo, double hi, double M) { return M > 0.0 ? lo : (M < 0.0 ? hi : 0.5 * (lo + hi)); };
+    int hi[3] = {g.n[0] + 1, g.n[1] + 1, g.n[2] + 1};
+    hi[c] = g.n[c];                                        // edges along c: zones 0 .. N_c - 1 in that direction
+    for (int k = 0; k < hi[2]; k++) for (int j = 0; j < hi[1]; j++) for (int i = 0; i < hi[0]; i++) {
+      long n = g.idx(i, j, k);
+      double Ma0 = Fa[RHO * nt + n], Ma1 = Fa[RHO * nt + n - sb], Mb0 = Fb[RHO * nt + n], Mb1 = Fb[RHO * nt + n - sa];
+      double v = 0.25 * (efa(n) + efa(n - sb) + efb(n) + efb(n - sa))
+               + 0.125 * (up(db_m(n - sa), db_m(n), Ma1) - up(db_p(n - sa), db_p(n), Ma0))
+               + 0.125 * (up(da_m(n - sb), da_m(n), Mb1) - up(da_p(n - sb), da_p(n), Mb0));
+      if (c != 1 && polar_face(g, j)) v = 0.0;             // S10
+      E[c][n] = v;
     }
   }
 }
@@ -973,7 +1030,8 @@ void substep(kho_grid& g, const double* Pi, const double* Ps, double* Pf, double
   if (g.p.fofc) {
     // speculative update with the high-order fluxes: which zones would fail the inversion or hit a floor?
     std::vector<double> raw[3] = {g.F[0], g.F[1], g.F[2]};                      // flux_ct rewrites the B components in place
-    flux_ct(g, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data());
+    if (g.p.emf == KHO_EMF_UPWIND) emf_upwind(g, Ps, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data());
+    flux_ct(g, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data(), g.p.emf == KHO_EMF_UPWIND);
     if (Pf != Pi) std::memcpy(Pf, Pi, sizeof(double) * NP * nt);
     update_zones(g, Pi, Ps, Pf, Dt);
     std::vector<int> mask(nt, 0);
@@ -982,7 +1040,8 @@ void substep(kho_grid& g, const double* Pi, const double* Ps, double* Pf, double
     for (int d = 0; d < 3; d++) g.F[d] = raw[d];
     fofc_reflux(g, Ps, mask);
   }
-  flux_ct(g, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data());
+  if (g.p.emf == KHO_EMF_UPWIND) emf_upwind(g, Ps, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data());
+  flux_ct(g, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data(), g.p.emf == KHO_EMF_UPWIND);
   if (Pf != Pi) std::memcpy(Pf, Pi, sizeof(double) * NP * nt);   // ghosts of Pf start from Pi (matters for FIXED)
   if (Bfi) face_ct_update(g, Bfi, Bff, Dt);
   update_zones(g, Pi, Ps, Pf, Dt, Bfi ? Bff : nullptr);
@@ -1269,6 +1328,19 @@ int kho_divB_face(kho_grid* g, double* max_abs) {
     if (std::fabs(div) > m) m = std::fabs(div);
   }
   *max_abs = m;
+  return KHO_OK;
+}
+int kho_debug_emf(kho_grid* g) {
+  if (!g) return KHO_EINVAL;
+  const double* P = g->P.data();
+  for (int d = 0; d < 3; d++) compute_flux(*g, P, d);
+  if (g->p.emf == KHO_EMF_UPWIND) {
+    emf_upwind(*g, P, g->F[0].data(), g->F[1].data(), g->F[2].data(), g->emf[0].data(), g->emf[1].data(), g->emf[2].data());
+  } else {
+    std::vector<double> raw[3] = {g->F[0], g->F[1], g->F[2]};
+    flux_ct(*g, g->F[0].data(), g->F[1].data(), g->F[2].data(), g->emf[0].data(), g->emf[1].data(), g->emf[2].data());
+    for (int d = 0; d < 3; d++) g->F[d] = raw[d];
+  }
   return KHO_OK;
 }
 int kho_debug_fofc(kho_grid* g, const int* mask_with_ghosts) {

@@ -27,6 +27,7 @@ enum { KHO_RECON_MC = 0, KHO_RECON_WENO5 = 1 };
 enum { KHO_INV_1DW = 0, KHO_INV_KASTAUN = 1 };
 enum { KHO_FRAME_FLUID = 0, KHO_FRAME_DRIFT = 1, KHO_FRAME_NORMAL = 2 };
 enum { KHO_B_FLUX_CT = 0, KHO_B_FACE_CT = 1 };
+enum { KHO_EMF_ARITHMETIC = 0, KHO_EMF_UPWIND = 1 };
 enum { KHO_LOC_CENT = 0, KHO_LOC_FACE1 = 1, KHO_LOC_FACE2 = 2, KHO_LOC_FACE3 = 3 };
 
 typedef struct {
@@ -44,6 +45,7 @@ typedef struct {
   int fofc;                                        /* 1: first-order flux correction (NEXT-3) */
   int floor_frame;                                 /* KHO_FRAME_FLUID | _DRIFT | _NORMAL (NEXT-4) */
   int transport;                                   /* KHO_B_FLUX_CT | KHO_B_FACE_CT (NEXT-1) */
+  int emf;                                         /* KHO_EMF_ARITHMETIC | KHO_EMF_UPWIND (NEXT-1) */
 } kho_params;
 
 typedef struct kho_grid kho_grid;
@@ -72,6 +74,9 @@ int kho_get_conn(kho_grid* g, double* conn64);            /* [(n2+6)(n1+6)][lam]
 int kho_fill_ghosts(kho_grid* g);
 /* test hook: C9 fix-up (+ floors) of the current primitives for a caller-supplied pflag array [nt] */
 int kho_debug_fixup(kho_grid* g, const int* pflag_with_ghosts);
+/* test hook (NEXT-1): high-order fluxes of the current primitives and the edge EMFs of the configured kind; leaves the RAW
+ * face fluxes (no Flux-CT rewrite) for kho_get_flux and the EMFs for kho_get_emf */
+int kho_debug_emf(kho_grid* g);
 /* test hook (NEXT-3): high-order fluxes of the current primitives, then the first-order flux correction for a caller-
  * supplied zone mask [nt] (its ghosts are filled like pflag); leaves the RAW fluxes (no Flux-CT) for kho_get_flux */
 int kho_debug_fofc(kho_grid* g, const int* mask_with_ghosts);

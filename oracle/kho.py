@@ -27,7 +27,7 @@ class Params(C.Structure):
         ("gamma", C.c_double), ("cfl", C.c_double), ("recon", C.c_int),
         ("rho_min", C.c_double), ("u_min", C.c_double), ("r_char", C.c_double),
         ("bsq_over_rho_max", C.c_double), ("bsq_over_u_max", C.c_double), ("u_over_rho_max", C.c_double),
-        ("gamma_max", C.c_double), ("dt_growth_max", C.c_double), ("inverter", C.c_int), ("fofc", C.c_int), ("floor_frame", C.c_int), ("transport", C.c_int),
+        ("gamma_max", C.c_double), ("dt_growth_max", C.c_double), ("inverter", C.c_int), ("fofc", C.c_int), ("floor_frame", C.c_int), ("transport", C.c_int), ("emf", C.c_int),
     ]
 
 
@@ -277,6 +277,9 @@ class Grid:
         m = C.c_double()
         _chk(self.L.kho_divB_face(self.h, C.byref(m)))
         return m.value
+
+    def debug_emf(self):
+        _chk(self.L.kho_debug_emf(self.h))
 
     def debug_fofc(self, mask_with_ghosts):
         m = np.ascontiguousarray(mask_with_ghosts, dtype=np.int32)

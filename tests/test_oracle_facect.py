@@ -99,3 +99,83 @@ def test_torus_face_ct_matches_flux_ct_and_axis_faces_stay_empty(kho):
         assert np.array_equal(f[1][NG:-NG, jj, NG:-NG], faces[1][NG:-NG, jj, NG:-NG])
         assert np.abs(f[1][NG:-NG, jj, NG:-NG]).max() < 1e-30
     assert g_face.divB_face() < 1e-14
+
+
+# ------------------------------------------------------------------------------------------ upwinded edge EMFs (S29)
+def _one_d_state(p, d, seed):
+    """A state that varies only along direction d (1..3), moving along d, with all three field components."""
+    rng = np.random.default_rng(seed)
+    n = (p["n1"], p["n2"], p["n3"])[d - 1]
+    x = (np.arange(n) + 0.5) / n
+    prof = lambda a, b: a + b * np.sin(2 * np.pi * x + rng.uniform(0, 6.28))
+    shp = [1, 1, 1]; shp[3 - d] = n
+    P = np.zeros((8, p["n3"], p["n2"], p["n1"]))
+    P[0] = prof(1.0, 0.3).reshape(shp); P[1] = prof(0.5, 0.2).reshape(shp)
+    P[1 + d] = prof(0.1, 0.4).reshape(shp)                       # velocity along d, changing sign
+    for e in (1, 2, 3):
+        P[4 + e] = 0.3 if e == d else prof(0.2, 0.5).reshape(shp)
+    return P
+
+
+def test_upwinded_emf_reduces_to_the_face_value_for_grid_aligned_flow(kho):
+    """The design condition of the contact-upwind EMF: plane-parallel flow along a grid direction must see the
+    one-dimensional face value at the edge (no multidimensional averaging left)."""
+    p = dict(ki.config_params(5, n=(12, 10, 8), recon=kp.RECON_WENO5), emf=kp.EMF_UPWIND)
+    I = (slice(NG, -NG),) * 3
+    for d in (1, 2, 3):
+        g = kho.Grid(p)
+        g.set_prims(_one_d_state(p, d, seed=d))
+        g.debug_emf()
+        F, _ = g.get_flux(d)                                       # raw face fluxes of direction d
+        a, b = d % 3 + 1, (d + 1) % 3 + 1                          # (d, a, b) cyclic
+        e_b, e_a = g.get_emf(b), g.get_emf(a)
+        # eps_b = F^d[B^a] ... with (b; d, a) cyclic: eps_b = F^d[B^a];  eps_a = -F^d[B^b] with (a; b, d) cyclic
+        assert np.abs(e_b[I] - F[4 + a][I]).max() <= 1e-14 * np.abs(F[4 + a][I]).max(), d
+        assert np.abs(e_a[I] + F[4 + b][I]).max() <= 1e-14 * np.abs(F[4 + b][I]).max(), d
+        # the arithmetic average does NOT have this property (it mixes in the zone-centred values)
+        g0 = kho.Grid(dict(p, emf=kp.EMF_ARITHMETIC))
+        g0.set_prims(_one_d_state(p, d, seed=d)); g0.debug_emf()
+        assert np.abs(g0.get_emf(b)[I] - F[4 + a][I]).max() > 1e-4
+
+
+def test_upwinded_emf_uniform_state_and_face_divergence(kho):
+    from kharm_inputs import facefield
+    p = dict(ki.config_params(5, n=(8, 8, 8)), emf=kp.EMF_UPWIND)
+    P0 = np.zeros((8, 8, 8, 8)); P0[0] = 1.0; P0[1] = 0.7; P0[2] = 0.3; P0[3] = -0.2; P0[4] = 0.1; P0[5] = 0.4; P0[6] = -0.3; P0[7] = 0.2
+    g = kho.Grid(p); g.set_prims(P0); g.debug_emf()
+    gamma = np.sqrt(1 + 0.3 ** 2 + 0.2 ** 2 + 0.1 ** 2)
+    v = np.array([0.3, -0.2, 0.1]) / gamma; B = np.array([0.4, -0.3, 0.2])
+    I = (slice(NG, -NG),) * 3
+    for c in range(3):
+        a, b = (c + 1) % 3, (c + 2) % 3
+        assert np.allclose(g.get_emf(c + 1)[I], B[b] * v[a] - B[a] * v[b], rtol=1e-13, atol=1e-15)
+    # a run: the face divergence stays at round-off, and the result differs from the arithmetic-EMF run
+    q = ki.config_params(5, n=(12, 10, 8), recon=kp.RECON_WENO5)
+    P0 = modes.config5(q, seed=2, amp=5e-2)
+    faces = facefield.face_from_potential(q, *facefield.periodic_potential(q, seed=3, amp=5e-2))
+    res = []
+    for emf in (kp.EMF_ARITHMETIC, kp.EMF_UPWIND):
+        g = kho.Grid(dict(q, transport=kp.B_FACE_CT, emf=emf))
+        g.set_prims(P0); g.set_face_B(*faces)
+        dt = g.estimate_dt()
+        for _ in range(5):
+            dt = g.step(dt)
+        assert g.divB_face() < 1e-12
+        res.append(g.get_prims())
+    d = np.abs(res[0][5:] - res[1][5:]).max()
+    assert 1e-9 < d < 0.2 * np.abs(res[0][5:]).max()          # a different, but not a wildly different, discretisation
+
+
+def test_upwinded_emf_keeps_second_order_convergence_of_a_rotated_mode(kho):
+    errs = []
+    for n in (16, 32):
+        p = dict(ki.config_params(1, n=(n, n, 4)), emf=kp.EMF_UPWIND)
+        P0, T = modes.config1(p, rotated=True)
+        g = kho.Grid(p, omp=True); g.set_prims(P0)
+        dt, t = g.estimate_dt(), 0.0
+        while t < T * (1 - 1e-12):
+            dt = min(dt, T - t); t += dt
+            dt = g.step(dt)
+        errs.append(np.abs(g.get_prims() - P0).mean(axis=(1, 2, 3)).max())
+    slope = np.log2(errs[0] / errs[1])
+    assert 1.7 < slope < 2.4, (errs, slope)
