@@ -44,6 +44,7 @@ WORKLOADS = {
     "torus_sane_192x128x128_weno5_fofc": (3, None, None),         # same block, kh_params.fofc = 1
     "torus_sane_192x128x128_weno5_drift": (3, None, None),        # same block, kh_params.floor_frame = KH_FRAME_DRIFT
     "torus_sane_192x128x128_weno5_facect": (3, None, None),       # same block, kh_params.transport = KH_B_FACE_CT
+    "torus_sane_192x128x128_weno5_facect_upwind": (3, None, None),  # ... and kh_params.emf = KH_EMF_UPWIND
     "minkowski_128_mc": (5, 128, 0), "minkowski_128_weno5": (5, 128, 1),
     "minkowski_256_mc": (5, 256, 0), "minkowski_256_weno5": (5, 256, 1),
     "minkowski_64_mc": (5, 64, 0), "minkowski_192_mc": (5, 192, 0), "minkowski_320_mc": (5, 320, 0),
@@ -96,8 +97,10 @@ def workload_params(name):
         p["fofc"] = 1
     if name.endswith("_drift"):
         p["floor_frame"] = ki.params.FRAME_DRIFT
-    if name.endswith("_facect"):
+    if name.endswith("_facect") or name.endswith("_facect_upwind"):
         p["transport"] = ki.params.B_FACE_CT
+    if name.endswith("_upwind"):
+        p["emf"] = ki.params.EMF_UPWIND
     return cfg, p
 
 

@@ -40,6 +40,7 @@ enum { KH_RECON_MC = 0, KH_RECON_WENO5 = 1 };                                 /*
 enum { KH_INV_1DW = 0, KH_INV_KASTAUN = 1 };
 enum { KH_FRAME_FLUID = 0, KH_FRAME_DRIFT = 1, KH_FRAME_NORMAL = 2 };
 enum { KH_B_FLUX_CT = 0, KH_B_FACE_CT = 1 };
+enum { KH_EMF_ARITHMETIC = 0, KH_EMF_UPWIND = 1 };
 enum { KH_MEM_DEVICE = 0, KH_MEM_HOST = 1 };
 enum { KH_LOC_CENT = 0, KH_LOC_FACE1 = 1, KH_LOC_FACE2 = 2, KH_LOC_FACE3 = 3 };
 
@@ -64,7 +65,9 @@ typedef struct {
                                  KH_FRAME_NORMAL (added as gas at rest for the normal observer, then re-inverted)   */
   int transport;              /* magnetic field transport: KH_B_FLUX_CT (zone-centred field, Toth's Flux-CT) |
                                  KH_B_FACE_CT (face-centred field advanced by the circulation of the edge EMFs;
-                                 EMF = arithmetic four-point average; needs kh_set_face_B)                     */
+                                 needs kh_set_face_B)                                                          */
+  int emf;                    /* edge EMFs of either transport ("with and without upwinding"): KH_EMF_ARITHMETIC
+                                 (four-point average of the face fluxes) | KH_EMF_UPWIND (contact-upwinded)     */
 } kh_params;
 
 typedef struct kh_grid kh_grid;   /* opaque */

@@ -871,7 +871,9 @@ void flux_ct(const kho_grid& g, double* F1, double* F2, double* F3, double* e1, 
 //   each upwinded in the OTHER direction by the sign of the mass flux through the face between the two candidates,
 //   eps_edge = 1/4 (efa(n) + efa(n - s_b) + efb(n) + efb(n - s_a))
 //            + 1/8 [ up_a(db_m; M_a(n - s_b)) - up_a(db_p; M_a(n)) ] + 1/8 [ up_b(da_m; M_b(n - s_a)) - up_b(da_p; M_b(n)) ],
-//   up_a(d; M) = d(n - s_a) if M > 0, d(n) if M < 0, their mean if M = 0.
+//   up_a(d; M) = d(n - s_a) if M > tol Dsum, d(n) if M < -tol Dsum, their mean otherwise, where Dsum is the sum of the
+//   conserved densities sqrt(-g) rho u^t of the two zones the face separates and tol = 1e-10: a mass flux that small is
+//   "no flow" (by symmetry it is often exactly zero, and then its computed sign is round-off noise).
 // For plane-parallel, grid-aligned flow this reduces to the one-dimensional face value (the design condition of that
 // paper; pinned in tests/test_oracle_facect.py).  Writes the same emf arrays as flux_ct's first loop.
 void emf_upwind(const kho_grid& g, const double* Ps, const double* F1, const double* F2, const double* F3, double* e1, double* e2, double* e3) {
@@ -880,7 +882,7 @@ void emf_upwind(const kho_grid& g, const double* Ps, const double* F1, const dou
   const double* F[3] = {F1, F2, F3};
   double* E[3] = {e1, e2, e3};
   // zone-centred reference values, zones -1 .. N in every direction
-  std::vector<double> ec[3];
+  std::vector<double> ec[3], Dc(nt, 0.0);
   for (int c = 0; c < 3; c++) ec[c].assign(nt, 0.0);
   for (int k = -1; k <= g.n[2]; k++) for (int j = -1; j <= g.n[1]; j++) for (int i = -1; i <= g.n[0]; i++) {
     long n = g.idx(i, j, k);
@@ -893,6 +895,7 @@ void emf_upwind(const kho_grid& g, const double* Ps, const double* F1, const dou
       int a = (c + 1) % 3, b = (c + 2) % 3;
       ec[c][n] = G.gdet * (P[B1 + b] * D.ucon[1 + a] - P[B1 + a] * D.ucon[1 + b]) / D.ucon[0];
     }
+    Dc[n] = G.gdet * P[RHO] * D.ucon[0];
   }
   for (int c = 0; c < 3; c++) {
     const int a = (c + 1) % 3, b = (c + 2) % 3;
@@ -904,15 +907,18 @@ void emf_upwind(const kho_grid& g, const double* Ps, const double* F1, const dou
     auto da_p = [&](long n) { return 2.0 * (ec[c][n] - efa(n)); };
     auto db_m = [&](long n) { return 2.0 * (efb(n) - ec[c][n - sb]); };
     auto db_p = [&](long n) { return 2.0 * (ec[c][n] - efb(n)); };
-    auto up = [&](double lo, double hi, double M) { return M > 0.0 ? lo : (M < 0.0 ? hi : 0.5 * (lo + hi)); };
+    auto up = [&](double lo, double hi, double M, double Dsum) {
+      const double t = 1e-10 * Dsum;
+      return M > t ? lo : (M < -t ? hi : 0.5 * (lo + hi));
+    };
     int hi[3] = {g.n[0] + 1, g.n[1] + 1, g.n[2] + 1};
     hi[c] = g.n[c];                                        // edges along c: zones 0 .. N_c - 1 in that direction
     for (int k = 0; k < hi[2]; k++) for (int j = 0; j < hi[1]; j++) for (int i = 0; i < hi[0]; i++) {
       long n = g.idx(i, j, k);
       double Ma0 = Fa[RHO * nt + n], Ma1 = Fa[RHO * nt + n - sb], Mb0 = Fb[RHO * nt + n], Mb1 = Fb[RHO * nt + n - sa];
       double v = 0.25 * (efa(n) + efa(n - sb) + efb(n) + efb(n - sa))
-               + 0.125 * (up(db_m(n - sa), db_m(n), Ma1) - up(db_p(n - sa), db_p(n), Ma0))
-               + 0.125 * (up(da_m(n - sb), da_m(n), Mb1) - up(da_p(n - sb), da_p(n), Mb0));
+               + 0.125 * (up(db_m(n - sa), db_m(n), Ma1, Dc[n - sb - sa] + Dc[n - sb]) - up(db_p(n - sa), db_p(n), Ma0, Dc[n - sa] + Dc[n]))
+               + 0.125 * (up(da_m(n - sb), da_m(n), Mb1, Dc[n - sa - sb] + Dc[n - sa]) - up(da_p(n - sb), da_p(n), Mb0, Dc[n - sb] + Dc[n]));
       if (c != 1 && polar_face(g, j)) v = 0.0;             // S10
       E[c][n] = v;
     }

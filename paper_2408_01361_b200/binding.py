@@ -40,7 +40,7 @@ class Params(C.Structure):
         ("gamma", C.c_double), ("cfl", C.c_double), ("recon", C.c_int),
         ("rho_min", C.c_double), ("u_min", C.c_double), ("r_char", C.c_double),
         ("bsq_over_rho_max", C.c_double), ("bsq_over_u_max", C.c_double), ("u_over_rho_max", C.c_double),
-        ("gamma_max", C.c_double), ("dt_growth_max", C.c_double), ("inverter", C.c_int), ("fofc", C.c_int), ("floor_frame", C.c_int), ("transport", C.c_int),
+        ("gamma_max", C.c_double), ("dt_growth_max", C.c_double), ("inverter", C.c_int), ("fofc", C.c_int), ("floor_frame", C.c_int), ("transport", C.c_int), ("emf", C.c_int),
     ]
 
 

@@ -255,7 +255,10 @@ __device__ __forceinline__ void llf_row(const StateQ& S, double s, double Gs[KH_
   if (DIR == 1) T1 += S.ptot;
   if (DIR == 2) T2 += S.ptot;
   if (DIR == 3) T3 += S.ptot;
-  Gs[RHO] = S.rho * us;
+  // not contractable into the caller's sum of the two states: with mirror-symmetric states the two mass-flux terms are
+  // exact negatives and must cancel to an exact zero (an FMA would leave the rounding error of one product), which the
+  // contact-upwinded EMFs read as "no flow through this face"
+  Gs[RHO] = __dmul_rn(S.rho, us);
   Gs[UU] = fma(S.rho, us, T0);
   Gs[U1] = T1; Gs[U2] = T2; Gs[U3] = T3;
   constexpr int I = (DIR == 1) ? 2 : 1, J = (DIR == 3) ? 2 : 3;

@@ -266,6 +266,80 @@ emf_kernel(GV g, const double* __restrict__ F1, const double* __restrict__ F2, c
   }
 }
 
+// Upwinded edge EMFs ("with and without upwinding"; S29): the contact-upwind
+// construction of Gardiner & Stone.  ecent_kernel tabulates the zone-centred reference values
+//   ec_c = sqrt(-g) (B^b v^a - B^a v^b),  v^i = u^i/u^t = ut^i alpha/gamma - alpha^2 g^{ti},  (c, a, b) cyclic,
+// on zones -1 .. N; emf_upwind_kernel then forms, per edge, the four-point face average plus the half-zone gradient
+// differences, each upwinded by the sign of the mass flux through the face between its two candidates.
+template <bool FLAT>
+__global__ void __launch_bounds__(128)
+ecent_kernel(GV g, const double* __restrict__ P, double* __restrict__ c1, double* __restrict__ c2, double* __restrict__ c3,
+             double* __restrict__ dc) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x - 1, j = (int)blockIdx.y - 1, k = (int)blockIdx.z - 1;
+  if (i > g.n1) return;
+  const long n = zidx(g, i, j, k), nt = g.ntot;
+  Geo G;
+  load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, pidx(g, i, j));
+  const double u1 = P[U1 * nt + n], u2 = P[U2 * nt + n], u3 = P[U3 * nt + n];
+  const double b1 = P[B1 * nt + n], b2 = P[B2 * nt + n], b3 = P[B3 * nt + n];
+  const double ig = 1.0 / sqrt(1.0 + spatial_norm2<FLAT>(G, u1, u2, u3));
+  double v1, v2, v3;
+  if (FLAT) { v1 = u1 * ig; v2 = u2 * ig; v3 = u3 * ig; }
+  else {
+    const double ag = G.alpha * ig, a2 = G.alpha * G.alpha;
+    v1 = fma(u1, ag, -a2 * G.n01); v2 = fma(u2, ag, -a2 * G.n02); v3 = u3 * ag;     // g^03 = 0
+  }
+  const double sg = FLAT ? 1.0 : G.gdet;
+  c1[n] = sg * (b3 * v2 - b2 * v3);
+  c2[n] = sg * (b1 * v3 - b3 * v1);
+  c3[n] = sg * (b2 * v1 - b1 * v2);
+  dc[n] = sg * P[RHO * nt + n] / (FLAT ? ig : ig * G.alpha);        // conserved density sqrt(-g) rho u^t: scale of the mass fluxes
+}
+
+// upwind choice by the mass flux M through the face between the two candidates; |M| <= 1e-10 of the two zones' conserved
+// densities is "no flow" (often an exact zero by symmetry, whose computed sign would be round-off noise): the mean
+__device__ __forceinline__ double upw(double lo, double hi, double M, double Dsum) {
+  const double t = 1e-10 * Dsum;
+  return M > t ? lo : (M < -t ? hi : 0.5 * (lo + hi));
+}
+
+// one edge value: Fa = F^a (component B^b is +eps), Fb = F^b (component B^a is -eps), ec the zone-centred table
+__device__ __forceinline__ double edge_emf_upwind(const double* __restrict__ Fa, const double* __restrict__ Fb, const double* __restrict__ ec,
+                                                  const double* __restrict__ dc, long nt, long n, long sa, long sb, int vb /* B^b slot */,
+                                                  int va /* B^a slot */) {
+  const double* fa = Fa + (long)vb * nt;
+  const double* fb = Fb + (long)va * nt;
+  const double efa0 = fa[n], efa_b = fa[n - sb], efa_ab = 0.0;
+  (void)efa_ab;
+  const double efb0 = -fb[n], efb_a = -fb[n - sa];
+  const double ec0 = ec[n], ec_a = ec[n - sa], ec_b = ec[n - sb], ec_ab = ec[n - sa - sb];
+  // gradients along b (at columns n - sa and n), below (m) and above (p) the b-faces
+  const double dbm_lo = 2.0 * (efb_a - ec_ab), dbm_hi = 2.0 * (efb0 - ec_b);
+  const double dbp_lo = 2.0 * (ec_a - efb_a), dbp_hi = 2.0 * (ec0 - efb0);
+  // gradients along a (at rows n - sb and n)
+  const double dam_lo = 2.0 * (efa_b - ec_ab), dam_hi = 2.0 * (efa0 - ec_a);
+  const double dap_lo = 2.0 * (ec_b - efa_b), dap_hi = 2.0 * (ec0 - efa0);
+  const double Ma0 = Fa[n], Ma1 = Fa[n - sb], Mb0 = Fb[n], Mb1 = Fb[n - sa];            // mass fluxes (slot RHO = 0)
+  const double d0 = dc[n], d_a = dc[n - sa], d_b = dc[n - sb], d_ab = dc[n - sa - sb];
+  return 0.25 * (efa0 + efa_b + efb0 + efb_a) + 0.125 * (upw(dbm_lo, dbm_hi, Ma1, d_ab + d_b) - upw(dbp_lo, dbp_hi, Ma0, d_a + d0)) +
+         0.125 * (upw(dam_lo, dam_hi, Mb1, d_ab + d_a) - upw(dap_lo, dap_hi, Mb0, d_b + d0));
+}
+
+__global__ void __launch_bounds__(128)
+emf_upwind_kernel(GV g, const double* __restrict__ F1, const double* __restrict__ F2, const double* __restrict__ F3,
+                  const double* __restrict__ c1, const double* __restrict__ c2, const double* __restrict__ c3, const double* __restrict__ dc,
+                  double* __restrict__ e1,
+                  double* __restrict__ e2, double* __restrict__ e3) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+  if (i > g.n1) return;
+  const long n = zidx(g, i, j, k), nt = g.ntot;
+  const bool axis = polar_face(g, j);
+  // (c; a, b) cyclic: eps_3 = F^1[B^2] = -F^2[B^1];  eps_1 = F^2[B^3] = -F^3[B^2];  eps_2 = F^3[B^1] = -F^1[B^3]
+  if (k < g.n3) { double v = edge_emf_upwind(F1, F2, c3, dc, nt, n, 1, g.s2, B2, B1); e3[n] = axis ? 0.0 : v; }
+  if (j < g.n2) { double v = edge_emf_upwind(F3, F1, c2, dc, nt, n, g.s3, 1, B1, B3); e2[n] = v; }
+  if (i < g.n1) { double v = edge_emf_upwind(F2, F3, c1, dc, nt, n, g.s2, g.s3, B3, B2); e1[n] = axis ? 0.0 : v; }
+}
+
 // ---------------------------------------------------------------------------------------------
 // K4 + K5 (+ K6 in the corrector): per interior zone
 //   U_f = U(P_i) + Dt [ -sum_d (F^d(+1) - F^d)/dx_d + S(P_s) ],  S_nu = sqrt(-g) T^kap_lam Gamma^lam_{nu kap}

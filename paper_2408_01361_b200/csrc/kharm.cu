@@ -39,6 +39,7 @@ struct kh_grid {
   double* ctop[3];
   double* emf[3];
   unsigned char *pflag, *fflag;
+  double* ecent[4];      // upwinded EMFs: zone-centred reference values + conserved density (allocated on demand)
   double* Bf[3][3];      // face-centred CT: Phi^d per rotation state [state][d], [ntot] each (allocated on demand)
   unsigned char* mask;   // FOFC: troubled zones of the speculative update (with ghost images)
   unsigned* faillist;    // zones (device-layout index) whose inversion failed in the current sub-step
@@ -191,7 +192,15 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
   const int passes = g->p.fofc ? 2 : 1;       // FOFC: a speculative update first, then the re-flux, then the real one
   for (int pass = 0; pass < passes; pass++) {
     prof_begin(g, KH_K_EMF);
-    emf_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], g->emf[2]);
+    if (g->p.emf == KH_EMF_UPWIND) {
+      if (g->flat) ecent_kernel<true><<<zone_grid(v.n1 + 2, v.n2 + 2, v.n3 + 2), 128, 0, g->stream>>>(v, Ps, g->ecent[0], g->ecent[1], g->ecent[2], g->ecent[3]);
+      else ecent_kernel<false><<<zone_grid(v.n1 + 2, v.n2 + 2, v.n3 + 2), 128, 0, g->stream>>>(v, Ps, g->ecent[0], g->ecent[1], g->ecent[2], g->ecent[3]);
+      emf_upwind_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, g->F[0], g->F[1], g->F[2], g->ecent[0], g->ecent[1],
+                                                                                          g->ecent[2], g->ecent[3], g->emf[0], g->emf[1], g->emf[2]);
+      g->launches++;
+    } else {
+      emf_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], g->emf[2]);
+    }
     prof_end(g);
     g->launches++;
     const unsigned grid = (unsigned)(((long)v.n1 * v.n2 * v.n3 + 127) / 128);
@@ -291,7 +300,8 @@ int kh_grid_destroy(kh_grid* g) {
   cudaFree(g->conn); cudaFree(g->dg); cudaFree(g->floorp);
   for (int b = 0; b < 3; b++) { cudaFree(g->P[b]); cudaFree(g->F[b]); cudaFree(g->ctop[b]); cudaFree(g->emf[b]); }
   cudaFree(g->pflag); cudaFree(g->fflag); cudaFree(g->mask);
-  for (int b = 0; b < 3; b++) for (int d = 0; d < 3; d++) cudaFree(g->Bf[b][d]); cudaFree(g->faillist); cudaFree(g->sc); cudaFree(g->fix); cudaFree(g->stage);
+  for (int b = 0; b < 3; b++) for (int d = 0; d < 3; d++) cudaFree(g->Bf[b][d]);
+  for (int d = 0; d < 4; d++) cudaFree(g->ecent[d]); cudaFree(g->faillist); cudaFree(g->sc); cudaFree(g->fix); cudaFree(g->stage);
   if (g->sc_host) cudaFreeHost(g->sc_host);
   if (g->pev) { for (int e = 0; e < 2 * KH_PROF_POOL; e++) if (g->pev[e]) cudaEventDestroy(g->pev[e]); delete[] g->pev; }
   delete[] g->pkind;
@@ -303,7 +313,7 @@ int kh_grid_destroy(kh_grid* g) {
 int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   if (!p || !out) return KH_EINVAL;
   if (p->n1 < 1 || p->n2 < 1 || p->n3 < 1) return KH_EINVAL;
-  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1 || p->inverter < 0 || p->inverter > 1 || p->fofc < 0 || p->fofc > 1 || p->floor_frame < 0 || p->floor_frame > 2 || p->transport < 0 || p->transport > 1) return KH_EINVAL;
+  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1 || p->inverter < 0 || p->inverter > 1 || p->fofc < 0 || p->fofc > 1 || p->floor_frame < 0 || p->floor_frame > 2 || p->transport < 0 || p->transport > 1 || p->emf < 0 || p->emf > 1) return KH_EINVAL;
   if (!(p->gamma > 1.0) || !(p->cfl > 0.0) || !(p->dt_growth_max > 0.0)) return KH_EINVAL;
   const int N[3] = {p->n1, p->n2, p->n3};
   for (int d = 0; d < 3; d++) {
@@ -385,6 +395,7 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   ALLOC(g->fflag, v.ntot);
   if (p->fofc) ALLOC(g->mask, v.ntot);
   if (p->transport == KH_B_FACE_CT) for (int b = 0; b < 3; b++) for (int d = 0; d < 3; d++) ALLOC(g->Bf[b][d], fb);
+  if (p->emf == KH_EMF_UPWIND) for (int d = 0; d < 4; d++) ALLOC(g->ecent[d], fb);
   ALLOC(g->faillist, sizeof(unsigned) * (size_t)v.n1 * v.n2 * v.n3);
   ALLOC(g->sc, sizeof(StepScalars));
 #undef ALLOC

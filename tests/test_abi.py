@@ -55,7 +55,7 @@ def test_no_cpu_fallback_and_no_oracle_in_product():
 
 def test_params_struct_layout_matches_header():
     import paper_2408_01361_b200 as m
-    # 1 int + pad, 5 doubles, 3 ints + pad, 6 doubles, 6 ints, 2 doubles, int + pad, 8 doubles, 4 ints
-    assert ctypes.sizeof(m.Params) == 8 + 5 * 8 + 16 + 6 * 8 + 24 + 16 + 8 + 8 * 8 + 16
+    # 1 int + pad, 5 doubles, 3 ints + pad, 6 doubles, 6 ints, 2 doubles, int + pad, 8 doubles, 5 ints + pad
+    assert ctypes.sizeof(m.Params) == 8 + 5 * 8 + 16 + 6 * 8 + 24 + 16 + 8 + 8 * 8 + 24
     p = m.make_params(ki.config_params(3))
     assert (p.n1, p.n2, p.n3) == (192, 128, 128) and p.recon == 1 and abs(p.a - 0.9375) < 1e-15

@@ -501,3 +501,41 @@ def test_face_centred_ct_parity(kh, kho, case):
         sc = max(np.abs(fo[d][I]).max(), 1e-300)
         assert np.abs(fg[d][I] - fo[d][I]).max() <= 1e-9 * max(sc, np.abs(fo[0][I]).max()), d
     assert gg.divB_face() <= 1e-11 * max(np.abs(fo[0]).max(), np.abs(fo[1]).max()) * max(p["n1"], p["n2"]) + 4 * d0
+
+
+@pytest.mark.parametrize("case", ["flux_ct_torus", "face_ct_minkowski", "face_ct_torus_stress"])
+def test_upwinded_emf_parity(kh, kho, case):
+    """kh_params.emf = KH_EMF_UPWIND on both sides ("with and without upwinding"), with either
+    transport: stage EMFs, one step, a 10-step run."""
+    from kharm_inputs import facefield
+    faces = None
+    if case == "flux_ct_torus":
+        p = ki.config_params(3, n=(48, 32, 8)); P0 = torus.torus_state(p, seed=2)
+    elif case == "face_ct_minkowski":
+        p = dict(ki.config_params(5, n=(24, 18, 10), recon=kp.RECON_WENO5), transport=kp.B_FACE_CT)
+        P0 = modes.config5(p, seed=2, amp=5e-2)
+        faces = facefield.face_from_potential(p, *facefield.periodic_potential(p, seed=3, amp=5e-2))
+    else:
+        p = dict(ki.config_params(4, n=(48, 32, 8)), transport=kp.B_FACE_CT)
+        P0 = torus.torus_state(p, mad=True, seed=3, stress=True, stress_fraction=0.02)
+        faces = facefield.face_from_potential(p, *facefield.axisymmetric_loop_potential(p, amp=2e-3, x1c=2.3))
+    p = dict(p, emf=kp.EMF_UPWIND)
+    gg, go = kh.Grid(p), kho.Grid(p, omp=True)
+    for g in (gg, go):
+        g.set_prims(P0)
+        if faces is not None:
+            g.set_face_B(*faces)
+    dt = go.estimate_dt()
+    n_g, n_o = gg.step(dt), go.step(dt)
+    assert abs(n_g / n_o - 1) < 1e-11
+    _assert_step_parity(p, gg.get_prims(), go.get_prims(), gg.get_flags()[0], go.get_flags()[0], "upwind emf " + case)
+    I = (slice(3, -3), slice(3, -3), slice(3, -3))
+    for d in (1, 2, 3):
+        eg, eo = gg.get_emf(d), go.get_emf(d)
+        assert np.abs(eg[I] - eo[I]).max() <= 1e-11 * (max(np.abs(go.get_emf(c)[I]).max() for c in (1, 2, 3)) + 1e-300), d
+    for _ in range(9):
+        n_g, n_o = gg.step(n_g), go.step(n_o)
+    l1 = l1_diff(p, gg.get_prims(), go.get_prims())
+    assert l1.max() <= TOL_RUN_L1, l1
+    if faces is not None:
+        assert gg.divB_face() <= 4 * go.divB_face() + 1e-13
