@@ -466,7 +466,7 @@ def _face_pair(kh, kho, p, P0, faces):
     return p, gg, go
 
 
-@pytest.mark.parametrize("case", ["minkowski_weno5", "torus_mc", "torus_weno5_kastaun_fofc"])
+@pytest.mark.parametrize("case", ["minkowski_weno5", "torus_mc", "torus_weno5_kastaun_fofc", "two_d_upwind"])
 def test_face_centred_ct_parity(kh, kho, case):
     """kh_params.transport = KH_B_FACE_CT on both sides: the face field agrees to round-off, its
     divergence stays at round-off on both sides, the primitives meet the one-step and run bars."""
@@ -475,6 +475,10 @@ def test_face_centred_ct_parity(kh, kho, case):
         p = ki.config_params(5, n=(24, 18, 10), recon=kp.RECON_WENO5)
         P0 = modes.config5(p, seed=2, amp=1e-2)
         faces = facefield.face_from_potential(p, *facefield.periodic_potential(p, seed=3, amp=5e-2))
+    elif case == "two_d_upwind":          # n3 = 1 (S21) with the face field, upwinded EMFs and drift-frame floors
+        p = dict(ki.config_params(3, n=(64, 48, 1)), emf=kp.EMF_UPWIND, floor_frame=kp.FRAME_DRIFT)
+        P0 = torus.torus_state(p, seed=2)
+        faces = facefield.face_from_potential(p, *facefield.axisymmetric_loop_potential(p, amp=2e-3, x1c=2.3))
     else:
         p = ki.config_params(3, n=(48, 32, 8), recon=kp.RECON_MC if case == "torus_mc" else kp.RECON_WENO5)
         if case != "torus_mc":
