@@ -277,6 +277,36 @@ def test_full_size_config3_one_step_sampled(kh, kho):
     assert gg.divB() < 1e-10
 
 
+def test_full_size_config4_one_step(kh, kho):
+    """BASELINE config 4 at its full 288 x 128 x 128 size (MAD field, MC), all interior zones."""
+    p = ki.config_params(4)
+    P0 = torus.torus_state(p, mad=True, seed=1)
+    gg, go = _both(kh, kho, p, P0)
+    dt = go.estimate_dt()
+    n_g, n_o = gg.step(dt), go.step(dt)
+    assert abs(n_g / n_o - 1) < 1e-11
+    _assert_step_parity(p, gg.get_prims(), go.get_prims(), gg.get_flags()[0], go.get_flags()[0], "cfg4 full")
+    assert gg.divB() < 1e-10
+
+
+def test_full_size_config3_with_every_extension(kh, kho):
+    """The 192 x 128 x 128 block with the SURVEY 8(f) extensions switched on together: Kastaun inverter, first-order flux
+    correction, drift-frame floors, face-centred CT with upwinded EMFs.  One step, all interior zones."""
+    from kharm_inputs import facefield
+    p = dict(ki.config_params(3), inverter=kp.INV_KASTAUN, fofc=1, floor_frame=kp.FRAME_DRIFT, transport=kp.B_FACE_CT, emf=kp.EMF_UPWIND)
+    P0 = torus.torus_state(p, seed=1)
+    faces = facefield.face_from_potential(p, *facefield.axisymmetric_loop_potential(p, amp=2e-3, x1c=2.5))
+    gg, go = kh.Grid(p), kho.Grid(p, omp=True)
+    for g in (gg, go):
+        g.set_prims(P0)
+        g.set_face_B(*faces)
+    dt = go.estimate_dt()
+    n_g, n_o = gg.step(dt), go.step(dt)
+    assert abs(n_g / n_o - 1) < 1e-11
+    _assert_step_parity(p, gg.get_prims(), go.get_prims(), gg.get_flags()[0], go.get_flags()[0], "cfg3 full, all extensions")
+    assert gg.divB_face() <= 4 * go.divB_face() + 1e-14
+
+
 # ------------------------------------------------------------------------------------------ second inverter (NEXT-2)
 @pytest.mark.parametrize("case", ["torus_weno5", "mad_mc", "minkowski", "bondi"])
 def test_one_step_kastaun_inverter(kh, kho, case):
