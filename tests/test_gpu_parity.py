@@ -277,6 +277,20 @@ def test_full_size_config3_one_step_sampled(kh, kho):
     assert gg.divB() < 1e-10
 
 
+@pytest.mark.parametrize("n,recon", [(64, kp.RECON_MC), (128, kp.RECON_WENO5), (192, kp.RECON_MC)])
+def test_config5_sweep_sizes_one_step(kh, kho, n, recon):
+    """BASELINE config 5 (Minkowski throughput sweep) at its own sizes up to 192^3, all interior zones (256^3 and 320^3 are
+    timed by bench.py; their oracle runs need 8-17 GB of host memory and are left out of the test suite)."""
+    p = ki.config_params(5, n=n, recon=recon)
+    P0 = modes.config5(p, seed=1, amp=1e-3)
+    gg, go = _both(kh, kho, p, P0)
+    dt = go.estimate_dt()
+    n_g, n_o = gg.step(dt), go.step(dt)
+    assert abs(n_g / n_o - 1) < 1e-11
+    _assert_step_parity(p, gg.get_prims(), go.get_prims(), gg.get_flags()[0], go.get_flags()[0], "cfg5 %d^3" % n)
+    assert gg.divB() < 1e-10
+
+
 def test_full_size_config4_one_step(kh, kho):
     """BASELINE config 4 at its full 288 x 128 x 128 size (MAD field, MC), all interior zones."""
     p = ki.config_params(4)
