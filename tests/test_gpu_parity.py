@@ -587,3 +587,28 @@ def test_upwinded_emf_parity(kh, kho, case):
     assert l1.max() <= TOL_RUN_L1, l1
     if faces is not None:
         assert gg.divB_face() <= 4 * go.divB_face() + 1e-13
+
+
+# ------------------------------------------------------------------------------------------ the paper's own acceptance tests, on the CUDA path
+@pytest.mark.parametrize("rotated,recon", [(False, kp.RECON_MC), (True, kp.RECON_MC), (True, kp.RECON_WENO5)])
+def test_cuda_path_linear_mode_convergence(kh, rotated, recon):
+    """the L1 error of a linear mode after one period falls at second order with resolution.  Full 16^3, 32^3,
+    64^3 cubes of config 1 through the C ABI alone (no oracle); same windows as the oracle's own pin."""
+    errs = []
+    for n in (16, 32, 64):
+        p = ki.config_params(1, n=n, recon=recon)
+        P0, T = modes.config1(p, rotated=rotated)
+        g = kh.Grid(p)
+        g.set_prims(P0)
+        dt, t = g.estimate_dt(), 0.0
+        while t < T * (1 - 1e-12):
+            dt = min(dt, T - t)
+            t += dt
+            dt = g.step(dt)
+        assert g.divB() < 1e-12 and g.count_flags()[0] == 0
+        errs.append(np.abs(g.get_prims() - P0).mean(axis=(1, 2, 3)))
+    _, r = modes.eigenmode([1, 1, 0] / np.sqrt(2) if rotated else [1, 0, 0], modes.FAST)
+    act = np.abs(r) > 0.05
+    total = [e[act].sum() for e in errs]
+    assert -2.9 < np.log2(total[1] / total[0]) < -1.3, total
+    assert -2.5 < np.log2(total[2] / total[1]) < -1.75, total
