@@ -496,8 +496,9 @@ int u2p(const Geom& G, const double U[NP], const double Pg[NP], double gam, doub
 //   nuB = (1 + ahat)(1 + qbar - mu rbar^2),  f(mu) = mu - 1/(max(nuA, nuB) + rbar^2 mu);
 // bracket (0, mu+], mu+ = 1/h0 if r < h0, else the root of fa(mu) = mu sqrt(h0^2 + rbar^2(mu)) - 1 in (0, 1/h0];
 // velocity v^i = mu x (r^i + mu (r.b) b^i), ut^i = What v^i.
-// Root finder (the paper uses a library bracketing method; S24): Illinois regula falsi on the bracket, stop when the
-// bracket is narrower than 4e-16 of its upper end or f vanishes, at most 100 evaluations (flag 2 otherwise).
+// Root finder (the paper uses a library bracketing method; S24): Illinois regula falsi on the bracket for 40 evaluations,
+// plain bisection after that; stop when the bracket is narrower than 4e-16 of its upper end, cannot be split any more or
+// f vanishes; at most 100 evaluations (flag 2 otherwise: reached only through NaN).
 // Flags as for u2p: 1 bad input, 2 not converged, 3 speed limit v0 acted at the root, 5 eps < 0 at the root (the
 // hydro primitives keep the guess), 7 non-finite result.
 // ---------------------------------------------------------------------------------------------
@@ -535,8 +536,9 @@ bool illinois(Fn fn, double a, double fa, double b, double fb, double& lo, doubl
   int side = 0;
   for (int it = 0; it < 100; it++) {
     if (!(b - a > 4e-16 * b)) { lo = a; hi = b; return true; }
-    double m = b - fb * (b - a) / (fb - fa);
+    double m = (it < 40) ? b - fb * (b - a) / (fb - fa) : 0.5 * (a + b);    // after 40 evaluations: plain bisection
     if (!(m > a && m < b)) m = 0.5 * (a + b);
+    if (!(m > a && m < b)) { lo = a; hi = b; return true; }                 // a and b are neighbouring numbers
     double fm = fn(m);
     if (fm == 0.0) { lo = hi = m; return true; }
     if (fm > 0.0) { b = m; fb = fm; if (side == 1) fa *= 0.5; side = 1; }
@@ -626,8 +628,8 @@ int u2p_kastaun(const Geom& G, const double U[NP], const double Pg[NP], double g
 //   * the momentum along the field, S_i B^i/|B| = w gamma^2 v_par (w = rho + Gamma u), is conserved:
 //       A = w gamma^2 v_par / w',   v_par' / (1 - v_perp^2 - v_par'^2) = A
 //       =>  v_par' = 2 A (1 - v_perp^2) / (1 + sqrt(1 + 4 A^2 (1 - v_perp^2))).
-// (b^2 = B^2 (1 - v_perp^2) is then unchanged too, so the magnetisation limits stay consistent.)  B = 0: no direction,
-// the velocity is kept.  The Lorentz-factor ceiling acts on the adjusted velocity.
+// (b^2 = B^2 (1 - v_perp^2) is then unchanged too, so the magnetisation limits stay consistent.)  B^2 <= 1e-12 w': no
+// direction, the velocity is kept.  The Lorentz-factor ceiling acts on the adjusted velocity.
 // ---------------------------------------------------------------------------------------------
 void drift_frame_velocity(const Geom& G, double gam, double rho_old, double u_old, double rho_new, double u_new, double P[NP]) {
   double Bcov[4] = {0, 0, 0, 0}, qsq = 0.0, Bsq = 0.0, uB = 0.0;
@@ -636,7 +638,9 @@ void drift_frame_velocity(const Geom& G, double gam, double rho_old, double u_ol
     Bcov[i] += G.gcov[i][j] * P[B1 + j - 1];
   }
   for (int i = 1; i < 4; i++) { Bsq += Bcov[i] * P[B1 + i - 1]; uB += Bcov[i] * P[U1 + i - 1]; }
-  if (!(Bsq > 0.0)) return;
+  // no field direction to speak of: B^2 below 1e-12 of the enthalpy (a magnetisation double precision cannot see in T^mu_nu;
+  // such fields are often pure round-off, whose direction is noise) keeps the velocity
+  if (!(Bsq > 1e-12 * (rho_new + gam * u_new))) return;
   double gamma = std::sqrt(1.0 + qsq), B = std::sqrt(Bsq);
   double vpar = uB / (gamma * B);                          // v^i B_i / |B|
   double vsq = qsq / (gamma * gamma);

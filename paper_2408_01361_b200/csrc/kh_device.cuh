@@ -364,7 +364,7 @@ __device__ __forceinline__ void drift_frame_velocity(const Geo& G, double gam, d
   double l1, l2, l3;
   lower3<FLAT>(G, b1, b2, b3, l1, l2, l3);                               // B_i
   const double Bsq = fma(b3, l3, fma(b2, l2, b1 * l1));
-  if (!(Bsq > 0.0)) return;
+  if (!(Bsq > 1e-12 * fma(gam, u_new, rho_new))) return;               // no field direction to speak of (S26): velocity kept
   const double uB = fma(ut3, l3, fma(ut2, l2, ut1 * l1));                // ut^i B_i
   const double qsq = spatial_norm2<FLAT>(G, ut1, ut2, ut3);
   const double gsq = 1.0 + qsq, gamma = sqrt(gsq), iB = 1.0 / sqrt(Bsq), ig = 1.0 / gamma;
@@ -534,7 +534,8 @@ __device__ __forceinline__ int u_to_p_floors(const Geo& G, const double Uh[KH_NP
 //   x = 1/(1 + mu b^2),  rbar^2 = x (r^2 x + mu (1 + x)(r.b)^2),  qbar = q - b^2/2 - mu^2 x^2 (b^2 r^2 - (r.b)^2)/2,
 //   f(mu) = mu - 1/(nu + rbar^2 mu),  nu = max((1 + Gamma eps)/W, (1 + a)(1 + qbar - mu rbar^2)),  a = (Gamma-1) eps/(1+eps),
 //   v^2 = min(mu^2 rbar^2, v0^2), W = (1 - v^2)^(-1/2), eps = W (qbar - mu rbar^2) + v^2 W^2/(1 + W) (clamped at 0 in f),
-// bracket (0, mu+], mu+ = 1 or the root of mu sqrt(1 + rbar^2) - 1; Illinois regula falsi to a bracket of 4e-16.
+// bracket (0, mu+], mu+ = 1 or the root of mu sqrt(1 + rbar^2) - 1; Illinois regula falsi (bisection after 40 evaluations) to a
+// bracket of 4e-16.
 // ---------------------------------------------------------------------------------------------
 struct KastaunC {
   double q, rsq, bsq, rbsq, brperp, v0sq, gam;
@@ -574,8 +575,9 @@ __device__ __forceinline__ bool kastaun_root(const KastaunC& c, double a, double
 #pragma unroll 1
   for (int it = 0; it < 100; it++) {
     if (!(b - a > 4e-16 * b)) { lo = a; hi = b; return true; }
-    double m = fma(-fb, (b - a) / (fb - fa), b);
+    double m = (it < 40) ? fma(-fb, (b - a) / (fb - fa), b) : 0.5 * (a + b);   // after 40 evaluations: plain bisection
     if (!(m > a && m < b)) m = 0.5 * (a + b);
+    if (!(m > a && m < b)) { lo = a; hi = b; return true; }                    // a and b are neighbouring numbers
     double t0, t1, t2, t3;
     const double fm = AUX ? kastaun_fa(c, m) : kastaun_f(c, m, t0, t1, t2, t3);
     if (fm == 0.0) { lo = hi = m; return true; }
