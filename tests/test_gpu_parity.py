@@ -686,3 +686,41 @@ def test_fuzz_one_step_random_configurations(kh, kho, seed):
     _assert_step_parity(p, gg.get_prims(), go.get_prims(), pf_g, pf_o, label, tol=tol)
     if opts["floor_frame"] != kp.FRAME_NORMAL:      # (after a normal-frame injection rho sits AT its floor: the second-pass bit is a coin flip)
         assert (ff_g != ff_o).sum() <= max(2, (1e-2 if opts["fofc"] else 5e-3) * ff_o.size), label    # marginal floor decisions may flip
+
+
+@pytest.mark.parametrize("seed", list(range(8)))
+def test_fuzz_graph_replay_matches_direct_launches_for_every_option_mix(kh, seed):
+    """CUDA-graph replay with the device-resident dt, direct launches and profiled launches give bitwise the same state
+    for random mixes of the options (the graph then holds the FOFC memset / mask nodes, the face-field kernels, ...)."""
+    from kharm_inputs import facefield
+    rng = np.random.default_rng(77 + seed)
+    p = ki.config_params(3, n=(int(rng.integers(12, 40)), int(rng.integers(8, 24)), int(rng.integers(1, 8))))
+    opts = dict(recon=int(rng.integers(0, 2)), inverter=int(rng.integers(0, 2)), floor_frame=int(rng.integers(0, 3)),
+                fofc=int(rng.integers(0, 2)), transport=int(rng.integers(0, 2)), emf=int(rng.integers(0, 2)))
+    p = dict(p, **opts)
+    P0 = torus.torus_state(p, mad=bool(seed % 2), seed=seed, stress=True, stress_fraction=0.02)
+    faces = facefield.face_from_potential(p, *facefield.axisymmetric_loop_potential(p, amp=1e-3, x1c=2.5)) if opts["transport"] else None
+    outs = []
+    for mode in ("graph_device_dt", "direct", "profiled"):
+        g = kh.Grid(p)
+        g.set_prims(P0)
+        if faces is not None:
+            g.set_face_B(*faces)
+        dt = g.estimate_dt()
+        if mode == "graph_device_dt":
+            g.step(dt, sync=False)
+            for _ in range(3):
+                g.step(-1.0, sync=False)
+        else:
+            if mode == "direct":
+                g.set_graph(False)
+            else:
+                g.set_profile(True)
+            for _ in range(4):
+                dt = g.step(dt)
+        outs.append((g.get_prims(), g.get_flags(), g.get_face_B() if faces is not None else None))
+    for o in outs[1:]:
+        assert np.array_equal(outs[0][0], o[0]), opts
+        assert np.array_equal(outs[0][1][0], o[1][0]) and np.array_equal(outs[0][1][1], o[1][1]), opts
+        if faces is not None:
+            assert all(np.array_equal(a, b) for a, b in zip(outs[0][2], o[2])), opts
