@@ -179,3 +179,26 @@ def test_upwinded_emf_keeps_second_order_convergence_of_a_rotated_mode(kho):
         errs.append(np.abs(g.get_prims() - P0).mean(axis=(1, 2, 3)).max())
     slope = np.log2(errs[0] / errs[1])
     assert 1.7 < slope < 2.4, (errs, slope)
+
+
+def test_face_ct_equals_flux_ct_for_any_emf_and_option_mix(kho):
+    """The zone-centred mean of the face field obeys the Flux-CT update for ANY edge EMFs (the identity is algebra on the
+    EMF arrays), so the two transports must agree to round-off whatever the EMF kind, inverter, floor frame or FOFC."""
+    rng = np.random.default_rng(9)
+    for trial in range(6):
+        n = (int(rng.integers(8, 20)), int(rng.integers(6, 14)), int(rng.integers(1, 6)))
+        opts = dict(recon=int(rng.integers(0, 2)), inverter=int(rng.integers(0, 2)), floor_frame=int(rng.integers(0, 3)),
+                    fofc=int(rng.integers(0, 2)), emf=int(rng.integers(0, 2)))
+        p = dict(ki.config_params(3, n=n), **opts)
+        P0 = torus.torus_state(p, seed=trial)
+        faces = facefield.face_from_potential(p, *facefield.axisymmetric_loop_potential(p, amp=2e-3, x1c=2.3))
+        g_flux, g_face = _grids(kho, p, P0, faces)
+        dt = g_flux.estimate_dt()
+        for _ in range(2):
+            d1, d2 = g_flux.step(dt), g_face.step(dt)
+            dt = d1
+        a, b = g_flux.get_prims(), g_face.get_prims()
+        assert np.array_equal(g_flux.get_flags()[0], g_face.get_flags()[0]), opts
+        for v in range(8):
+            assert np.abs(a[v] - b[v]).max() <= 1e-10 * max(np.abs(a[v]).max(), 1e-12), (opts, v)
+        assert g_face.divB_face() < 1e-13
