@@ -353,7 +353,8 @@ emf_upwind_kernel(GV g, const double* __restrict__ F1, const double* __restrict_
 // ~50 fp64 instructions instead of the 40-entry Gamma table and a 64-term contraction.
 // One thread per interior zone, flattened index (no idle lanes when n1 is not a multiple of the block).
 // ---------------------------------------------------------------------------------------------
-// MODE = inverter (bit 0: 0 1D_W, 1 Kastaun) + 2 * floor frame (0 fluid, 1 drift, 2 normal observer)
+// MODE = inverter (bit 0: 0 1D_W, 1 Kastaun) + 2 * floor frame (0 fluid, 1 drift, 2 normal observer) + 8 if the zone-centred
+// field comes from the face field (face-centred CT)
 template <bool FLAT, bool CORR, int MODE>
 __global__ void __launch_bounds__(128, KH_MINB_UPDATE)
 update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps, double* __restrict__ Pf,
@@ -361,7 +362,8 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
               const double* __restrict__ e1, const double* __restrict__ e2, const double* __restrict__ e3,
               const double* __restrict__ ct1, const double* __restrict__ ct2, const double* __restrict__ ct3,
               unsigned char* __restrict__ pflag, unsigned char* __restrict__ fflag, unsigned* __restrict__ faillist,
-              StepScalars* __restrict__ sc, double dt_factor) {
+              StepScalars* __restrict__ sc, double dt_factor, const double* __restrict__ Bface1, const double* __restrict__ Bface2,
+              const double* __restrict__ Bface3) {
   const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
   const long nzone = (long)g.n1 * g.n2 * g.n3;
   const bool active = t < nzone;
@@ -441,7 +443,12 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
       Uh[v] = fma(dtg, src - div, Uh[v]);
     }
     // induction: Flux-CT fluxes from the edge EMFs (S15a); the factors 1/2 are applied once per component
-    {
+    if (MODE & 8) {   // face-centred CT (S28): the zone's conserved field is the mean of its two (already advanced) face values
+      const double hs = FLAT ? 0.5 : 0.5 * fast_rcp(G.gdet);
+      Uh[B1] = hs * (Bface1[n] + Bface1[n + 1]);
+      Uh[B2] = hs * (Bface2[n] + Bface2[n + g.s2]);
+      Uh[B3] = hs * (Bface3[n] + Bface3[n + g.s3]);
+    } else {
       const long s2 = g.s2, s3 = g.s3;
       const double a00 = e3[n], a10 = e3[n + 1], a01 = e3[n + s2], a11 = e3[n + s2 + 1];          // emf3 at (i,j) corners
       const double b00 = e2[n], b10 = e2[n + 1], b01 = e2[n + s3], b11 = e2[n + s3 + 1];          // emf2 at (i,k) corners
@@ -458,7 +465,7 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
     {
       const double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2);
       const double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
-      pf_flag = invert_with_floors<FLAT, MODE & 1>(G, Uh, W0, g.gam, g.fp, MODE >> 1, rho_g, u_g, pf, ff);
+      pf_flag = invert_with_floors<FLAT, MODE & 1>(G, Uh, W0, g.gam, g.fp, (MODE & 7) >> 1, rho_g, u_g, pf, ff);
     }
     if (pf_flag != 0) {          // rare: the hydro primitives keep the guess (S16); queue the zone for the fix-up
 #pragma unroll

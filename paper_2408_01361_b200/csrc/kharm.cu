@@ -203,16 +203,31 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
     }
     prof_end(g);
     g->launches++;
+    const double *fb1 = nullptr, *fb2 = nullptr, *fb3 = nullptr;
+    if (Bfi && pass + 1 == passes) {
+      // face-centred CT: advance the face field by the EMF circulation; the update then takes the zone's field from it
+      prof_begin(g, KH_K_EMF);
+      face_ct_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, Bfi[0], Bfi[1], Bfi[2], Bff[0], Bff[1], Bff[2], g->emf[0],
+                                                                                       g->emf[1], g->emf[2], g->sc, dt_factor);
+      prof_end(g);
+      g->launches++;
+      CK(cudaGetLastError());
+      fb1 = Bff[0]; fb2 = Bff[1]; fb3 = Bff[2];
+    }
     const unsigned grid = (unsigned)(((long)v.n1 * v.n2 * v.n3 + 127) / 128);
 #define UPD(FL, CO, IN)                                                                                                  \
   update_kernel<FL, CO, IN><<<grid, 128, 0, g->stream>>>(v, Pi, Ps, Pf, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], \
-                                                         g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, g->fflag, g->faillist, g->sc, dt_factor)
+                                                         g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, g->fflag, g->faillist, g->sc, dt_factor, \
+                                                         fb1, fb2, fb3)
     prof_begin(g, KH_K_UPDATE);
 #define UPD2(FL, CO)                                                                 \
-    switch (g->p.inverter + 2 * g->p.floor_frame) {                                  \
+    switch (g->p.inverter + 2 * g->p.floor_frame + (fb1 ? 8 : 0)) {                  \
       case 0: UPD(FL, CO, 0); break; case 1: UPD(FL, CO, 1); break;                  \
       case 2: UPD(FL, CO, 2); break; case 3: UPD(FL, CO, 3); break;                  \
-      case 4: UPD(FL, CO, 4); break; default: UPD(FL, CO, 5); break;                 \
+      case 4: UPD(FL, CO, 4); break; case 5: UPD(FL, CO, 5); break;                  \
+      case 8: UPD(FL, CO, 8); break; case 9: UPD(FL, CO, 9); break;                  \
+      case 10: UPD(FL, CO, 10); break; case 11: UPD(FL, CO, 11); break;              \
+      case 12: UPD(FL, CO, 12); break; default: UPD(FL, CO, 13); break;              \
     }
     if (g->flat) { if (corrector) { UPD2(true, true) } else { UPD2(true, false) } }
     else { if (corrector) { UPD2(false, true) } else { UPD2(false, false) } }
@@ -221,17 +236,6 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
 #undef UPD
     g->launches++;
     CK(cudaGetLastError());
-    if (Bfi && pass + 1 == passes) {
-      // face-centred CT: advance the face field by the EMF circulation and slave the zone-centred field to it (the
-      // update kernel's own induction update equals the face mean to round-off for the arithmetic EMF: Toth 2000)
-      prof_begin(g, KH_K_EMF);
-      face_ct_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, Bfi[0], Bfi[1], Bfi[2], Bff[0], Bff[1], Bff[2], g->emf[0],
-                                                                                       g->emf[1], g->emf[2], g->sc, dt_factor);
-      face_to_cent_kernel<<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, Bff[0], Bff[1], Bff[2], Pf, g->flat ? 1 : 0);
-      prof_end(g);
-      g->launches += 2;
-      CK(cudaGetLastError());
-    }
     if (pass + 1 < passes) {
       // troubled zones of the speculative update -> mask (+ ghost images) -> donor-cell LLF on their faces
       prof_begin(g, KH_K_FOFC);

@@ -680,9 +680,7 @@ def test_fuzz_one_step_random_configurations(kh, kho, seed):
     pf_g, ff_g = gg.get_flags()
     pf_o, ff_o = go.get_flags()
     # two steps double the bar; the normal-frame floors invert twice per zone, which squares the conditioning of u
-    # (and under face-centred CT the kernel inverts with the Flux-CT form of the zone-centred field, which equals the face
-    # mean only to round-off: S28)
-    tol = TOL_ONE_STEP * (2 if seed % 2 else 1) * (4 if (opts["floor_frame"] == kp.FRAME_NORMAL or opts["transport"] == kp.B_FACE_CT) else 1)
+    tol = TOL_ONE_STEP * (2 if seed % 2 else 1) * (4 if opts["floor_frame"] == kp.FRAME_NORMAL else 1)
     _assert_step_parity(p, gg.get_prims(), go.get_prims(), pf_g, pf_o, label, tol=tol)
     if opts["floor_frame"] != kp.FRAME_NORMAL:      # (after a normal-frame injection rho sits AT its floor: the second-pass bit is a coin flip)
         assert (ff_g != ff_o).sum() <= max(2, (1e-2 if opts["fofc"] else 5e-3) * ff_o.size), label    # marginal floor decisions may flip
