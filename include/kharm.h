@@ -127,7 +127,8 @@ int kh_get_flux(kh_grid* g, int dir, double* F, double* ctop, int mem);
 /* Face-centred CT (kh_params.transport = KH_B_FACE_CT).  Phi^d = sqrt(-g) B^d on the lower d-face of each zone, three
  * arrays with ghosts [nt] (faces i_d in [0, N_d] with interior transverse indices are used, the rest ignored).
  * kh_set_face_B also sets the zone-centred field of the current state to the mean of each zone's two face values over
- * sqrt(-g) and fills its ghosts: call it AFTER kh_set_prims.  kh_divB_face: max over interior zones of
+ * sqrt(-g) and fills its ghosts: call it AFTER kh_set_prims; kh_step returns KH_EINVAL on a face-CT grid until it has been
+ * called.  kh_divB_face: max over interior zones of
  * |sum_d (Phi^d(upper) - Phi^d(lower))/dx_d|, which the transport keeps at its initial value to round-off. */
 int kh_set_face_B(kh_grid* g, const double* f1, const double* f2, const double* f3, int mem);
 int kh_get_face_B(kh_grid* g, double* f1, double* f2, double* f3, int mem);

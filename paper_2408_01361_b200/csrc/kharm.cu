@@ -40,6 +40,7 @@ struct kh_grid {
   double* emf[3];
   unsigned char *pflag, *fflag;
   double* ecent[4];      // upwinded EMFs: zone-centred reference values + conserved density (allocated on demand)
+  bool faces_set;        // face-centred CT: kh_set_face_B has been called
   double* Bf[3][3];      // face-centred CT: Phi^d per rotation state [state][d], [ntot] each (allocated on demand)
   unsigned char* mask;   // FOFC: troubled zones of the speculative update (with ghost images)
   unsigned* faillist;    // zones (device-layout index) whose inversion failed in the current sub-step
@@ -534,6 +535,8 @@ int kh_estimate_dt(kh_grid* g, double* dt) {
 }
 
 int kh_step(kh_grid* g, double dt, double* dt_next) {
+  if (g && g->p.transport == KH_B_FACE_CT && !g->faces_set) return KH_EINVAL;   // the face field is the magnetic state: set it first
+
   if (!g || dt != dt) return KH_EINVAL;
   set_dt_kernel<<<1, 1, 0, g->stream>>>(g->sc, dt, dt > 0.0 ? 0 : 1);
   g->launches++;
@@ -602,6 +605,7 @@ int kh_set_face_B(kh_grid* g, const double* f1, const double* f2, const double* 
   int rc = fill_ghosts(g, g->P[g->cur], nullptr);
   if (rc) return rc;
   CK(cudaStreamSynchronize(g->stream));
+  g->faces_set = true;
   return KH_OK;
 }
 
@@ -702,6 +706,7 @@ int kh_get_emf(kh_grid* g, int dir, double* emf, int mem) {
 
 int kh_debug_predictor(kh_grid* g, double dt) {
   if (!g || !(dt > 0.0)) return KH_EINVAL;
+  if (g->p.transport == KH_B_FACE_CT && !g->faces_set) return KH_EINVAL;
   set_dt_kernel<<<1, 1, 0, g->stream>>>(g->sc, dt, 0);
   g->launches++;
   const bool face = g->p.transport == KH_B_FACE_CT;

@@ -256,6 +256,13 @@ def test_torch_device_buffers(kh):
     with pytest.raises(kh.KharmError):
         bad = dict(p); bad["n1"] = 0
         kh.Grid(bad)
+    # a face-centred CT grid refuses to step before its magnetic state (the face field) is set
+    gf = kh.Grid(dict(p, transport=kp.B_FACE_CT))
+    gf.set_prims(P0)
+    with pytest.raises(kh.KharmError):
+        gf.step(1e-3)
+    with pytest.raises(kh.KharmError):          # and the face calls are refused on a Flux-CT grid
+        g.divB_face()
 
 
 # ------------------------------------------------------------------------------------------ full size, bench configuration
