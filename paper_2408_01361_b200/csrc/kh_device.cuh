@@ -293,7 +293,7 @@ __device__ __forceinline__ void mc_zone(double x2, double x3, double x4, double&
 //   weights d_k / (beta_k + eps)^2 over the common denominator: (1, 6, 3) x products of the other two squares
 //   candidate values as offsets from x3, times 6:  upper face (5 D2 - 2 D1, D2 + 2 D3, 4 D3 - D4),
 //   lower face the mirror image (2 D4 - 5 D3, -(D3 + 2 D2), D1 - 4 D2); the smoothness indicators are shared.
-// 56 fp64 instructions per variable for both faces.
+// 54 fp64 instructions per variable for both faces.
 __device__ __forceinline__ void weno5_zone(double x1, double x2, double x3, double x4, double x5, double& qm, double& qp) {
   const double c = 4.0e-26, k13 = 13.0 / 3.0;
   double D1 = x2 - x1, D2 = x3 - x2, D3 = x4 - x3, D4 = x5 - x4;
@@ -306,14 +306,14 @@ __device__ __forceinline__ void weno5_zone(double x1, double x2, double x3, doub
   double p23 = a2 * a3, p13 = 6.0 * (a1 * a3), p12 = a1 * a2;
   {
     double w3 = 3.0 * p12;
-    double V1 = fma(5.0, D2, -2.0 * D1), V2 = fma(2.0, D3, D2), V3 = fma(4.0, D3, -D4);
+    double V1 = fma(2.0, e1, -D2), V2 = fma(2.0, D3, D2), V3 = fma(4.0, D3, -D4);      // 5 D2 - 2 D1 = 2 e1 - D2
     double N = fma(w3, V3, fma(p13, V2, p23 * V1));
     double S = p23 + p13 + w3;
     qp = fma(N * fast_rcp(S), 1.0 / 6.0, x3);
   }
   {
     double m3 = 3.0 * p23;
-    double M1 = fma(-5.0, D3, 2.0 * D4), M2 = fma(2.0, D2, D3), M3 = fma(-4.0, D2, D1);
+    double M1 = fma(2.0, e3, D3), M2 = fma(2.0, D2, D3), M3 = fma(-4.0, D2, D1);        // 2 D4 - 5 D3 = 2 e3 + D3
     double N = fma(m3, M3, fma(-p13, M2, p12 * M1));
     double S = p12 + p13 + m3;
     qm = fma(N * fast_rcp(S), 1.0 / 6.0, x3);
