@@ -126,7 +126,7 @@ class ClockSampler:
             fd, self.path = tempfile.mkstemp(prefix="kh_clocks_", suffix=".csv")
             os.close(fd)
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
         except OSError:
             self.proc = None
@@ -172,28 +172,75 @@ def oracle_sample_params(p):
     return q
 
 
-def time_oracle(name, steps, warmup, seed=1):
-    """Zone-cycles/s of the oracle (OpenMP build of the same source, bit-identical to the single-thread one)."""
+def time_oracle(name, steps, warmup, seed=1, omp=True, full=False, budget_s=None):
+    """Zone-cycles/s of the oracle as it stands: omp=True the OpenMP build of the same source (bit-identical to the
+    single-thread one; tested), omp=False the single-thread library.  full=False cuts the block to 32 zones in x3.
+    budget_s: stop after the first step that ends beyond this many seconds (at least one step is timed)."""
     from oracle import kho
     _, p = workload_params(name)
-    q = oracle_sample_params(p)
+    q = dict(p) if full else oracle_sample_params(p)
     cfg = WORKLOADS[name][0]
     from kharm_inputs import modes, torus
     P0 = torus.torus_state(q, mad=(cfg == 4), seed=seed) if cfg in (3, 4) else modes.config5(q, seed=seed, amp=1e-3)
-    g = kho.Grid(q, omp=True)
+    g = kho.Grid(q, omp=omp)
     g.set_prims(P0)
     dt = g.estimate_dt()
     for _ in range(warmup):
         dt = g.step(dt)
     t0 = time.perf_counter()
+    done = 0
     for _ in range(steps):
         dt = g.step(dt)
+        done += 1
+        if budget_s is not None and time.perf_counter() - t0 > budget_s:
+            break
     el = time.perf_counter() - t0
     zones = q["n1"] * q["n2"] * q["n3"]
-    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
-    return dict(value=zones * steps / el, unit="zone-cycles/s", cores=cores, kind="oracle",
-                sample="%s cut to %dx%dx%d (same zone size), %d steps after %d warm-up, oracle/libkho_omp.so"
-                       % (name, q["n1"], q["n2"], q["n3"], steps, warmup)), el / steps * 1e3
+    if omp:
+        cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    else:
+        cores = 1
+    what = "%s at %dx%dx%d%s" % (name, q["n1"], q["n2"], q["n3"], "" if full or q["n3"] == p["n3"] else " (cut in x3, same zone size)")
+    return dict(value=zones * done / el, unit="zone-cycles/s", cores=cores, kind="oracle",
+                sample="%s, %d steps after %d warm-up, oracle/%s" % (what, done, warmup, "libkho_omp.so" if omp else "libkho.so")), el / done * 1e3
+
+
+def single_thread_leg(name, steps, budget_s):
+    """SURVEY 8(d) 'Timing the oracle beside it': the single-threaded oracle pinned with `taskset -c 0` in a child
+    process; returns its cpu_baseline dict with '1 of N cores' stated."""
+    cmd = ["taskset", "-c", "0", sys.executable, os.path.abspath(__file__), "--oracle-leg", name, "--steps", str(steps),
+           "--leg-budget", str(budget_s)]
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    try:
+        r = subprocess.run(cmd, capture_output=True, text=True, env=env, timeout=max(600.0, 20 * budget_s))
+        d = json.loads(r.stdout.strip().splitlines()[-1])
+    except Exception as e:       # taskset missing, oracle not built, ...: report, do not fail the GPU line
+        return {"error": "%s: %s" % (type(e).__name__, str(e)[:200])}
+    d["pinning"] = "taskset -c 0, 1 of %d cores" % (os.cpu_count() or 1)
+    return d
+
+
+def run_oracle_leg(args):
+    cb, _ = time_oracle(args.oracle_leg, steps=args.steps, warmup=0, omp=False, full=True, budget_s=args.leg_budget)
+    print(json.dumps(cb))
+    return 0
+
+
+def cpu_baseline_legs(workload, full_protocol):
+    """The oracle timed on this box's host cores (a reported baseline, not the target).  `value` is the OpenMP build on
+    all cores on the default bounded sample; `single_thread` holds the SURVEY 8(d) single-thread legs: config 5 at 64^3
+    (MC and WENO5) and the full config-3 block.  full_protocol: 20 steps / 2 steps as 8(d) states (minutes of CPU work);
+    otherwise each leg stops after the first step that ends beyond ~10 s, so the default run stays within a few minutes."""
+    cb, _ = time_oracle(workload, steps=8, warmup=1)
+    cb["label"] = "OpenMP build of the oracle, %d threads" % cb["cores"]
+    budget = 1e9 if full_protocol else 10.0
+    legs = {}
+    for leg, steps in (("minkowski_64_mc", 20), ("minkowski_64_weno5", 20), ("torus_sane_192x128x128_weno5", 2)):
+        legs[leg] = single_thread_leg(leg, steps, budget)
+    cb["single_thread"] = legs
+    cb["protocol"] = "SURVEY 8(d): 64^3 x 20 steps, config 3 x 2 steps" if full_protocol else \
+        "bounded: each single-thread leg stops after the first step ending beyond 10 s (--cpu-full runs 20 / 2 steps)"
+    return cb
 
 
 def run_reference(args):
@@ -314,12 +361,12 @@ def run_ours(args):
             g.set_face_B(*facefield.face_from_potential(p, *facefield.axisymmetric_loop_potential(p, amp=2e-3, x1c=2.5)))
         dt0 = g.estimate_dt()
         # ---- device-resident timing: W warm-up steps, then exactly K steps between two events on the grid's stream
+        clocks = ClockSampler(local)      # samples the warm-up and the timed steps (both under load)
+        clocks.start()
         g.step(dt0, sync=False)
         for _ in range(W - 1):
             g.step(-1.0, sync=False)
         barrier()
-        clocks = ClockSampler(local)
-        clocks.start()
         l0 = g.launch_count()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
@@ -370,18 +417,35 @@ def run_ours(args):
     value = world * zones * K / (ms_total * 1e-3)
     kern = kernel_table(prof, K, zones, p["recon"], flat, hbm_peak, fp64_tf)
     timed = {k: v for k, v in kern.items() if "bound" in v}
-    # dominant kernel = the largest share of the instrumented step (the three flux directions are one kernel template)
-    dom = max(kern, key=lambda k: kern[k]["ms_per_step"])
-    d = kern[dom]
-    if d.get("bound") == "alu":
-        roof = {"kernel": dom, "bound": "alu", "achieved": d["tflops"], "peak": fp64_tf, "unit": "TFLOP/s",
-                "frac": d["frac_alu"], "peak_source": "measured here: kh_measure_fp64_peak (DFMA chains)"}
+    # The three flux directions are ONE kernel template (flux_x1_kernel / flux_march_kernel<2|3> share the reconstruction
+    # and the face flux): aggregate them before picking the dominant kernel of the step.
+    fl = [kern[k] for k in ("flux1", "flux2", "flux3") if k in kern]
+    groups = {k: v["ms_per_step"] for k, v in kern.items() if not k.startswith("flux")}
+    if fl:
+        groups["flux"] = sum(v["ms_per_step"] for v in fl)
+    dom = max(groups, key=groups.get)
+    if dom == "flux":
+        nl = sum(v["launch_groups_per_step"] for v in fl)
+        byts = sum(v["alg_bytes_per_launch"] * v["launch_groups_per_step"] for v in fl)
+        flops = sum(v["alg_flops_per_launch"] * v["launch_groups_per_step"] for v in fl)
+        t = groups["flux"] * 1e-3
+        d = {"ms_per_launch": groups["flux"] / nl, "gbs": byts / t / 1e9, "tflops": flops / t / 1e12}
+        d["frac_hbm"], d["frac_alu"] = d["gbs"] / hbm_peak, d["tflops"] / fp64_tf
+        d["bound"] = "hbm" if byts / (hbm_peak * 1e9) >= flops / (fp64_tf * 1e12) else "alu"
+        traffic = float(np.mean([NCU_DRAM_BYTES_PER_LAUNCH[k] for k in ("flux1", "flux2", "flux3")]))
     else:
-        roof = {"kernel": dom, "bound": "hbm", "achieved": d.get("gbs"), "peak": hbm_peak, "unit": "GB/s",
-                "frac": d.get("frac_hbm"), "peak_source": hbm_src}
+        d = kern[dom]
+        traffic = NCU_DRAM_BYTES_PER_LAUNCH.get(dom)
+    roof = {"kernel": dom, "bound": d.get("bound"), "share_of_step": groups[dom] / sum(groups.values())}
+    if d.get("bound") == "alu":
+        roof.update(achieved=d["tflops"], peak=fp64_tf, unit="TFLOP/s", frac=d["frac_alu"],
+                    peak_source="measured here: kh_measure_fp64_peak (DFMA chains)")
+    else:
+        roof.update(achieved=d.get("gbs"), peak=hbm_peak, unit="GB/s", frac=d.get("frac_hbm"), peak_source=hbm_src)
+    roof["frac_hbm"], roof["frac_alu"] = d.get("frac_hbm"), d.get("frac_alu")
     # dram__bytes_read.sum + dram__bytes_write.sum per launch of that kernel from the committed ncu --set full capture
     # (not measurable in-process); only the default workload has one
-    roof["traffic"] = NCU_DRAM_BYTES_PER_LAUNCH.get(dom) if args.workload == DEFAULT_WORKLOAD else None
+    roof["traffic"] = traffic if args.workload == DEFAULT_WORKLOAD else None
     roof["traffic_source"] = NCU_DRAM_SOURCE if roof["traffic"] else None
     roof["ms_per_launch"] = d.get("ms_per_launch")
     prof_ms_step = sum(v["ms_per_step"] for v in kern.values())
@@ -390,7 +454,7 @@ def run_ours(args):
     step_tf = step_flops / (ms_step * 1e-3) / 1e12
     t_hbm, t_alu = ALG_BYTES_PER_ZONE_STEP * zones / (hbm_peak * 1e9), step_flops / (fp64_tf * 1e12)
 
-    cb, _ = time_oracle(args.workload, steps=8, warmup=1) if not args.no_cpu else (None, None)
+    cb = cpu_baseline_legs(args.workload, args.cpu_full) if not args.no_cpu else None
     line = {
         "metric": "zone-cycles/sec (fp64 HARM step)", "value": value, "unit": "zone-cycles/s", "n_gpus": world,
         "steps": K, "warmup": W, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
@@ -432,7 +496,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    ap.add_argument("--cpu-full", action="store_true", help="single-thread oracle legs with SURVEY 8(d)'s full step counts")
+    ap.add_argument("--oracle-leg", default=None, choices=sorted(WORKLOADS), help=argparse.SUPPRESS)   # child of single_thread_leg
+    ap.add_argument("--leg-budget", type=float, default=10.0, help=argparse.SUPPRESS)
     args = ap.parse_args()
+    if args.oracle_leg:
+        return run_oracle_leg(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

