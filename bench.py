@@ -265,24 +265,32 @@ def kernel_table(prof, steps, zones, recon, flat, hbm_peak, fp64_peak_tf):
     """Per kernel kind: ms per step, launches per step, achieved GB/s and TFLOP/s of the algorithmic work and
     the fraction of each roof; `bound` = the roof that takes longer for that kernel's algorithmic work."""
     rows = {}
+    # The three flux directions of a sub-step run CONCURRENTLY (x2 and x3 on side streams, DESIGN.md "Launch"): the library
+    # then brackets the group as one entry under "flux1" and reports nothing for flux2 / flux3.  It is listed as "flux" here:
+    # one launch group = the three kernels of one sub-step.
+    grouped = prof.get("flux1", (0, 0))[1] > 0 and prof.get("flux2", (0, 0))[1] == 0 and prof.get("flux3", (0, 0))[1] == 0
     for kind, (ms, cnt) in prof.items():
         if cnt == 0:
             continue
         per_step, lps = ms / steps, cnt / steps
+        if grouped and kind == "flux1":
+            kind = "flux"
         row = {"ms_per_step": per_step, "launch_groups_per_step": lps}
         base = "flux" if kind.startswith("flux") else kind
         if base in ("flux", "emf", "update"):
+            ndir = 3 if kind == "flux" else 1              # kernels per launch group
             if base == "update":   # one predictor + one corrector launch per step
                 dbl = ALG_DOUBLES["update_pred"] + ALG_DOUBLES["update_corr"]
                 nl = 2
             else:
-                dbl, nl = ALG_DOUBLES[base] * 2, 2
+                dbl, nl = ALG_DOUBLES[base] * 2 * ndir, 2 * ndir
             byts = 8.0 * dbl * zones                       # per step (nl launches)
             flops = ALG_FLOPS[(base, recon, flat)] * nl * zones
             t = per_step * 1e-3
             gbs, tfs = byts / t / 1e9, flops / t / 1e12
             t_hbm, t_alu = byts / (hbm_peak * 1e9), flops / (fp64_peak_tf * 1e12)
             row.update(alg_bytes_per_launch=byts / nl, alg_flops_per_launch=flops / nl, ms_per_launch=per_step / nl,
+                       alg_bytes_per_step=byts, alg_flops_per_step=flops, kernel_launches_per_step=nl,
                        gbs=gbs, tflops=tfs, frac_hbm=gbs / hbm_peak, frac_alu=tfs / fp64_peak_tf,
                        bound="hbm" if t_hbm >= t_alu else "alu")
         rows[kind] = row
@@ -419,15 +427,15 @@ def run_ours(args):
     timed = {k: v for k, v in kern.items() if "bound" in v}
     # The three flux directions are ONE kernel template (flux_x1_kernel / flux_march_kernel<2|3> share the reconstruction
     # and the face flux): aggregate them before picking the dominant kernel of the step.
-    fl = [kern[k] for k in ("flux1", "flux2", "flux3") if k in kern]
+    fl = [kern[k] for k in ("flux", "flux1", "flux2", "flux3") if k in kern]
     groups = {k: v["ms_per_step"] for k, v in kern.items() if not k.startswith("flux")}
     if fl:
         groups["flux"] = sum(v["ms_per_step"] for v in fl)
     dom = max(groups, key=groups.get)
     if dom == "flux":
-        nl = sum(v["launch_groups_per_step"] for v in fl)
-        byts = sum(v["alg_bytes_per_launch"] * v["launch_groups_per_step"] for v in fl)
-        flops = sum(v["alg_flops_per_launch"] * v["launch_groups_per_step"] for v in fl)
+        nl = 6.0                                                   # kernel launches of the template per step (3 directions x 2 sub-steps)
+        byts = sum(v["alg_bytes_per_step"] for v in fl)
+        flops = sum(v["alg_flops_per_step"] for v in fl)
         t = groups["flux"] * 1e-3
         d = {"ms_per_launch": groups["flux"] / nl, "gbs": byts / t / 1e9, "tflops": flops / t / 1e12}
         d["frac_hbm"], d["frac_alu"] = d["gbs"] / hbm_peak, d["tflops"] / fp64_tf
@@ -450,7 +458,7 @@ def run_ours(args):
     roof["ms_per_launch"] = d.get("ms_per_launch")
     prof_ms_step = sum(v["ms_per_step"] for v in kern.values())
     step_gbs = ALG_BYTES_PER_ZONE_STEP * zones / (ms_step * 1e-3) / 1e9
-    step_flops = sum(v["alg_flops_per_launch"] * 2 for v in timed.values())
+    step_flops = sum(v["alg_flops_per_step"] for v in timed.values())
     step_tf = step_flops / (ms_step * 1e-3) / 1e12
     t_hbm, t_alu = ALG_BYTES_PER_ZONE_STEP * zones / (hbm_peak * 1e9), step_flops / (fp64_tf * 1e12)
 

@@ -22,7 +22,12 @@
  *   - errors: every call returns KH_OK (0) or a negative code; no exceptions or aborts cross the ABI;
  *     out-parameters are untouched on error.  U->P failures are DATA (pflag), not errors.
  *   - threading: calls on one grid must be serialised by the caller; all work is enqueued on the
- *     stream given at creation (0 = the legacy default stream)
+ *     grid's stream: the one given at creation, or, for NULL, a blocking stream the grid creates for
+ *     itself (the legacy default stream cannot be captured into a CUDA graph).  That own stream orders
+ *     against the legacy default stream only; callers on other streams order against the grid with
+ *     kh_get_stream / kh_sync.  KH_MEM_DEVICE transfers and kh_step(..., NULL) return without waiting.
+ *   - device: a grid lives on the CUDA device that was current at kh_grid_create; every call makes that
+ *     device current for the calling thread.
  */
 #ifndef KHARM_H
 #define KHARM_H
@@ -75,12 +80,19 @@ typedef struct kh_grid kh_grid;   /* opaque */
 /* Create a grid on the current CUDA device and run the one-time geometry precompute (kernel K1:
  * gcov, gcon, sqrt(-g), lapse at zone centres and the three face centres, connection coefficients
  * and floor profiles at centres; the "caches of expensive-to-calculate quantities" of P:285).
- * cuda_stream: a cudaStream_t (as void*), or NULL for the default stream. */
+ * cuda_stream: a cudaStream_t (as void*), or NULL: the grid then creates its own blocking stream. */
 int kh_grid_create(const kh_params* params, void* cuda_stream, kh_grid** out);
 int kh_grid_destroy(kh_grid* g);
+/* The stream every call on this grid enqueues on (a cudaStream_t as void*), and a wait for all of it. */
+int kh_get_stream(kh_grid* g, void** cuda_stream);
+int kh_sync(kh_grid* g);
 
 /* Load primitives and fill the ghost zones (periodic / outflow / polar as configured; KH_BC_FIXED
- * ghosts keep what a with_ghosts = 1 array supplies).  Kernel K7. */
+ * ghosts keep what a with_ghosts = 1 array supplies).  Kernel K7.
+ * A grid with a KH_BC_FIXED side needs one with_ghosts = 1 load before anything else: until then
+ * kh_set_prims(with_ghosts = 0) and kh_step return KH_EINVAL (the fixed layers would be vacuum).
+ * On a face-centred CT grid whose face field has been set (kh_set_face_B), the face field remains the
+ * magnetic state: the B components of p are replaced by the face means. */
 int kh_set_prims(kh_grid* g, const double* p, int with_ghosts, int mem);
 int kh_get_prims(kh_grid* g, double* p, int with_ghosts, int mem);
 
@@ -94,7 +106,9 @@ int kh_get_cons(kh_grid* g, double* u, int mem);
  * 16 u/rho ceiling, 32 Lorentz-factor ceiling.  Either pointer may be NULL. */
 int kh_get_flags(kh_grid* g, int* pflag, int* fflag, int mem);
 
-/* CFL time step from zone-centred fast-magnetosonic speeds (for the first step).  *dt is a HOST double. */
+/* CFL time step dt = cfl / max_zones sum_d c^d / dx_d from zone-centred fast-magnetosonic speeds c^d, for the
+ * first step (the step is set by the signal crossing time of the smallest zones; S22).
+ * *dt is a HOST double.  KH_ENAN if a zone's speed is not finite. */
 int kh_estimate_dt(kh_grid* g, double* dt);
 
 /* One full predictor-corrector step:
@@ -103,9 +117,12 @@ int kh_estimate_dt(kh_grid* g, double* dt);
  * conserved update + 1D_W inversion + floors (K4/K5), ghost fill (K7), fix-up of failed zones (K5b),
  * ghost fill; the corrector's face speeds give the next CFL step (K6).
  *   dt > 0   : use this step
- *   dt <= 0  : use the device-resident dt_next of the previous step (no host round trip)
+ *   dt <= 0  : use the device-resident dt_next of the previous step (no host round trip); KH_EINVAL
+ *              before the first completed step of the grid
  *   dt_next  : HOST pointer receiving min(cfl * min_zones dt_zone, dt_growth_max * dt), or NULL to
- *              return without synchronising (the value stays on the device for the next dt <= 0 call) */
+ *              return without synchronising (the value stays on the device for the next dt <= 0 call)
+ * KH_ENAN (with dt_next given): a zone's CFL rate of this step was not finite; dt_next is untouched.
+ * The step replays a CUDA graph; if the stream cannot be captured the same kernels are launched directly. */
 int kh_step(kh_grid* g, double dt, double* dt_next);
 
 /* max |div B| of the corner-centred divergence that Flux-CT preserves.  HOST double. */

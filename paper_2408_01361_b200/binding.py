@@ -21,7 +21,7 @@ EXPORTED_SYMBOLS = (
     "kh_grid_create", "kh_grid_destroy", "kh_set_prims", "kh_get_prims", "kh_get_cons", "kh_get_flags",
     "kh_estimate_dt", "kh_step", "kh_divB", "kh_set_face_B", "kh_get_face_B", "kh_divB_face", "kh_count_flags", "kh_get_geom", "kh_get_conn", "kh_get_flux",
     "kh_get_emf", "kh_debug_fixup", "kh_debug_predictor", "kh_launch_count", "kh_set_graph", "kh_set_profile", "kh_get_profile", "kh_measure_fp64_peak", "kh_strerror",
-    "kh_last_cuda_error",
+    "kh_last_cuda_error", "kh_get_stream", "kh_sync",
 )
 
 
@@ -95,6 +95,8 @@ def lib():
         L.kh_set_profile.argtypes = [C.c_void_p, C.c_int]
         L.kh_get_profile.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
         L.kh_measure_fp64_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.kh_get_stream.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
+        L.kh_sync.argtypes = [C.c_void_p]
         _LIB = L
     return _LIB
 
@@ -265,6 +267,14 @@ class Grid:
         pf = np.ascontiguousarray(pflag_with_ghosts, dtype=np.int32)
         assert pf.shape == self.shape_gh[1:]
         _chk(self.L.kh_debug_fixup(self.h, _np_ptr(pf), MEM_HOST))
+
+    def get_stream(self):
+        s = C.c_void_p()
+        _chk(self.L.kh_get_stream(self.h, C.byref(s)))
+        return int(s.value or 0)
+
+    def sync(self):
+        _chk(self.L.kh_sync(self.h))
 
     def launch_count(self):
         return int(self.L.kh_launch_count(self.h))

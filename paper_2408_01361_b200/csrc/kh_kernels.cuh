@@ -46,6 +46,7 @@ struct StepScalars {        // device-resident scalars of the time stepping
   unsigned long long rate_bits;  // running max of sum_d(c^d/dx_d) as ordered bits (non-negative doubles): dt = cfl / max
   unsigned long long max_bits;   // scratch for max reductions
   unsigned long long n_pflag, n_fflag;
+  unsigned long long nonfinite;  // sticky: a zone's CFL rate was not finite (fmax drops NaNs, so the maximum alone would hide it)
 };
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
@@ -355,6 +356,200 @@ emf_upwind_kernel(GV g, const double* __restrict__ F1, const double* __restrict_
 // ---------------------------------------------------------------------------------------------
 // MODE = inverter (bit 0: 0 1D_W, 1 Kastaun) + 2 * floor frame (0 fluid, 1 drift, 2 normal observer) + 8 if the zone-centred
 // field comes from the face field (face-centred CT)
+//
+// The zone's arithmetic (update_zone) is written once against an accessor A that hands out the streamed inputs of the zone:
+//   A.pi(v), A.ps(v)                      primitives P_i, P_s
+//   A.f1(v, d), A.f2(v, d), A.f3(v, d)    hydro flux component v at the lower (d = 0) / upper (d = 1) face of the direction
+//   A.e3(di, dj), A.e2(di, dk), A.e1(dj, dk)   edge EMFs at the zone's corners;  A.bf1(d), A.bf2(d), A.bf3(d) face field
+//   A.c1(d), A.c2(d), A.c3(d)             c_top at the lower / upper face
+// GlobalAcc reads them from HBM / L2 per thread (update_kernel); TileAcc reads them from the warp's shared-memory tile that
+// TMA bulk copies filled (update_tma_kernel).  Same arithmetic, bit-identical results.
+struct GlobalAcc {
+  const double *Pi, *Ps, *F1, *F2, *F3, *E1, *E2, *E3, *C1, *C2, *C3, *Bf1, *Bf2, *Bf3;
+  long n, nt, s2, s3;
+  __device__ __forceinline__ double pi(int v) const { return Pi[v * nt + n]; }
+  __device__ __forceinline__ double ps(int v) const { return Ps[v * nt + n]; }
+  __device__ __forceinline__ double f1(int v, int d) const { return F1[v * nt + n + d]; }
+  __device__ __forceinline__ double f2(int v, int d) const { return F2[v * nt + n + d * s2]; }
+  __device__ __forceinline__ double f3(int v, int d) const { return F3[v * nt + n + d * s3]; }
+  __device__ __forceinline__ double e3(int di, int dj) const { return E3[n + di + dj * s2]; }
+  __device__ __forceinline__ double e2(int di, int dk) const { return E2[n + di + dk * s3]; }
+  __device__ __forceinline__ double e1(int dj, int dk) const { return E1[n + dj * s2 + dk * s3]; }
+  __device__ __forceinline__ double bf1(int d) const { return Bf1[n + d]; }
+  __device__ __forceinline__ double bf2(int d) const { return Bf2[n + d * s2]; }
+  __device__ __forceinline__ double bf3(int d) const { return Bf3[n + d * s3]; }
+  __device__ __forceinline__ double c1(int d) const { return C1[n + d]; }
+  __device__ __forceinline__ double c2(int d) const { return C2[n + d * s2]; }
+  __device__ __forceinline__ double c3(int d) const { return C3[n + d * s3]; }
+};
+
+// Layout of a warp's tile (32 zones of one x1 row) in shared memory, in doubles.  Rows whose x1 neighbour i+1 is read hold
+// 34 doubles (272 B: a multiple of 16 B for the bulk copy), the others 32.
+template <bool FLAT, bool CORR, int MODE>
+struct TileLayout {
+  static constexpr bool FACE = (MODE & 8) != 0;
+  static constexpr bool PS = CORR && !FLAT;            // a separate P_s (predictor: P_s = P_i; Minkowski: no source term)
+  static constexpr int WL = 34, WS = 32;
+  static constexpr int F1 = 0;                                   // 5 long rows
+  static constexpr int E3 = F1 + 5 * WL;                         // 2 long rows (j, j+1)          | face CT: BF1, 1 long row
+  static constexpr int E2 = E3 + (FACE ? 1 : 2) * WL;            // 2 long rows (k, k+1)          | face CT: none
+  static constexpr int C1 = E2 + (FACE ? 0 : 2) * WL;            // 1 long row (corrector)
+  static constexpr int F2 = C1 + (CORR ? 1 : 0) * WL;            // 5 x 2 rows
+  static constexpr int F3 = F2 + 10 * WS;                        // 5 x 2 rows
+  static constexpr int E1 = F3 + 10 * WS;                        // 4 rows (j, k), (j+1, k), (j, k+1), (j+1, k+1) | face CT: BF2 x 2, BF3 x 2
+  static constexpr int PI = E1 + 4 * WS;                         // 8 rows
+  static constexpr int PSO = PI + 8 * WS;                        // 8 rows if PS
+  static constexpr int C2 = PSO + (PS ? 8 : 0) * WS;             // 2 rows (corrector)
+  static constexpr int C3 = C2 + (CORR ? 2 : 0) * WS;            // 2 rows (corrector)
+  static constexpr int DOUBLES = C3 + (CORR ? 2 : 0) * WS;
+  static constexpr int BYTES = DOUBLES * 8;                      // per warp; a multiple of 16
+};
+
+template <bool FLAT, bool CORR, int MODE>
+struct TileAcc {
+  using L = TileLayout<FLAT, CORR, MODE>;
+  const double* t;      // the warp's tile + lane
+  __device__ __forceinline__ double pi(int v) const { return t[L::PI + v * L::WS]; }
+  __device__ __forceinline__ double ps(int v) const { return t[(L::PS ? L::PSO : L::PI) + v * L::WS]; }
+  __device__ __forceinline__ double f1(int v, int d) const { return t[L::F1 + v * L::WL + d]; }
+  __device__ __forceinline__ double f2(int v, int d) const { return t[L::F2 + (2 * v + d) * L::WS]; }
+  __device__ __forceinline__ double f3(int v, int d) const { return t[L::F3 + (2 * v + d) * L::WS]; }
+  __device__ __forceinline__ double e3(int di, int dj) const { return t[L::E3 + dj * L::WL + di]; }
+  __device__ __forceinline__ double e2(int di, int dk) const { return t[L::E2 + dk * L::WL + di]; }
+  __device__ __forceinline__ double e1(int dj, int dk) const { return t[L::E1 + (2 * dk + dj) * L::WS]; }
+  __device__ __forceinline__ double bf1(int d) const { return t[L::E3 + d]; }
+  __device__ __forceinline__ double bf2(int d) const { return t[L::E1 + d * L::WS]; }
+  __device__ __forceinline__ double bf3(int d) const { return t[L::E1 + (2 + d) * L::WS]; }
+  __device__ __forceinline__ double c1(int d) const { return t[L::C1 + d]; }
+  __device__ __forceinline__ double c2(int d) const { return t[L::C2 + d * L::WS]; }
+  __device__ __forceinline__ double c3(int d) const { return t[L::C3 + d * L::WS]; }
+};
+
+// Phase A: everything that consumes the streamed inputs -- the advanced conserved state Uh = U_f / sqrt(-g), the guess W0 and
+// (corrector) the zone's CFL rate.
+template <bool FLAT, bool CORR, int MODE, class ACC>
+__device__ __forceinline__ void update_zone_a(const GV& g, const ACC& A, const Geo& G, long p2, double Dt, double Uh[KH_NP], double& W0,
+                                              double& rate) {
+  const double ialpha = FLAT ? 1.0 : -G.n00 * G.alpha;
+  const double gm1 = g.gam - 1.0;
+  double S1 = 0.0, S2 = 0.0;
+  {
+    double pi[KH_NP];
+#pragma unroll
+    for (int v = 0; v < KH_NP; v++) pi[v] = A.pi(v);
+    FourVec D;
+    four_vectors<FLAT>(G, ialpha, pi, D);
+    double pg = gm1 * pi[UU], ef = fma(g.gam, pi[UU], pi[RHO]);
+    double ee = ef + D.bsq, ptot = fma(0.5, D.bsq, pg);
+    double eu[4] = {ee * D.ucov[0], ee * D.ucov[1], ee * D.ucov[2], ee * D.ucov[3]};
+    flux_row(pi, D, eu, ptot, 0, Uh);
+    W0 = ef * D.x;
+    if (!FLAT) {
+      double ps[KH_NP];
+      if (CORR) {
+#pragma unroll
+        for (int v = 0; v < KH_NP; v++) ps[v] = A.ps(v);
+        four_vectors<FLAT>(G, ialpha, ps, D);
+        pg = gm1 * ps[UU];
+        ee = fma(g.gam, ps[UU], ps[RHO]) + D.bsq;
+        ptot = fma(0.5, D.bsq, pg);
+      }
+      // T^{kap lam} = (w + b^2) u^kap u^lam + (p + b^2/2) g^{kap lam} - b^kap b^lam on the packed pairs with d g != 0
+      const double* __restrict__ dg = g.dg + p2;
+      const long m = g.n2d;
+      double eu0 = ee * D.ucon[0], eu1 = ee * D.ucon[1], eu2 = ee * D.ucon[2], eu3 = ee * D.ucon[3];
+#define KH_T(a, b, gc) fma(eu##a, D.ucon[b], fma(ptot, gc, -D.bcon[a] * D.bcon[b]))
+#define KH_ACC(c, T) { double T_ = (T); S1 = fma(T_, __ldg(dg + (long)(c) * m), S1); S2 = fma(T_, __ldg(dg + (long)(10 + (c)) * m), S2); }
+      KH_ACC(G00, KH_T(0, 0, G.n00));
+      KH_ACC(G01, KH_T(0, 1, G.n01));
+      KH_ACC(G03, fma(eu0, D.ucon[3], -D.bcon[0] * D.bcon[3]));            // g^03 = 0
+      KH_ACC(G11, KH_T(1, 1, G.n11));
+      KH_ACC(G12, KH_T(1, 2, G.n12));
+      KH_ACC(G13, KH_T(1, 3, G.n13));
+      KH_ACC(G22, KH_T(2, 2, G.n22));
+      KH_ACC(G33, KH_T(3, 3, G.n33));
+#undef KH_T
+#undef KH_ACC
+    }
+  }
+  const double dtg = FLAT ? Dt : Dt * fast_rcp(G.gdet);
+  // hydro flux divergence
+#pragma unroll
+  for (int v = 0; v < 5; v++) {
+    double div = fma(A.f3(v, 1) - A.f3(v, 0), g.idx3, fma(A.f2(v, 1) - A.f2(v, 0), g.idx2, (A.f1(v, 1) - A.f1(v, 0)) * g.idx1));
+    double src = (v == 2) ? S1 : (v == 3 ? S2 : 0.0);
+    Uh[v] = fma(dtg, src - div, Uh[v]);
+  }
+  // induction: Flux-CT fluxes from the edge EMFs (S15a); the factors 1/2 are applied once per component
+  if (MODE & 8) {   // face-centred CT (S28): the zone's conserved field is the mean of its two (already advanced) face values
+    const double hs = FLAT ? 0.5 : 0.5 * fast_rcp(G.gdet);
+    Uh[B1] = hs * (A.bf1(0) + A.bf1(1));
+    Uh[B2] = hs * (A.bf2(0) + A.bf2(1));
+    Uh[B3] = hs * (A.bf3(0) + A.bf3(1));
+  } else {
+    const double a00 = A.e3(0, 0), a10 = A.e3(1, 0), a01 = A.e3(0, 1), a11 = A.e3(1, 1);          // emf3 at (i,j) corners
+    const double b00 = A.e2(0, 0), b10 = A.e2(1, 0), b01 = A.e2(0, 1), b11 = A.e2(1, 1);          // emf2 at (i,k) corners
+    const double c00 = A.e1(0, 0), c10 = A.e1(1, 0), c01 = A.e1(0, 1), c11 = A.e1(1, 1);          // emf1 at (j,k) corners
+    const double h = 0.5 * dtg;
+    // dB1/dt = -[d2 F2[B1] + d3 F3[B1]],  F2[B1] = -1/2 (e3(i,j)+e3(i+1,j)),  F3[B1] = 1/2 (e2(i,k)+e2(i+1,k))
+    Uh[B1] = fma(h, ((a01 + a11) - (a00 + a10)) * g.idx2 - ((b01 + b11) - (b00 + b10)) * g.idx3, Uh[B1]);
+    // dB2/dt = -[d1 F1[B2] + d3 F3[B2]],  F1[B2] = 1/2 (e3(i,j)+e3(i,j+1)),  F3[B2] = -1/2 (e1(j,k)+e1(j+1,k))
+    Uh[B2] = fma(h, ((c01 + c11) - (c00 + c10)) * g.idx3 - ((a10 + a11) - (a00 + a01)) * g.idx1, Uh[B2]);
+    // dB3/dt = -[d1 F1[B3] + d2 F2[B3]],  F1[B3] = -1/2 (e2(i,k)+e2(i,k+1)),  F2[B3] = 1/2 (e1(j,k)+e1(j,k+1))
+    Uh[B3] = fma(h, ((b10 + b11) - (b00 + b01)) * g.idx1 - ((c10 + c11) - (c00 + c01)) * g.idx2, Uh[B3]);
+  }
+  if (CORR) {   // K6: CFL from the corrector's face speeds (S22): dt_zone = 1 / rate
+    if (g.ndim_mask & 1) rate = fmax(A.c1(0), A.c1(1)) * g.idx1;
+    if (g.ndim_mask & 2) rate = fma(fmax(A.c2(0), A.c2(1)), g.idx2, rate);
+    if (g.ndim_mask & 4) rate = fma(fmax(A.c3(0), A.c3(1)), g.idx3, rate);
+  }
+}
+// a zone rate that is not a finite number must not vanish in the fmax reduction: the high word decides on the integer pipe
+__device__ __forceinline__ bool rate_nonfinite(double r) { return ((unsigned)__double2hiint(r) & 0x7ff00000u) == 0x7ff00000u; }
+
+// Phase B: inversion + floors of the advanced state, stores.  Pi: the guess (global memory; read only by the rare failed zone).
+template <bool FLAT, int MODE>
+__device__ __forceinline__ void update_zone_b(const GV& g, const Geo& G, const double Uh[KH_NP], double W0, long n, long p2,
+                                              const double* __restrict__ Pi, double* __restrict__ Pf, unsigned char* __restrict__ pflag,
+                                              unsigned char* __restrict__ fflag, unsigned* __restrict__ faillist,
+                                              StepScalars* __restrict__ sc, int& pf_flag, int& ff) {
+  const long nt = g.ntot;
+  double pf[KH_NP];
+  {
+    const double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2);
+    const double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
+    pf_flag = invert_with_floors<FLAT, MODE & 1>(G, Uh, W0, g.gam, g.fp, (MODE & 7) >> 1, rho_g, u_g, pf, ff);
+  }
+  if (pf_flag != 0) {          // rare: the hydro primitives keep the guess (S16); queue the zone for the fix-up
+#pragma unroll
+    for (int v = 0; v < 5; v++) pf[v] = Pi[v * nt + n];
+    faillist[atomicAdd(&sc->n_pflag, 1ULL)] = (unsigned)n;
+  }
+#pragma unroll
+  for (int v = 0; v < KH_NP; v++) Pf[v * nt + n] = pf[v];
+  pflag[n] = (unsigned char)pf_flag;
+  fflag[n] = (unsigned char)ff;
+}
+
+// block-level bookkeeping of both update kernels: failure counters and the CFL rate maximum (min over zones of 1/rate)
+template <bool CORR>
+__device__ __forceinline__ void update_block_tail(StepScalars* __restrict__ sc, double rate, int ff) {
+  unsigned nf = __syncthreads_count(ff != 0);
+  if (threadIdx.x == 0 && nf) atomicAdd(&sc->n_fflag, (unsigned long long)nf);
+  if (CORR) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) rate = fmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
+    __shared__ double wmax[4];
+    if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = rate;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      double m = fmax(fmax(wmax[0], wmax[1]), fmax(wmax[2], wmax[3]));
+      atomicMax(&sc->rate_bits, (unsigned long long)__double_as_longlong(m));   // non-negative doubles order as integers
+    }
+  }
+}
+
+// Variant 1 (any grid): one thread per interior zone, flattened index, every input read by the thread itself.
 template <bool FLAT, bool CORR, int MODE>
 __global__ void __launch_bounds__(128, KH_MINB_UPDATE)
 update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps, double* __restrict__ Pf,
@@ -389,112 +584,181 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
     const double Dt = dt_factor * sc->dt;
     Geo G;
     load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, p2);
-    const double ialpha = FLAT ? 1.0 : -G.n00 * G.alpha;
-    const double gm1 = g.gam - 1.0;
-    double Uh[KH_NP], W0, S1 = 0.0, S2 = 0.0;
+    GlobalAcc A{Pi, Ps, F1, F2, F3, e1, e2, e3, ct1, ct2, ct3, Bface1, Bface2, Bface3, n, nt, g.s2, g.s3};
+    double Uh[KH_NP], W0;
+    update_zone_a<FLAT, CORR, MODE>(g, A, G, p2, Dt, Uh, W0, rate);
+    if (CORR && rate_nonfinite(rate)) { sc->nonfinite = 1ULL; rate = 0.0; }
+    update_zone_b<FLAT, MODE>(g, G, Uh, W0, n, p2, Pi, Pf, pflag, fflag, faillist, sc, pf_flag, ff);
+  }
+  update_block_tail<CORR>(sc, rate, ff);
+}
+
+// Variant 2 (even n1; the library's arrays start 8 B past a 16 B boundary so that interior zone i = 0 of every row is
+// 16 B aligned): a warp owns a tile of 32 zones of one x1 row.  One lane issues a TMA bulk copy (cp.async.bulk, completion
+// on the warp's mbarrier) per input row -- 41 (predictor) to 54 (corrector) rows of 256 / 272 B, ~14 KB per warp -- so that
+// ALL streamed inputs of the tile are in flight at once and cost neither registers nor issue slots of the other lanes; the
+// geometry loads go out meanwhile.  After the wait the zone arithmetic reads shared memory only.  (The per-thread variant
+// keeps ~5 loads in flight per warp and spends 58 % of its cycles with every warp waiting on one of five dependent load
+// phases: profiles/r02_*.)
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "KH_MBAR_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra KH_MBAR_DONE;\n"
+      "bra KH_MBAR_WAIT;\n"
+      "KH_MBAR_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(double* dst, const double* src, unsigned bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src),
+               "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+__device__ __forceinline__ bool elect_one() {     // one lane of the (converged) warp, chosen by the hardware
+  unsigned p;
+  asm volatile("{\n.reg .pred P;\nelect.sync _|P, 0xffffffff;\nselp.u32 %0, 1, 0, P;\n}\n" : "=r"(p));
+  return p != 0;
+}
+
+template <bool FLAT, bool CORR, int MODE>
+__device__ __forceinline__ void issue_tile(const GV& g, double* tile, unsigned long long* bar, long n0, const double* __restrict__ Pi,
+                                           const double* __restrict__ Ps, const double* __restrict__ F1, const double* __restrict__ F2,
+                                           const double* __restrict__ F3, const double* __restrict__ e1, const double* __restrict__ e2,
+                                           const double* __restrict__ e3, const double* __restrict__ ct1, const double* __restrict__ ct2,
+                                           const double* __restrict__ ct3, const double* __restrict__ Bface1, const double* __restrict__ Bface2,
+                                           const double* __restrict__ Bface3) {
+  using L = TileLayout<FLAT, CORR, MODE>;
+  const long nt = g.ntot, s2 = g.s2, s3 = g.s3;
+  constexpr unsigned BL = L::WL * 8, BS = L::WS * 8;
+  mbar_expect_tx(bar, (unsigned)L::BYTES);
+#pragma unroll
+  for (int v = 0; v < 5; v++) {
+    bulk_g2s(tile + L::F1 + v * L::WL, F1 + v * nt + n0, BL, bar);
+    bulk_g2s(tile + L::F2 + (2 * v) * L::WS, F2 + v * nt + n0, BS, bar);
+    bulk_g2s(tile + L::F2 + (2 * v + 1) * L::WS, F2 + v * nt + n0 + s2, BS, bar);
+    bulk_g2s(tile + L::F3 + (2 * v) * L::WS, F3 + v * nt + n0, BS, bar);
+    bulk_g2s(tile + L::F3 + (2 * v + 1) * L::WS, F3 + v * nt + n0 + s3, BS, bar);
+  }
+  if (MODE & 8) {
+    bulk_g2s(tile + L::E3, Bface1 + n0, BL, bar);
+    bulk_g2s(tile + L::E1, Bface2 + n0, BS, bar);
+    bulk_g2s(tile + L::E1 + L::WS, Bface2 + n0 + s2, BS, bar);
+    bulk_g2s(tile + L::E1 + 2 * L::WS, Bface3 + n0, BS, bar);
+    bulk_g2s(tile + L::E1 + 3 * L::WS, Bface3 + n0 + s3, BS, bar);
+  } else {
+    bulk_g2s(tile + L::E3, e3 + n0, BL, bar);
+    bulk_g2s(tile + L::E3 + L::WL, e3 + n0 + s2, BL, bar);
+    bulk_g2s(tile + L::E2, e2 + n0, BL, bar);
+    bulk_g2s(tile + L::E2 + L::WL, e2 + n0 + s3, BL, bar);
+    bulk_g2s(tile + L::E1, e1 + n0, BS, bar);
+    bulk_g2s(tile + L::E1 + L::WS, e1 + n0 + s2, BS, bar);
+    bulk_g2s(tile + L::E1 + 2 * L::WS, e1 + n0 + s3, BS, bar);
+    bulk_g2s(tile + L::E1 + 3 * L::WS, e1 + n0 + s2 + s3, BS, bar);
+  }
+#pragma unroll
+  for (int v = 0; v < KH_NP; v++) {
+    bulk_g2s(tile + L::PI + v * L::WS, Pi + v * nt + n0, BS, bar);
+    if (L::PS) bulk_g2s(tile + L::PSO + v * L::WS, Ps + v * nt + n0, BS, bar);
+  }
+  if (CORR) {
+    bulk_g2s(tile + L::C1, ct1 + n0, BL, bar);
+    bulk_g2s(tile + L::C2, ct2 + n0, BS, bar);
+    bulk_g2s(tile + L::C2 + L::WS, ct2 + n0 + s2, BS, bar);
+    bulk_g2s(tile + L::C3, ct3 + n0, BS, bar);
+    bulk_g2s(tile + L::C3 + L::WS, ct3 + n0 + s3, BS, bar);
+  }
+}
+
+// Persistent: the grid is sized to the resident blocks; every warp walks over the tiles T = warp, warp + #warps, ...  The
+// tile buffer is dead once phase A has formed the advanced conserved state, so the NEXT tile's copies are issued before the
+// inversion (phase B, ~60 % of a zone's instructions) and land while it runs: the loads of tile t+1 overlap the arithmetic of
+// tile t without a second buffer (16 warps x 14 KB already fill the SM's shared memory).
+template <bool FLAT, bool CORR, int MODE>
+__global__ void __launch_bounds__(128, KH_MINB_UPDATE)
+update_tma_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps, double* __restrict__ Pf,
+                  const double* __restrict__ F1, const double* __restrict__ F2, const double* __restrict__ F3,
+                  const double* __restrict__ e1, const double* __restrict__ e2, const double* __restrict__ e3,
+                  const double* __restrict__ ct1, const double* __restrict__ ct2, const double* __restrict__ ct3,
+                  unsigned char* __restrict__ pflag, unsigned char* __restrict__ fflag, unsigned* __restrict__ faillist,
+                  StepScalars* __restrict__ sc, double dt_factor, const double* __restrict__ Bface1, const double* __restrict__ Bface2,
+                  const double* __restrict__ Bface3) {
+  using L = TileLayout<FLAT, CORR, MODE>;
+  extern __shared__ __align__(16) double tiles[];
+  // warp-uniform by construction (the shuffle tells the compiler so: tile addresses then live in uniform registers)
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
+  double* const tile = tiles + warp * L::DOUBLES;
+  unsigned long long* const bar = reinterpret_cast<unsigned long long*>(tiles + 4 * L::DOUBLES) + warp;
+  const unsigned tpr = ((unsigned)g.n1 + 31u) >> 5;                      // tiles per row
+  const unsigned ntiles = tpr * (unsigned)g.n2 * (unsigned)g.n3, stride = gridDim.x * 4u;
+  unsigned T = blockIdx.x * 4u + (unsigned)warp;
+  double rate = 0.0;
+  int nff = 0;
+  const double Dt = dt_factor * sc->dt;
+  auto tile_origin = [&](unsigned t, int& i0, int& j, int& k) {
+    const unsigned row = t / tpr;
+    i0 = (int)(t - row * tpr) << 5;
+    k = (int)(row / (unsigned)g.n2);
+    j = (int)(row - (unsigned)k * (unsigned)g.n2);
+  };
+  int i0, j, k;
+  if (T < ntiles) {
+    tile_origin(T, i0, j, k);
+    if (elect_one()) {
+      mbar_init(bar, 1);
+      issue_tile<FLAT, CORR, MODE>(g, tile, bar, zidx(g, i0, j, k), Pi, Ps, F1, F2, F3, e1, e2, e3, ct1, ct2, ct3, Bface1, Bface2, Bface3);
+    }
+    __syncwarp();
+  }
+  unsigned parity = 0;
+  while (T < ntiles) {
+    const long n0 = zidx(g, i0, j, k);
+    const int i = i0 + lane;
+    const bool active = i < g.n1;
+    const long p2 = pidx(g, active ? i : g.n1 - 1, j);
+    Geo G;                                              // geometry of the zone (L2 resident tables): in flight during the wait
+    load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, p2);
+    mbar_wait(bar, parity);
+    parity ^= 1u;
+    double Uh[KH_NP], W0, r = 0.0;
     {
-      double pi[KH_NP];
-#pragma unroll
-      for (int v = 0; v < KH_NP; v++) pi[v] = Pi[v * nt + n];
-      FourVec D;
-      four_vectors<FLAT>(G, ialpha, pi, D);
-      double pg = gm1 * pi[UU], ef = fma(g.gam, pi[UU], pi[RHO]);
-      double ee = ef + D.bsq, ptot = fma(0.5, D.bsq, pg);
-      double eu[4] = {ee * D.ucov[0], ee * D.ucov[1], ee * D.ucov[2], ee * D.ucov[3]};
-      flux_row(pi, D, eu, ptot, 0, Uh);
-      W0 = ef * D.x;
-      if (!FLAT) {
-        double ps[KH_NP];
-        if (CORR) {
-#pragma unroll
-          for (int v = 0; v < KH_NP; v++) ps[v] = Ps[v * nt + n];
-          four_vectors<FLAT>(G, ialpha, ps, D);
-          pg = gm1 * ps[UU];
-          ee = fma(g.gam, ps[UU], ps[RHO]) + D.bsq;
-          ptot = fma(0.5, D.bsq, pg);
-        }
-        // T^{kap lam} = (w + b^2) u^kap u^lam + (p + b^2/2) g^{kap lam} - b^kap b^lam on the packed pairs with d g != 0
-        const double* __restrict__ dg = g.dg + p2;
-        const long m = g.n2d;
-        double eu0 = ee * D.ucon[0], eu1 = ee * D.ucon[1], eu2 = ee * D.ucon[2], eu3 = ee * D.ucon[3];
-#define KH_T(a, b, gc) fma(eu##a, D.ucon[b], fma(ptot, gc, -D.bcon[a] * D.bcon[b]))
-#define KH_ACC(c, T) { double T_ = (T); S1 = fma(T_, __ldg(dg + (long)(c) * m), S1); S2 = fma(T_, __ldg(dg + (long)(10 + (c)) * m), S2); }
-        KH_ACC(G00, KH_T(0, 0, G.n00));
-        KH_ACC(G01, KH_T(0, 1, G.n01));
-        KH_ACC(G03, fma(eu0, D.ucon[3], -D.bcon[0] * D.bcon[3]));            // g^03 = 0
-        KH_ACC(G11, KH_T(1, 1, G.n11));
-        KH_ACC(G12, KH_T(1, 2, G.n12));
-        KH_ACC(G13, KH_T(1, 3, G.n13));
-        KH_ACC(G22, KH_T(2, 2, G.n22));
-        KH_ACC(G33, KH_T(3, 3, G.n33));
-#undef KH_T
-#undef KH_ACC
+      TileAcc<FLAT, CORR, MODE> A{tile + lane};
+      update_zone_a<FLAT, CORR, MODE>(g, A, G, p2, Dt, Uh, W0, r);
+    }
+    __syncwarp();                                       // every lane has read its part of the tile
+    T += stride;
+    if (T < ntiles) {
+      tile_origin(T, i0, j, k);
+      if (elect_one()) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic-proxy reads before the async-proxy overwrite
+        issue_tile<FLAT, CORR, MODE>(g, tile, bar, zidx(g, i0, j, k), Pi, Ps, F1, F2, F3, e1, e2, e3, ct1, ct2, ct3, Bface1, Bface2, Bface3);
       }
     }
-    const double dtg = FLAT ? Dt : Dt * fast_rcp(G.gdet);
-    // hydro flux divergence
-#pragma unroll
-    for (int v = 0; v < 5; v++) {
-      const double* f1 = F1 + v * nt + n;
-      const double* f2 = F2 + v * nt + n;
-      const double* f3 = F3 + v * nt + n;
-      double div = fma(f3[g.s3] - f3[0], g.idx3, fma(f2[g.s2] - f2[0], g.idx2, (f1[1] - f1[0]) * g.idx1));
-      double src = (v == 2) ? S1 : (v == 3 ? S2 : 0.0);
-      Uh[v] = fma(dtg, src - div, Uh[v]);
+    if (active) {
+      int pf_flag, ff;
+      update_zone_b<FLAT, MODE>(g, G, Uh, W0, n0 + lane, p2, Pi, Pf, pflag, fflag, faillist, sc, pf_flag, ff);
+      nff += (ff != 0);
+      if (CORR) { if (rate_nonfinite(r)) sc->nonfinite = 1ULL; else rate = fmax(rate, r); }
     }
-    // induction: Flux-CT fluxes from the edge EMFs (S15a); the factors 1/2 are applied once per component
-    if (MODE & 8) {   // face-centred CT (S28): the zone's conserved field is the mean of its two (already advanced) face values
-      const double hs = FLAT ? 0.5 : 0.5 * fast_rcp(G.gdet);
-      Uh[B1] = hs * (Bface1[n] + Bface1[n + 1]);
-      Uh[B2] = hs * (Bface2[n] + Bface2[n + g.s2]);
-      Uh[B3] = hs * (Bface3[n] + Bface3[n + g.s3]);
-    } else {
-      const long s2 = g.s2, s3 = g.s3;
-      const double a00 = e3[n], a10 = e3[n + 1], a01 = e3[n + s2], a11 = e3[n + s2 + 1];          // emf3 at (i,j) corners
-      const double b00 = e2[n], b10 = e2[n + 1], b01 = e2[n + s3], b11 = e2[n + s3 + 1];          // emf2 at (i,k) corners
-      const double c00 = e1[n], c10 = e1[n + s2], c01 = e1[n + s3], c11 = e1[n + s2 + s3];        // emf1 at (j,k) corners
-      const double h = 0.5 * dtg;
-      // dB1/dt = -[d2 F2[B1] + d3 F3[B1]],  F2[B1] = -1/2 (e3(i,j)+e3(i+1,j)),  F3[B1] = 1/2 (e2(i,k)+e2(i+1,k))
-      Uh[B1] = fma(h, ((a01 + a11) - (a00 + a10)) * g.idx2 - ((b01 + b11) - (b00 + b10)) * g.idx3, Uh[B1]);
-      // dB2/dt = -[d1 F1[B2] + d3 F3[B2]],  F1[B2] = 1/2 (e3(i,j)+e3(i,j+1)),  F3[B2] = -1/2 (e1(j,k)+e1(j+1,k))
-      Uh[B2] = fma(h, ((c01 + c11) - (c00 + c10)) * g.idx3 - ((a10 + a11) - (a00 + a01)) * g.idx1, Uh[B2]);
-      // dB3/dt = -[d1 F1[B3] + d2 F2[B3]],  F1[B3] = -1/2 (e2(i,k)+e2(i,k+1)),  F2[B3] = 1/2 (e1(j,k)+e1(j,k+1))
-      Uh[B3] = fma(h, ((b10 + b11) - (b00 + b01)) * g.idx1 - ((c10 + c11) - (c00 + c01)) * g.idx2, Uh[B3]);
-    }
-    double pf[KH_NP];
-    {
-      const double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2);
-      const double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
-      pf_flag = invert_with_floors<FLAT, MODE & 1>(G, Uh, W0, g.gam, g.fp, (MODE & 7) >> 1, rho_g, u_g, pf, ff);
-    }
-    if (pf_flag != 0) {          // rare: the hydro primitives keep the guess (S16); queue the zone for the fix-up
-#pragma unroll
-      for (int v = 0; v < 5; v++) pf[v] = Pi[v * nt + n];
-      faillist[atomicAdd(&sc->n_pflag, 1ULL)] = (unsigned)n;
-    }
-#pragma unroll
-    for (int v = 0; v < KH_NP; v++) Pf[v * nt + n] = pf[v];
-    pflag[n] = (unsigned char)pf_flag;
-    fflag[n] = (unsigned char)ff;
-    if (CORR) {   // K6: CFL from the corrector's face speeds (S22): dt_zone = 1 / rate
-      if (g.ndim_mask & 1) rate = fmax(ct1[n], ct1[n + 1]) * g.idx1;
-      if (g.ndim_mask & 2) rate = fma(fmax(ct2[n], ct2[n + g.s2]), g.idx2, rate);
-      if (g.ndim_mask & 4) rate = fma(fmax(ct3[n], ct3[n + g.s3]), g.idx3, rate);
-    }
+    __syncwarp();
   }
-  // block-level bookkeeping: failure counters and the CFL rate maximum (min over zones of 1/rate = 1/max rate)
-  unsigned nf = __syncthreads_count(ff != 0);
-  if (threadIdx.x == 0 && nf) atomicAdd(&sc->n_fflag, (unsigned long long)nf);
+  // block-level bookkeeping, once per block: floor-hit counter and the CFL rate maximum
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) nff += __shfl_xor_sync(0xffffffffu, nff, o);
+  if (lane == 0 && nff) atomicAdd(&sc->n_fflag, (unsigned long long)nff);
   if (CORR) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) rate = fmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
-    __shared__ double wmax[4];
-    if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = rate;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      double m = fmax(fmax(wmax[0], wmax[1]), fmax(wmax[2], wmax[3]));
-      atomicMax(&sc->rate_bits, (unsigned long long)__double_as_longlong(m));   // non-negative doubles order as integers
-    }
+    if (lane == 0) atomicMax(&sc->rate_bits, (unsigned long long)__double_as_longlong(rate));   // non-negative doubles order as integers
   }
 }
 
@@ -502,10 +766,10 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
 __global__ void finalize_dt_kernel(StepScalars* sc, double cfl, double growth) {
   double m = 1.0 / __longlong_as_double((long long)sc->rate_bits);
   double d = cfl * m, cap = growth * sc->dt;
-  sc->dt_next = d < cap ? d : cap;
+  sc->dt_next = sc->nonfinite ? __longlong_as_double(0x7ff8000000000000LL) : (d < cap ? d : cap);     // kh_step reports KH_ENAN
   sc->rate_bits = 0ULL;
 }
-__global__ void set_dt_kernel(StepScalars* sc, double dt, int from_next) { sc->dt = from_next ? sc->dt_next : dt; }
+__global__ void set_dt_kernel(StepScalars* sc, double dt, int from_next) { sc->dt = from_next ? sc->dt_next : dt; sc->nonfinite = 0ULL; }
 __global__ void reset_counters_kernel(StepScalars* sc, int also_rate) {
   sc->n_pflag = 0; sc->n_fflag = 0;
   if (also_rate) sc->rate_bits = 0ULL;      // FOFC: the speculative corrector update has written its CFL maximum
@@ -846,6 +1110,7 @@ __global__ void estimate_dt_kernel(GV g, const double* __restrict__ P, StepScala
     if (g.ndim_mask & 2) rate = fma(cfast<FLAT>(D, ee, gg1u, G.n00, G.n02, G.n22, fma(G.n02, G.n02, -G.n00 * G.n22), 2), g.idx2, rate);
     if (g.ndim_mask & 4) rate = fma(cfast<FLAT>(D, ee, gg1u, G.n00, 0.0, G.n33, -G.n00 * G.n33, 3), g.idx3, rate);
   }
+  if (rate_nonfinite(rate)) { sc->nonfinite = 1ULL; rate = 0.0; }
   for (int o = 16; o > 0; o >>= 1) rate = fmax(rate, __shfl_xor_sync(0xffffffffu, rate, o));
   if ((threadIdx.x & 31) == 0) atomicMax(&sc->rate_bits, (unsigned long long)__double_as_longlong(rate));
 }

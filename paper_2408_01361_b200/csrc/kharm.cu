@@ -4,6 +4,7 @@
 #include "../../include/kharm.h"
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -40,7 +41,11 @@ struct kh_grid {
   double* emf[3];
   unsigned char *pflag, *fflag;
   double* ecent[4];      // upwinded EMFs: zone-centred reference values + conserved density (allocated on demand)
-  bool faces_set;        // face-centred CT: kh_set_face_B has been called
+  bool faces_set;        // face-centred CT: kh_set_face_B has been called (the face field is the magnetic state from then on)
+  bool has_fixed;        // some boundary is KH_BC_FIXED ...
+  bool fixed_ghosts_set; // ... and a with_ghosts = 1 load has supplied the ghost layers
+  bool have_dt_next;     // a completed step has left a dt_next on the device (kh_step(dt <= 0) is legal)
+  int device;            // the CUDA device the grid lives on
   double* Bf[3][3];      // face-centred CT: Phi^d per rotation state [state][d], [ntot] each (allocated on demand)
   unsigned char* mask;   // FOFC: troubled zones of the speculative update (with ghost images)
   unsigned* faillist;    // zones (device-layout index) whose inversion failed in the current sub-step
@@ -60,6 +65,13 @@ struct kh_grid {
   int* pkind;
   int npev;
   int sm_count, flux_blocks_per_sm;
+  // the three flux directions of a sub-step are independent: x2 and x3 run on two side streams (fork / join by events,
+  // captured into the step's graph), so that the last partial wave of one kernel is filled by the blocks of the next
+  cudaStream_t side[2];
+  cudaEvent_t ev_fork, ev_join[2];
+  bool flux_concurrent;
+  bool update_tma;            // update_tma_kernel (needs an even padded row length) instead of update_kernel
+  int march_J;                // 0 = chosen by march_chunk()
   double prof_ms[KH_K_COUNT];
   long long prof_n[KH_K_COUNT];
 };
@@ -116,6 +128,31 @@ static void setup_march_kernels() {
   setup_march_one<3, 0, true>(); setup_march_one<3, 1, true>(); setup_march_one<3, 0, false>(); setup_march_one<3, 1, false>();
 }
 
+template <bool FL, bool CO, int MODE>
+static constexpr size_t tile_smem_bytes() { return 4 * (size_t)TileLayout<FL, CO, MODE>::BYTES + 64; }     // 4 warp tiles + 4 mbarriers
+template <bool FL, bool CO, int MODE>
+static cudaError_t setup_update_tma_one() {
+  cudaError_t e = cudaFuncSetAttribute(update_tma_kernel<FL, CO, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_smem_bytes<FL, CO, MODE>());
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(update_tma_kernel<FL, CO, MODE>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  return e;
+}
+template <int MODE>
+static cudaError_t setup_update_tma_mode(bool flat) {
+  cudaError_t e = flat ? setup_update_tma_one<true, false, MODE>() : setup_update_tma_one<false, false, MODE>();
+  if (e == cudaSuccess) e = flat ? setup_update_tma_one<true, true, MODE>() : setup_update_tma_one<false, true, MODE>();
+  return e;
+}
+static cudaError_t setup_update_tma(bool flat, int mode) {
+  switch (mode) {
+    case 0: return setup_update_tma_mode<0>(flat); case 1: return setup_update_tma_mode<1>(flat);
+    case 2: return setup_update_tma_mode<2>(flat); case 3: return setup_update_tma_mode<3>(flat);
+    case 4: return setup_update_tma_mode<4>(flat); case 5: return setup_update_tma_mode<5>(flat);
+    case 8: return setup_update_tma_mode<8>(flat); case 9: return setup_update_tma_mode<9>(flat);
+    case 10: return setup_update_tma_mode<10>(flat); case 11: return setup_update_tma_mode<11>(flat);
+    case 12: return setup_update_tma_mode<12>(flat); default: return setup_update_tma_mode<13>(flat);
+  }
+}
+
 // Chunk length of the marching kernels: long enough that the one extra reconstruction per chunk is
 // small, short enough that the grid fills the SMs in an almost whole number of waves.
 static int march_chunk(const kh_grid* g, long columns, int faces) {
@@ -132,39 +169,50 @@ static int march_chunk(const kh_grid* g, long columns, int faces) {
 }
 
 template <int DIR>
-static void launch_flux(kh_grid* g, const double* Ps) {
+static void launch_flux(kh_grid* g, const double* Ps, cudaStream_t stream, bool prof) {
   const GV& v = g->gv;
   double* F = g->F[DIR - 1];
   double* ct = g->ctop[DIR - 1];
   const bool mc = g->p.recon == KH_RECON_MC;
-  prof_begin(g, KH_K_FLUX1 + DIR - 1);
+  if (prof) prof_begin(g, KH_K_FLUX1 + DIR - 1);
   if (DIR == 1) {
     const long zones = (long)(v.n1 + 2) * (v.n2 + 2) * (v.n3 + 2);
     const long warps = (zones + 30) / 31;
     const unsigned blocks = (unsigned)((warps + 3) / 4);
     if (g->flat) {
-      if (mc) flux_x1_kernel<0, true><<<blocks, 128, 0, g->stream>>>(v, Ps, F, ct);
-      else flux_x1_kernel<1, true><<<blocks, 128, 0, g->stream>>>(v, Ps, F, ct);
+      if (mc) flux_x1_kernel<0, true><<<blocks, 128, 0, stream>>>(v, Ps, F, ct);
+      else flux_x1_kernel<1, true><<<blocks, 128, 0, stream>>>(v, Ps, F, ct);
     } else {
-      if (mc) flux_x1_kernel<0, false><<<blocks, 128, 0, g->stream>>>(v, Ps, F, ct);
-      else flux_x1_kernel<1, false><<<blocks, 128, 0, g->stream>>>(v, Ps, F, ct);
+      if (mc) flux_x1_kernel<0, false><<<blocks, 128, 0, stream>>>(v, Ps, F, ct);
+      else flux_x1_kernel<1, false><<<blocks, 128, 0, stream>>>(v, Ps, F, ct);
     }
   } else {
     const int N = (DIR == 2) ? v.n2 : v.n3;
     const long cols = (long)(v.n1 + 2) * ((DIR == 2 ? v.n3 : v.n2) + 2);
-    const int J = march_chunk(g, cols, N + 1);
+    // concurrent directions: whole columns (no redundant reconstruction at chunk starts; the x1 kernel's many small blocks fill
+    // the SMs the few long-running marching blocks leave free); alone: chunks that fill the SMs in whole waves
+    int J;
+    if (g->march_J > 0) J = g->march_J;
+    else if (g->flux_concurrent) {
+      // a marching thread is a serial chain of J faces (~5300 cycles each when the SM is full) that must not outlast the
+      // whole group (3 Z zone-faces at ~2000 cycles per warp-face on 4 x SMs sub-partitions): J <= ~6e-5 Z
+      const double Z = (double)(v.n1 + 2) * (v.n2 + 2) * (v.n3 + 2);
+      const int jmax = (int)(Z * (3.0 * 2000.0 / (32.0 * 5300.0)) / (4.0 * g->sm_count));
+      const int chunks = (N + 1 + (jmax > 8 ? jmax : 8) - 1) / (jmax > 8 ? jmax : 8);
+      J = (N + 1 + chunks - 1) / chunks;
+    } else J = march_chunk(g, cols, N + 1);
     dim3 grid((unsigned)((cols + 127) / 128), (unsigned)((N + 1 + J - 1) / J));
     constexpr int D = (DIR == 1) ? 2 : DIR;   // (keeps the DIR == 1 instantiation of this branch well-formed)
     const size_t sm0 = MarchRing<0>::BYTES, sm1 = MarchRing<1>::BYTES;
     if (g->flat) {
-      if (mc) flux_march_kernel<D, 0, true><<<grid, 128, sm0, g->stream>>>(v, Ps, F, ct, J);
-      else flux_march_kernel<D, 1, true><<<grid, 128, sm1, g->stream>>>(v, Ps, F, ct, J);
+      if (mc) flux_march_kernel<D, 0, true><<<grid, 128, sm0, stream>>>(v, Ps, F, ct, J);
+      else flux_march_kernel<D, 1, true><<<grid, 128, sm1, stream>>>(v, Ps, F, ct, J);
     } else {
-      if (mc) flux_march_kernel<D, 0, false><<<grid, 128, sm0, g->stream>>>(v, Ps, F, ct, J);
-      else flux_march_kernel<D, 1, false><<<grid, 128, sm1, g->stream>>>(v, Ps, F, ct, J);
+      if (mc) flux_march_kernel<D, 0, false><<<grid, 128, sm0, stream>>>(v, Ps, F, ct, J);
+      else flux_march_kernel<D, 1, false><<<grid, 128, sm1, stream>>>(v, Ps, F, ct, J);
     }
   }
-  prof_end(g);
+  if (prof) prof_end(g);
   g->launches++;
 }
 
@@ -187,9 +235,25 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
   const GV& v = g->gv;
   reset_counters_kernel<<<1, 1, 0, g->stream>>>(g->sc, 0);
   g->launches++;
-  launch_flux<1>(g, Ps);
-  launch_flux<2>(g, Ps);
-  launch_flux<3>(g, Ps);
+  if (g->flux_concurrent) {
+    // fork: x2 and x3 on the side streams, x1 (many short blocks, launched last: it fills what the marching blocks leave free)
+    // on the grid's stream; join.  Profiling brackets the group as one entry (kind flux1), since the three overlap.
+    prof_begin(g, KH_K_FLUX1);
+    CK(cudaEventRecord(g->ev_fork, g->stream));
+    for (int s = 0; s < 2; s++) CK(cudaStreamWaitEvent(g->side[s], g->ev_fork, 0));
+    launch_flux<2>(g, Ps, g->side[0], false);
+    launch_flux<3>(g, Ps, g->side[1], false);
+    launch_flux<1>(g, Ps, g->stream, false);      // measured: x1 first costs 13 % of the step (its blocks then fill every slot)
+    for (int s = 0; s < 2; s++) {
+      CK(cudaEventRecord(g->ev_join[s], g->side[s]));
+      CK(cudaStreamWaitEvent(g->stream, g->ev_join[s], 0));
+    }
+    prof_end(g);
+  } else {
+    launch_flux<1>(g, Ps, g->stream, true);
+    launch_flux<2>(g, Ps, g->stream, true);
+    launch_flux<3>(g, Ps, g->stream, true);
+  }
   const int passes = g->p.fofc ? 2 : 1;       // FOFC: a speculative update first, then the re-flux, then the real one
   for (int pass = 0; pass < passes; pass++) {
     prof_begin(g, KH_K_EMF);
@@ -216,10 +280,16 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
       fb1 = Bff[0]; fb2 = Bff[1]; fb3 = Bff[2];
     }
     const unsigned grid = (unsigned)(((long)v.n1 * v.n2 * v.n3 + 127) / 128);
-#define UPD(FL, CO, IN)                                                                                                  \
-  update_kernel<FL, CO, IN><<<grid, 128, 0, g->stream>>>(v, Pi, Ps, Pf, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], \
-                                                         g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, g->fflag, g->faillist, g->sc, dt_factor, \
-                                                         fb1, fb2, fb3)
+    // persistent: as many blocks as stay resident (4 per SM), never more than there are groups of 4 warp tiles
+    const long tgroups = ((long)((v.n1 + 31) / 32) * v.n2 * v.n3 + 3) / 4;
+    const unsigned tgrid = (unsigned)(tgroups < 4L * g->sm_count ? tgroups : 4L * g->sm_count);
+#define UPD_ARGS v, Pi, Ps, Pf, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, \
+                 g->fflag, g->faillist, g->sc, dt_factor, fb1, fb2, fb3
+#define UPD(FL, CO, IN)                                                                                       \
+  do {                                                                                                        \
+    if (g->update_tma) update_tma_kernel<FL, CO, IN><<<tgrid, 128, tile_smem_bytes<FL, CO, IN>(), g->stream>>>(UPD_ARGS); \
+    else update_kernel<FL, CO, IN><<<grid, 128, 0, g->stream>>>(UPD_ARGS);                                   \
+  } while (0)
     prof_begin(g, KH_K_UPDATE);
 #define UPD2(FL, CO)                                                                 \
     switch (g->p.inverter + 2 * g->p.floor_frame + (fb1 ? 8 : 0)) {                  \
@@ -235,6 +305,7 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
 #undef UPD2
     prof_end(g);
 #undef UPD
+#undef UPD_ARGS
     g->launches++;
     CK(cudaGetLastError());
     if (pass + 1 < passes) {
@@ -279,10 +350,24 @@ static int ensure_stage(kh_grid* g) {
   return KH_OK;
 }
 
+// Every entry point runs on the grid's device, whatever device the calling thread had current.
+static int enter(kh_grid* g) {
+  int dev = -1;
+  CK(cudaGetDevice(&dev));
+  if (dev != g->device) CK(cudaSetDevice(g->device));
+  return KH_OK;
+}
+#define ENTER(g) do { int rc_ = enter(g); if (rc_) return rc_; } while (0)
+
 static void destroy_graphs(kh_grid* g) {
   for (int c = 0; c < 3; c++)
     if (g->gexec[c]) { cudaGraphExecDestroy(g->gexec[c]); g->gexec[c] = nullptr; }
 }
+
+// The zone arrays start ONE DOUBLE past the (256 B aligned) allocation: with 3 ghost zones per side, interior zone i = 0 of every
+// row then sits on a 16 B boundary whenever the padded row length is even, which is what the TMA bulk copies of
+// update_tma_kernel need (source address and size multiples of 16 B).
+static void free_shifted(double* p) { if (p) cudaFree(p - 1); }
 
 extern "C" {
 
@@ -303,13 +388,15 @@ int kh_grid_destroy(kh_grid* g) {
   destroy_graphs(g);
   for (int l = 0; l < 4; l++) cudaFree(g->geom[l]);
   cudaFree(g->conn); cudaFree(g->dg); cudaFree(g->floorp);
-  for (int b = 0; b < 3; b++) { cudaFree(g->P[b]); cudaFree(g->F[b]); cudaFree(g->ctop[b]); cudaFree(g->emf[b]); }
+  for (int b = 0; b < 3; b++) { free_shifted(g->P[b]); free_shifted(g->F[b]); free_shifted(g->ctop[b]); free_shifted(g->emf[b]); }
   cudaFree(g->pflag); cudaFree(g->fflag); cudaFree(g->mask);
-  for (int b = 0; b < 3; b++) for (int d = 0; d < 3; d++) cudaFree(g->Bf[b][d]);
+  for (int b = 0; b < 3; b++) for (int d = 0; d < 3; d++) free_shifted(g->Bf[b][d]);
   for (int d = 0; d < 4; d++) cudaFree(g->ecent[d]); cudaFree(g->faillist); cudaFree(g->sc); cudaFree(g->fix); cudaFree(g->stage);
   if (g->sc_host) cudaFreeHost(g->sc_host);
   if (g->pev) { for (int e = 0; e < 2 * KH_PROF_POOL; e++) if (g->pev[e]) cudaEventDestroy(g->pev[e]); delete[] g->pev; }
   delete[] g->pkind;
+  for (int s = 0; s < 2; s++) { if (g->side[s]) cudaStreamDestroy(g->side[s]); if (g->ev_join[s]) cudaEventDestroy(g->ev_join[s]); }
+  if (g->ev_fork) cudaEventDestroy(g->ev_fork);
   if (g->own_stream) cudaStreamDestroy(g->stream);
   delete g;
   return KH_OK;
@@ -346,9 +433,11 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
     g->own_stream = true;
   }
   g->flat = (p->coords == KH_MINKOWSKI);
+  for (int b = 0; b < 6; b++) g->has_fixed = g->has_fixed || p->bc[b] == KH_BC_FIXED;
   {
     int dev = 0;
     cudaGetDevice(&dev);
+    g->device = dev;
     cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev);
     setup_march_kernels();
     int nb = 0;
@@ -363,6 +452,25 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
     if (g->sm_count < 1) g->sm_count = 148;
   }
   g->use_graph = true;
+  g->flux_concurrent = true;
+  for (int s = 0; s < 2; s++) {
+    if (cudaStreamCreateWithFlags(&g->side[s], cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&g->ev_join[s], cudaEventDisableTiming) != cudaSuccess) { kh_grid_destroy(g); return KH_ECUDA; }
+  }
+  if (cudaEventCreateWithFlags(&g->ev_fork, cudaEventDisableTiming) != cudaSuccess) { kh_grid_destroy(g); return KH_ECUDA; }
+  g->update_tma = (p->n1 % 2 == 0);
+  if (const char* e = getenv("KH_UPDATE_TMA")) g->update_tma = g->update_tma && atoi(e) != 0;
+  if (g->update_tma) {
+    // the FOFC pass and the face-CT flag select the MODE at launch: set up every instantiation this grid can launch
+    for (int face = 0; face < 2; face++) {
+      if (face && p->transport != KH_B_FACE_CT) continue;
+      if (setup_update_tma(g->flat, p->inverter + 2 * p->floor_frame + (face ? 8 : 0)) != cudaSuccess) g->update_tma = false;
+    }
+    cudaGetLastError();
+  }
+  // A/B switches for measurements (profiles/): the defaults are the product path
+  if (const char* e = getenv("KH_FLUX_CONCURRENT")) g->flux_concurrent = atoi(e) != 0;
+  if (const char* e = getenv("KH_MARCH_J")) g->march_J = atoi(e);
   GV& v = g->gv;
   v.n1 = p->n1; v.n2 = p->n2; v.n3 = p->n3;
   v.nt1 = v.n1 + 2 * KH_NGH; v.nt2 = v.n2 + 2 * KH_NGH; v.nt3 = v.n3 + 2 * KH_NGH;
@@ -384,25 +492,32 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
     e_ = cudaMemsetAsync((ptr), 0, (bytes), g->stream);                         \
     if (e_ != cudaSuccess) { kh_grid_destroy(g); return KH_ECUDA; }             \
   } while (0)
+#define ALLOC_SHIFTED(ptr, bytes)                                               \
+  do {                                                                          \
+    double* raw_ = nullptr;                                                     \
+    ALLOC(raw_, (bytes) + 16);                                                  \
+    (ptr) = raw_ + 1;                                                           \
+  } while (0)
   const size_t fb = sizeof(double) * v.ntot;
   for (int l = 0; l < 4; l++) ALLOC(g->geom[l], sizeof(double) * KH_NGEO * v.n2d);
   ALLOC(g->conn, sizeof(double) * KH_NCONN * v.n2d);
   ALLOC(g->dg, sizeof(double) * KH_NDG * v.n2d);
   ALLOC(g->floorp, sizeof(double) * 2 * v.n2d);
   for (int b = 0; b < 3; b++) {
-    ALLOC(g->P[b], KH_NP * fb);
-    ALLOC(g->F[b], KH_NP * fb);
-    ALLOC(g->ctop[b], fb);
-    ALLOC(g->emf[b], fb);
+    ALLOC_SHIFTED(g->P[b], KH_NP * fb);
+    ALLOC_SHIFTED(g->F[b], KH_NP * fb);
+    ALLOC_SHIFTED(g->ctop[b], fb);
+    ALLOC_SHIFTED(g->emf[b], fb);
   }
   ALLOC(g->fix, 5 * fb);
   ALLOC(g->pflag, v.ntot);
   ALLOC(g->fflag, v.ntot);
   if (p->fofc) ALLOC(g->mask, v.ntot);
-  if (p->transport == KH_B_FACE_CT) for (int b = 0; b < 3; b++) for (int d = 0; d < 3; d++) ALLOC(g->Bf[b][d], fb);
+  if (p->transport == KH_B_FACE_CT) for (int b = 0; b < 3; b++) for (int d = 0; d < 3; d++) ALLOC_SHIFTED(g->Bf[b][d], fb);
   if (p->emf == KH_EMF_UPWIND) for (int d = 0; d < 4; d++) ALLOC(g->ecent[d], fb);
   ALLOC(g->faillist, sizeof(unsigned) * (size_t)v.n1 * v.n2 * v.n3);
   ALLOC(g->sc, sizeof(StepScalars));
+#undef ALLOC_SHIFTED
 #undef ALLOC
   if (cudaMallocHost((void**)&g->sc_host, sizeof(StepScalars)) != cudaSuccess) { kh_grid_destroy(g); return KH_ENOMEM; }
   memset(g->sc_host, 0, sizeof(StepScalars));
@@ -436,6 +551,8 @@ static int xfer(kh_grid* g, void* dst, const void* src, size_t bytes, int mem, b
 
 int kh_set_prims(kh_grid* g, const double* p, int with_ghosts, int mem) {
   if (!g || !p || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  if (g->has_fixed && !with_ghosts && !g->fixed_ghosts_set) return KH_EINVAL;   // FIXED ghosts come from a with_ghosts = 1 load
+  ENTER(g);
   const GV& v = g->gv;
   double* Pn = g->P[g->cur];
   int rc;
@@ -444,6 +561,7 @@ int kh_set_prims(kh_grid* g, const double* p, int with_ghosts, int mem) {
     if (rc) return rc;
     // FIXED ghosts must exist in every rotating buffer
     for (int b = 1; b < 3; b++) CK(cudaMemcpyAsync(g->P[(g->cur + b) % 3], Pn, sizeof(double) * KH_NP * v.ntot, cudaMemcpyDeviceToDevice, g->stream));
+    g->fixed_ghosts_set = true;
   } else {
     size_t bytes = sizeof(double) * KH_NP * (size_t)v.n1 * v.n2 * v.n3;
     const double* src = p;
@@ -458,6 +576,13 @@ int kh_set_prims(kh_grid* g, const double* p, int with_ghosts, int mem) {
     g->launches++;
     CK(cudaGetLastError());
   }
+  if (g->p.transport == KH_B_FACE_CT && g->faces_set) {
+    // the face field is the magnetic state: the zone-centred B of the new primitives is slaved to it again
+    double* const* B = g->Bf[g->cur];
+    face_to_cent_kernel<<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, B[0], B[1], B[2], Pn, g->flat ? 1 : 0);
+    g->launches++;
+    CK(cudaGetLastError());
+  }
   rc = fill_ghosts(g, Pn, nullptr);
   if (rc) return rc;
   if (mem == KH_MEM_HOST) CK(cudaStreamSynchronize(g->stream));
@@ -466,6 +591,7 @@ int kh_set_prims(kh_grid* g, const double* p, int with_ghosts, int mem) {
 
 int kh_get_prims(kh_grid* g, double* p, int with_ghosts, int mem) {
   if (!g || !p || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  ENTER(g);
   const GV& v = g->gv;
   if (with_ghosts) return xfer(g, p, g->P[g->cur], sizeof(double) * KH_NP * v.ntot, mem, true);
   size_t bytes = sizeof(double) * KH_NP * (size_t)v.n1 * v.n2 * v.n3;
@@ -480,6 +606,7 @@ int kh_get_prims(kh_grid* g, double* p, int with_ghosts, int mem) {
 
 int kh_get_cons(kh_grid* g, double* u, int mem) {
   if (!g || !u || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  ENTER(g);
   const GV& v = g->gv;
   size_t bytes = sizeof(double) * KH_NP * (size_t)v.n1 * v.n2 * v.n3;
   if (mem == KH_MEM_HOST) { int rc = ensure_stage(g); if (rc) return rc; }
@@ -494,6 +621,7 @@ int kh_get_cons(kh_grid* g, double* u, int mem) {
 
 int kh_get_flags(kh_grid* g, int* pflag, int* fflag, int mem) {
   if (!g || (mem != KH_MEM_DEVICE && mem != KH_MEM_HOST)) return KH_EINVAL;
+  ENTER(g);
   const GV& v = g->gv;
   size_t nin = (size_t)v.n1 * v.n2 * v.n3;
   int* outs[2] = {pflag, fflag};
@@ -518,6 +646,7 @@ static int read_scalars(kh_grid* g) {
 
 int kh_estimate_dt(kh_grid* g, double* dt) {
   if (!g || !dt) return KH_EINVAL;
+  ENTER(g);
   const GV& v = g->gv;
   if (g->flat) estimate_dt_kernel<true><<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, g->P[g->cur], g->sc);
   else estimate_dt_kernel<false><<<zone_grid(v.n1, v.n2, v.n3), 128, 0, g->stream>>>(v, g->P[g->cur], g->sc);
@@ -529,50 +658,85 @@ int kh_estimate_dt(kh_grid* g, double* dt) {
   memcpy(&rate, &g->sc_host->rate_bits, sizeof(double));
   CK(cudaMemsetAsync(&g->sc->rate_bits, 0, sizeof(unsigned long long), g->stream));
   CK(cudaStreamSynchronize(g->stream));
-  if (!(rate == rate)) return KH_ENAN;
+  if (g->sc_host->nonfinite) {               // a non-finite wave speed (fmax would have dropped it from the maximum)
+    CK(cudaMemsetAsync(&g->sc->nonfinite, 0, sizeof(unsigned long long), g->stream));
+    return KH_ENAN;
+  }
+  if (!(rate > 0.0)) return KH_ENAN;
   *dt = g->p.cfl * (1.0 / rate);            // min over zones of 1/rate = 1/max rate
   return KH_OK;
 }
 
 int kh_step(kh_grid* g, double dt, double* dt_next) {
-  if (g && g->p.transport == KH_B_FACE_CT && !g->faces_set) return KH_EINVAL;   // the face field is the magnetic state: set it first
-
   if (!g || dt != dt) return KH_EINVAL;
+  if (g->p.transport == KH_B_FACE_CT && !g->faces_set) return KH_EINVAL;   // the face field is the magnetic state: set it first
+  if (g->has_fixed && !g->fixed_ghosts_set) return KH_EINVAL;               // FIXED ghost layers were never supplied
+  if (!(dt > 0.0) && !g->have_dt_next) return KH_EINVAL;                    // no dt_next on the device yet
+  ENTER(g);
   set_dt_kernel<<<1, 1, 0, g->stream>>>(g->sc, dt, dt > 0.0 ? 0 : 1);
   g->launches++;
   CK(cudaGetLastError());
   int cur = g->cur;
+  bool replayed = false;
   if (g->use_graph && !g->profile) {
     if (!g->gexec[cur]) {
-      long long before = g->launches;
-      cudaGraph_t graph;
-      CK(cudaStreamBeginCapture(g->stream, cudaStreamCaptureModeThreadLocal));
-      int rc = enqueue_step(g, cur);
-      cudaError_t e = cudaStreamEndCapture(g->stream, &graph);
-      if (rc) return rc;
-      CK(e);
-      g->graph_launches = g->launches - before;
-      g->launches = before;
-      CK(cudaGraphInstantiate(&g->gexec[cur], graph, 0));
-      cudaGraphDestroy(graph);
+      // Capture one step.  Any failure (a stream that cannot be captured, a capture already active on it, ...) switches
+      // this grid to direct launches for good: the same kernels, enqueued one by one.
+      const long long before = g->launches;
+      cudaGraph_t graph = nullptr;
+      cudaError_t e = cudaStreamBeginCapture(g->stream, cudaStreamCaptureModeThreadLocal);
+      int rc = KH_OK;
+      if (e == cudaSuccess) {
+        rc = enqueue_step(g, cur);
+        e = cudaStreamEndCapture(g->stream, &graph);
+        g->graph_launches = g->launches - before;
+        g->launches = before;
+        if (e == cudaSuccess && rc == KH_OK) e = cudaGraphInstantiate(&g->gexec[cur], graph, 0);
+        if (graph) cudaGraphDestroy(graph);
+      }
+      if (e != cudaSuccess || rc != KH_OK) {
+        cudaGetLastError();
+        if (g->gexec[cur]) { cudaGraphExecDestroy(g->gexec[cur]); g->gexec[cur] = nullptr; }
+        g->use_graph = false;
+      }
     }
-    CK(cudaGraphLaunch(g->gexec[cur], g->stream));
-    g->launches += g->graph_launches;
-  } else {
+    if (g->gexec[cur]) {
+      CK(cudaGraphLaunch(g->gexec[cur], g->stream));
+      g->launches += g->graph_launches;
+      replayed = true;
+    }
+  }
+  if (!replayed) {
     int rc = enqueue_step(g, cur);
     if (rc) return rc;
   }
   g->cur = (cur + 2) % 3;
+  g->have_dt_next = true;
   if (dt_next) {
     int rc = read_scalars(g);
     if (rc) return rc;
+    if (g->sc_host->nonfinite || !(g->sc_host->dt_next == g->sc_host->dt_next)) return KH_ENAN;   // a non-finite wave speed reached the CFL reduction
     *dt_next = g->sc_host->dt_next;
   }
   return KH_OK;
 }
 
+int kh_get_stream(kh_grid* g, void** cuda_stream) {
+  if (!g || !cuda_stream) return KH_EINVAL;
+  *cuda_stream = (void*)g->stream;
+  return KH_OK;
+}
+
+int kh_sync(kh_grid* g) {
+  if (!g) return KH_EINVAL;
+  ENTER(g);
+  CK(cudaStreamSynchronize(g->stream));
+  return KH_OK;
+}
+
 int kh_divB(kh_grid* g, double* max_abs) {
   if (!g || !max_abs) return KH_EINVAL;
+  ENTER(g);
   const GV& v = g->gv;
   int lo[3], cnt[3];
   const int N[3] = {v.n1, v.n2, v.n3};
@@ -639,6 +803,7 @@ int kh_divB_face(kh_grid* g, double* max_abs) {
 
 int kh_count_flags(kh_grid* g, long long* n_pflag, long long* n_fflag) {
   if (!g) return KH_EINVAL;
+  ENTER(g);
   int rc = read_scalars(g);
   if (rc) return rc;
   if (n_pflag) *n_pflag = (long long)g->sc_host->n_pflag;

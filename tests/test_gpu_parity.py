@@ -75,7 +75,20 @@ def test_ghost_fills_bit_exact(kh, kho):
     for p in cases:
         shp = (8, p["n3"], p["n2"], p["n1"])
         P0 = rng.normal(size=shp)
-        gg, go = _both(kh, kho, p, P0)
+        if kp.BC_FIXED in p["bc"]:
+            # a FIXED side needs its ghost layers from a with_ghosts load first: until then the library refuses
+            # (the fixed layers would silently be vacuum)
+            gg, go = kh.Grid(p), kho.Grid(p, omp=True)
+            with pytest.raises(kh.KharmError):
+                gg.set_prims(P0)
+            with pytest.raises(kh.KharmError):
+                gg.step(1e-3)
+            first = rng.normal(size=(8, p["n3"] + 6, p["n2"] + 6, p["n1"] + 6))
+            for g in (gg, go):
+                g.set_prims(first, with_ghosts=True)
+                g.set_prims(P0)
+        else:
+            gg, go = _both(kh, kho, p, P0)
         a, b = gg.get_prims(with_ghosts=True), go.get_prims(with_ghosts=True)
         # outflow ghosts rescale B by a ratio of tabulated sqrt(-g): identical up to the tables' own rounding
         assert np.array_equal(a[:5], b[:5])
