@@ -354,6 +354,70 @@ emf_upwind_kernel(GV g, const double* __restrict__ F1, const double* __restrict_
 // ~50 fp64 instructions instead of the 40-entry Gamma table and a 64-term contraction.
 // One thread per interior zone, flattened index (no idle lanes when n1 is not a multiple of the block).
 // ---------------------------------------------------------------------------------------------
+enum { KH_MAP_ID = 0, KH_MAP_COPY = 1, KH_MAP_OUTFLOW = 2, KH_MAP_POLAR = 3 };
+
+// index gi in [-NG, N+NG) along one direction -> source index and the kind of the map
+__device__ __forceinline__ int ghost_map(int gi, int N, int bc_lo, int bc_hi, int& kind) {
+  kind = KH_MAP_ID;
+  if (gi >= 0 && gi < N) return gi;
+  const int side = gi >= N;
+  const int bc = side ? bc_hi : bc_lo;
+  if (bc == 3) return gi;                                   // fixed: the ghost keeps its content
+  if (bc == 0) {                                            // periodic wrap (a block thinner than the ghost layer wraps more than once)
+    kind = KH_MAP_COPY;
+    return N >= KH_NGH ? (side ? gi - N : gi + N) : ((gi % N) + N) % N;
+  }
+  if (bc == 1) { kind = KH_MAP_OUTFLOW; return side ? N - 1 : 0; }
+  kind = KH_MAP_POLAR;
+  return side ? 2 * N - 1 - gi : -1 - gi;                   // ghost -1-m <- m ; ghost N+m <- N-1-m
+}
+
+// candidate q = 0 .. 2 NG - 1: the ghost indices of one direction, q = 2 NG: the zone's own index s.  Returns false if
+// ghost q is not an image of s.
+__device__ __forceinline__ bool image_candidate(int q, int s, int N, int bc_lo, int bc_hi, int& idx, int& kind) {
+  if (q == 2 * KH_NGH) { idx = s; kind = KH_MAP_ID; return true; }
+  idx = q < KH_NGH ? q - KH_NGH : N + q - KH_NGH;
+  return ghost_map(idx, N, bc_lo, bc_hi, kind) == s && kind != KH_MAP_ID;
+}
+template <int NV>
+__device__ __forceinline__ void store_ghost_images(const GV& g, double* __restrict__ P, unsigned char* __restrict__ flag, int i, int j, int k,
+                                                   const double pf[KH_NP], int flagval) {
+  if (i >= KH_NGH && i < g.n1 - KH_NGH && j >= KH_NGH && j < g.n2 - KH_NGH && k >= KH_NGH && k < g.n3 - KH_NGH) return;
+  const long nt = g.ntot;
+  const double* gd = g.geom[0] + 20 * g.n2d;
+#pragma unroll 1
+  for (int qz = 0; qz <= 2 * KH_NGH; qz++) {
+    int c, k3;
+    if (!image_candidate(qz, k, g.n3, g.bc[4], g.bc[5], c, k3)) continue;
+#pragma unroll 1
+    for (int qy = 0; qy <= 2 * KH_NGH; qy++) {
+      int b, k2;
+      if (!image_candidate(qy, j, g.n2, g.bc[2], g.bc[3], b, k2)) continue;
+#pragma unroll 1
+      for (int qx = 0; qx <= 2 * KH_NGH; qx++) {
+        int a, k1;
+        if (!image_candidate(qx, i, g.n1, g.bc[0], g.bc[1], a, k1)) continue;
+        if (qx + qy + qz == 3 * 2 * KH_NGH) continue;                 // the zone itself: stored by the caller
+        double r1 = 1.0, r2 = 1.0;
+        if (NV > 5) {
+          if (k1 == KH_MAP_OUTFLOW) r1 = __ldg(gd + pidx(g, i, j)) / __ldg(gd + pidx(g, a, j));     // pass 1 acts on row j
+          if (k2 == KH_MAP_OUTFLOW) r2 = __ldg(gd + pidx(g, a, j)) / __ldg(gd + pidx(g, a, b));     // pass 2 acts on column a
+        }
+        const long m = zidx(g, a, b, c);
+#pragma unroll
+        for (int v = 0; v < NV; v++) {
+          double val = pf[v];
+          if (v >= B1) { if (k1 == KH_MAP_OUTFLOW) val *= r1; }
+          if (k2 == KH_MAP_POLAR && (v == U2 || v == B2)) val = -val;
+          if (v >= B1) { if (k2 == KH_MAP_OUTFLOW) val *= r2; }
+          P[v * nt + m] = val;
+        }
+        if (NV > 5) flag[m] = (unsigned char)flagval;
+      }
+    }
+  }
+}
+
 // MODE = inverter (bit 0: 0 1D_W, 1 Kastaun) + 2 * floor frame (0 fluid, 1 drift, 2 normal observer) + 8 if the zone-centred
 // field comes from the face field (face-centred CT)
 //
@@ -509,8 +573,8 @@ __device__ __forceinline__ bool rate_nonfinite(double r) { return ((unsigned)__d
 
 // Phase B: inversion + floors of the advanced state, stores.  Pi: the guess (global memory; read only by the rare failed zone).
 template <bool FLAT, int MODE>
-__device__ __forceinline__ void update_zone_b(const GV& g, const Geo& G, const double Uh[KH_NP], double W0, long n, long p2,
-                                              const double* __restrict__ Pi, double* __restrict__ Pf, unsigned char* __restrict__ pflag,
+__device__ __forceinline__ void update_zone_b(const GV& g, const Geo& G, const double Uh[KH_NP], double W0, int i, int j, int k, long n,
+                                              long p2, const double* __restrict__ Pi, double* __restrict__ Pf, unsigned char* __restrict__ pflag,
                                               unsigned char* __restrict__ fflag, unsigned* __restrict__ faillist,
                                               StepScalars* __restrict__ sc, int& pf_flag, int& ff) {
   const long nt = g.ntot;
@@ -588,7 +652,7 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
     double Uh[KH_NP], W0;
     update_zone_a<FLAT, CORR, MODE>(g, A, G, p2, Dt, Uh, W0, rate);
     if (CORR && rate_nonfinite(rate)) { sc->nonfinite = 1ULL; rate = 0.0; }
-    update_zone_b<FLAT, MODE>(g, G, Uh, W0, n, p2, Pi, Pf, pflag, fflag, faillist, sc, pf_flag, ff);
+    update_zone_b<FLAT, MODE>(g, G, Uh, W0, i, j, k, n, p2, Pi, Pf, pflag, fflag, faillist, sc, pf_flag, ff);
   }
   update_block_tail<CORR>(sc, rate, ff);
 }
@@ -735,6 +799,7 @@ update_tma_kernel(GV g, const double* __restrict__ Pi, const double* __restrict_
       update_zone_a<FLAT, CORR, MODE>(g, A, G, p2, Dt, Uh, W0, r);
     }
     __syncwarp();                                       // every lane has read its part of the tile
+    const int jz = j, kz = k;
     T += stride;
     if (T < ntiles) {
       tile_origin(T, i0, j, k);
@@ -745,7 +810,7 @@ update_tma_kernel(GV g, const double* __restrict__ Pi, const double* __restrict_
     }
     if (active) {
       int pf_flag, ff;
-      update_zone_b<FLAT, MODE>(g, G, Uh, W0, n0 + lane, p2, Pi, Pf, pflag, fflag, faillist, sc, pf_flag, ff);
+      update_zone_b<FLAT, MODE>(g, G, Uh, W0, i, jz, kz, n0 + lane, p2, Pi, Pf, pflag, fflag, faillist, sc, pf_flag, ff);
       nff += (ff != 0);
       if (CORR) { if (rate_nonfinite(r)) sc->nonfinite = 1ULL; else rate = fmax(rate, r); }
     }
@@ -782,21 +847,6 @@ __global__ void reset_counters_kernel(StepScalars* sc, int also_rate) {
 // direction maps below, value transforms applied in pass order (outflow: B rescaled by the ratio of tabulated
 // sqrt(-g), S20b; polar: sign of ut^2, B^2).  One launch, bit-identical to the three passes.
 // ---------------------------------------------------------------------------------------------
-enum { KH_MAP_ID = 0, KH_MAP_COPY = 1, KH_MAP_OUTFLOW = 2, KH_MAP_POLAR = 3 };
-
-// index gi in [-NG, N+NG) along one direction -> source index and the kind of the map
-__device__ __forceinline__ int ghost_map(int gi, int N, int bc_lo, int bc_hi, int& kind) {
-  kind = KH_MAP_ID;
-  if (gi >= 0 && gi < N) return gi;
-  const int side = gi >= N;
-  const int bc = side ? bc_hi : bc_lo;
-  if (bc == 3) return gi;                                   // fixed: the ghost keeps its content
-  if (bc == 0) { kind = KH_MAP_COPY; return ((gi % N) + N) % N; }
-  if (bc == 1) { kind = KH_MAP_OUTFLOW; return side ? N - 1 : 0; }
-  kind = KH_MAP_POLAR;
-  return side ? 2 * N - 1 - gi : -1 - gi;                   // ghost -1-m <- m ; ghost N+m <- N-1-m
-}
-
 __global__ void __launch_bounds__(128)
 fill_kernel(GV g, double* __restrict__ P, unsigned char* __restrict__ flag) {
   // ghost shell = slab A (k ghost, all i, j) + slab B (j ghost, k interior, all i) + slab C (i ghost, j, k interior)
@@ -893,16 +943,6 @@ fixup_gather_kernel(GV g, const double* __restrict__ Pf, const unsigned char* __
   }
 }
 
-// ghost images of interior index s along one direction: writes up to 2*NG indices into img[], returns how many
-__device__ __forceinline__ int ghost_images(int s, int N, int bc_lo, int bc_hi, int img[2 * KH_NGH]) {
-  int cnt = 0;
-  for (int m = 0; m < 2 * KH_NGH; m++) {
-    int gi = m < KH_NGH ? m - KH_NGH : N + m - KH_NGH, kind;
-    if (ghost_map(gi, N, bc_lo, bc_hi, kind) == s && kind != KH_MAP_ID) img[cnt++] = gi;
-  }
-  return cnt;
-}
-
 template <bool FLAT>
 __global__ void __launch_bounds__(128)
 fixup_apply_kernel(GV g, double* __restrict__ Pf, const unsigned* __restrict__ list, unsigned char* __restrict__ fflag,
@@ -950,21 +990,9 @@ fixup_apply_kernel(GV g, double* __restrict__ Pf, const unsigned* __restrict__ l
     }
     fflag[n] |= (unsigned char)ff;
     // the zone and its ghost images (S20: copies; polar images flip ut^2)
-    int i1[2 * KH_NGH + 1], i2[2 * KH_NGH + 1], i3[2 * KH_NGH + 1];
-    int c1 = ghost_images(i, g.n1, g.bc[0], g.bc[1], i1), c2 = ghost_images(j, g.n2, g.bc[2], g.bc[3], i2),
-        c3 = ghost_images(k, g.n3, g.bc[4], g.bc[5], i3);
-    i1[c1++] = i; i2[c2++] = j; i3[c3++] = k;
-    for (int z = 0; z < c3; z++)
-      for (int y = 0; y < c2; y++) {
-        int kind;
-        ghost_map(i2[y], g.n2, g.bc[2], g.bc[3], kind);
-        const double sgn = (kind == KH_MAP_POLAR) ? -1.0 : 1.0;
-        for (int x = 0; x < c1; x++) {
-          const long m = zidx(g, i1[x], i2[y], i3[z]);
 #pragma unroll
-          for (int v = 0; v < 5; v++) Pf[v * nt + m] = (v == U2) ? sgn * P[v] : P[v];
-        }
-      }
+    for (int v = 0; v < 5; v++) Pf[v * nt + n] = P[v];
+    store_ghost_images<5>(g, Pf, nullptr, i, j, k, P, 0);
   }
 }
 

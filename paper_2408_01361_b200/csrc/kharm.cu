@@ -559,8 +559,6 @@ int kh_set_prims(kh_grid* g, const double* p, int with_ghosts, int mem) {
   if (with_ghosts) {
     rc = xfer(g, Pn, p, sizeof(double) * KH_NP * v.ntot, mem, false);
     if (rc) return rc;
-    // FIXED ghosts must exist in every rotating buffer
-    for (int b = 1; b < 3; b++) CK(cudaMemcpyAsync(g->P[(g->cur + b) % 3], Pn, sizeof(double) * KH_NP * v.ntot, cudaMemcpyDeviceToDevice, g->stream));
     g->fixed_ghosts_set = true;
   } else {
     size_t bytes = sizeof(double) * KH_NP * (size_t)v.n1 * v.n2 * v.n3;
@@ -585,6 +583,11 @@ int kh_set_prims(kh_grid* g, const double* p, int with_ghosts, int mem) {
   }
   rc = fill_ghosts(g, Pn, nullptr);
   if (rc) return rc;
+  if (with_ghosts && g->has_fixed) {
+    // FIXED ghost layers, and the ghost zones filled FROM them (edges and corners shared with another boundary), must exist in
+    // every rotating buffer: during a step only the images of interior zones are rewritten
+    for (int b = 1; b < 3; b++) CK(cudaMemcpyAsync(g->P[(g->cur + b) % 3], Pn, sizeof(double) * KH_NP * v.ntot, cudaMemcpyDeviceToDevice, g->stream));
+  }
   if (mem == KH_MEM_HOST) CK(cudaStreamSynchronize(g->stream));
   return KH_OK;
 }
