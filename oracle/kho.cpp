@@ -483,8 +483,8 @@ int u2p(const Geom& G, const double U[NP], const double Pg[NP], double gam, doub
 }
 
 // ---------------------------------------------------------------------------------------------
-// C7b. U -> P by the bracketed root find of Kastaun, Kalinani & Ciolfi ("the inverter
-// described in [25] ... greatly improves stability"; reading S24 in DESIGN.md).  Written in the
+// C7b. U -> P by the bracketed root find of Kastaun, Kalinani & Ciolfi ("the robust primitive
+// variable recovery of [27], which greatly improves stability"; reading S24 in DESIGN.md).  Written in the
 // paper's notation.  Inputs seen by the normal observer (same as in u2p above): D, tau = E - D, S_i, B^i;
 //   q = tau/D,  r_i = S_i/D,  b^i = B^i/sqrt(D),  h0 = 1 (ideal gas, eps >= 0),  v0^2 = r^2/(h0^2 + r^2);
 // functions of the unknown mu = 1/(W h):
@@ -1424,6 +1424,23 @@ void kho_source(const double gcov[16], const double gcon[16], double gdet, const
   Geom G; make_geom(gcov, gcon, gdet, G);
   source(G, conn, P, gamma, S);
 }
+// Test hook (tests/test_oracle_forms.py): the norm Qt^2 of the projected momentum exactly as u2p() forms it, from the
+// covariant components Q_mu it receives (no arithmetic of its own: the lines below are u2p()'s).
+double kho_qtsq(const double gcov16[16], const double gcon16[16], double alpha, const double Qcov[4]) {
+  double gcov[4][4], gcon[4][4];
+  unpack(gcov16, gcov); unpack(gcon16, gcon);
+  double Qcon[4];
+  for (int m = 0; m < 4; m++) { double s = 0.0; for (int n = 0; n < 4; n++) s += gcon[m][n] * Qcov[n]; Qcon[m] = s; }
+  double Qdotn = -alpha * Qcon[0];
+  double ncon[4];
+  for (int m = 0; m < 4; m++) ncon[m] = -alpha * gcon[m][0];
+  double Qtcon[4];
+  for (int m = 0; m < 4; m++) Qtcon[m] = Qcon[m] + Qdotn * ncon[m];
+  double Qtsq = 0.0;
+  for (int i = 1; i < 4; i++) for (int j = 1; j < 4; j++) Qtsq += gcov[i][j] * Qtcon[i] * Qtcon[j];
+  return Qtsq;
+}
+
 int kho_u2p(const double gcov[16], const double gcon[16], double gdet, const double U[8], const double Pguess[8], double gamma, double Pout[8]) {
   Geom G; make_geom(gcov, gcon, gdet, G);
   return u2p(G, U, Pguess, gamma, Pout);

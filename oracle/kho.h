@@ -109,6 +109,8 @@ void kho_llf(const double gcov[16], const double gcon[16], double gdet, const do
              const double PR[8], double gamma, int dir, double F[8], double* ctop);
 void kho_source(const double gcov[16], const double gcon[16], double gdet, const double conn[64],
                 const double P[8], double gamma, double S[8]);
+/* Test hook: Qt^2 = g_ij Qt^i Qt^j of the projected momentum exactly as kho_u2p forms it from the covariant Q_mu (DESIGN S16) */
+double kho_qtsq(const double gcov[16], const double gcon[16], double alpha, const double Qcov[4]);
 /* U -> P (1D_W); returns the flag (0 = ok). Pout holds guess hydro prims on failure. */
 int kho_u2p(const double gcov[16], const double gcon[16], double gdet, const double U[8],
             const double Pguess[8], double gamma, double Pout[8]);

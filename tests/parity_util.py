@@ -48,6 +48,27 @@ def conditioning(p, ref, gamma):
     return EPS * (ref[0] + b2) / ref[1]
 
 
+def oracle_sensitivity(kho, p, P0, faces, dts, realizations=5, seed=100):
+    """What 1-ulp noise on the INPUT does to the oracle's own result (S23c): the oracle is run on P0 (1 +- 2^-52)
+    with seeded random signs, for the same steps dts, and the per-zone, per-primitive difference to its unperturbed result
+    (S23 metric, maximum over the realisations) is returned, [8][n3][n2][n1].  It measures, from the oracle alone, how much
+    the step amplifies round-off in each zone -- the scale on which two correct fp64 evaluations of the scheme can differ."""
+    def run(P):
+        g = kho.Grid(p, omp=True)
+        g.set_prims(P)
+        if faces is not None:
+            g.set_face_B(*faces)
+        for dt in dts:
+            g.step(dt)
+        return g.get_prims()
+    ref = run(P0)
+    worst = np.zeros_like(ref)
+    for r in range(realizations):
+        rng = np.random.default_rng(seed + r)
+        worst = np.maximum(worst, rel_diff(p, run(P0 * (1.0 + 2.0 ** -52 * rng.choice([-1.0, 1.0], size=P0.shape))), ref))
+    return worst
+
+
 def l1_diff(p, got, ref):
     """L1 difference per primitive: sum|d| / sum|ref| for rho, u; for the vector components the denominator
     is the sum of the vector's norm (sum sqrt(g_ii)|d v^i| / sum |v|), so that a component that vanishes by

@@ -2,6 +2,8 @@
 seeded inputs.  Bars (BASELINE.json north_star): max relative difference 1e-10 per primitive after one
 step (metric: tests/parity_util.py, DESIGN.md S23), 1e-8 in L1 after a run, identical U->P flags;
 index / copy work (ghost fills) bit-exact."""
+import os
+
 import numpy as np
 import pytest
 
@@ -9,7 +11,7 @@ import kharm_inputs as ki
 from kharm_inputs import bondi, modes, torus
 from kharm_inputs import params as kp
 
-from parity_util import TOL_ONE_STEP, TOL_RUN_L1, conditioning, l1_diff, rel_diff
+from parity_util import TOL_ONE_STEP, TOL_RUN_L1, conditioning, l1_diff, oracle_sensitivity, rel_diff
 
 pytestmark = pytest.mark.gpu
 
@@ -31,16 +33,51 @@ def _both(kh, kho, p, P0, with_ghosts=False, omp=True):
     return gg, go
 
 
-def _assert_step_parity(p, got, ref, pf_g, pf_o, label="", tol=TOL_ONE_STEP):
+# Allowance of the one-step bar in zones where the scheme itself amplifies round-off (S23): the two sides evaluate
+# algebraically identical formulas in different association and contraction, so each of the ~30 rounded operations that
+# feed a zone's energy equation (7 face-flux components, source and U(P_i) per sub-step, the inversion's residual) may
+# differ by an ulp of its own operand; K_ROUNDINGS of them, amplified by the zone's conditioning number eps (rho + b^2) / u,
+# is the bar on u there.  S23c (fuzz cases): where the oracle itself turns 1-ulp input noise into more than a tenth of the
+# bar (parity_util.oracle_sensitivity), K_SENS times that measured sensitivity is the bar -- for any primitive.
+K_ROUNDINGS = 30.0
+K_SENS = 10.0
+MAX_RELAXED_FRACTION = 0.5      # no test may judge more than half of its zones on a relaxed bar (asserted)
+
+
+def _report(label, worst, relaxed, zones, tol):
+    """Append one row to the parity report (KH_PARITY_REPORT=<path>.md; profiles/parity_r02.md is such a file)."""
+    path = os.environ.get("KH_PARITY_REPORT")
+    if not path:
+        return
+    new = not os.path.exists(path)
+    with open(path, "a") as f:
+        if new:
+            f.write("| case | zones | bar | worst rho | worst u | worst ut1 | worst ut2 | worst ut3 | worst B1 | worst B2 | worst B3 |"
+                    " zones on a relaxed bar: rho | u | ut |\n|" + "---|" * 14 + "\n")
+        f.write("| %s | %d | %.0e | %s | %d | %d | %d |\n" % (label, zones, tol, " | ".join("%.2e" % w for w in worst),
+                                                             relaxed[0], relaxed[1], relaxed[2]))
+
+
+def _assert_step_parity(p, got, ref, pf_g, pf_o, label="", tol=TOL_ONE_STEP, sens=None):
+    """S23: per-zone, per-primitive relative difference <= tol, flags identical.  Relaxed bars:
+      u             : K_ROUNDINGS eps (rho + b^2) / u, the conditioning of the internal energy in U -> P (S16); u ONLY --
+                      rho, ut^i and B^i stay on the flat bar;
+      any primitive : K_SENS x the oracle's measured sensitivity to 1-ulp input noise, where `sens` is given (S23c).
+    Returns the worst difference per primitive; the number of zones judged on a relaxed bar is bounded and reported."""
     assert np.array_equal(pf_g, pf_o), "%s: U->P flags differ in %d zones" % (label, (pf_g != pf_o).sum())
     d = rel_diff(p, got, ref)
-    # zones whose internal energy is ill-conditioned by the scheme itself (eps (rho+b^2)/u > 1e-11) are
-    # judged against that conditioning instead of the flat bar -- reported, not hidden (S16/S23)
-    cond = conditioning(p, ref, p["gamma"])
-    allow = np.maximum(tol, 30.0 * cond)
+    allow = np.full(d.shape, tol)
+    allow[1] = np.maximum(tol, K_ROUNDINGS * conditioning(p, ref, p["gamma"]))
+    if sens is not None:
+        allow = np.maximum(allow, K_SENS * sens)
     worst = d.max(axis=(1, 2, 3))
-    bad = d > allow[None]
-    assert not bad.any(), "%s: max rel diff per primitive %s (bar %g); %d zones over" % (label, worst, tol, bad.sum())
+    bad = d > allow
+    zones = d[0].size
+    relaxed = [int((allow[0] > tol).sum()), int((allow[1] > tol).sum()), int((allow[2:5] > tol).any(axis=0).sum())]
+    _report(label, worst, relaxed, zones, tol)
+    assert not bad.any(), "%s: max rel diff per primitive %s (bar %g); %d zones over; worst excess %s" % (
+        label, worst, tol, bad.any(axis=0).sum(), (d / allow).max(axis=(1, 2, 3)))
+    assert max(relaxed) <= MAX_RELAXED_FRACTION * zones, "%s: %s of %d zones judged on a relaxed bar" % (label, relaxed, zones)
     return worst
 
 
@@ -651,11 +688,8 @@ def test_cuda_path_linear_mode_convergence(kh, rotated, recon):
 
 
 # ------------------------------------------------------------------------------------------ seeded fuzz over sizes, boundaries and options
-@pytest.mark.parametrize("seed", list(range(int(__import__("os").environ.get("KH_FUZZ_SEEDS", "48")))))
-def test_fuzz_one_step_random_configurations(kh, kho, seed):
-    """Random small blocks: ragged sizes (down to 3 zones), every boundary kind that is legal for the coordinate system,
-    and random choices of reconstruction, inverter, floor frame, FOFC, transport and EMF kind.  One step (plus one more
-    for the odd seeds), the usual bars."""
+def _fuzz_case(seed):
+    """Seeded random block of the fuzz test: (params, primitives, face field or None, options, label)."""
     from kharm_inputs import facefield
     rng = np.random.default_rng(1000 + seed)
     curved = seed % 2 == 0
@@ -692,9 +726,7 @@ def test_fuzz_one_step_random_configurations(kh, kho, seed):
     opts = dict(recon=int(rng.integers(0, 2)), inverter=int(rng.integers(0, 2)), floor_frame=int(rng.integers(0, 3)),
                 fofc=int(rng.integers(0, 2)), transport=int(rng.integers(0, 2)), emf=int(rng.integers(0, 2)))
     p = dict(p, **opts)
-    gg, go = kh.Grid(p), kho.Grid(p, omp=True)
-    for g in (gg, go):
-        g.set_prims(P0)
+    faces = None
     if opts["transport"] == kp.B_FACE_CT:
         if curved and p["coords"] == kp.FMKS:
             pot = facefield.axisymmetric_loop_potential(p, amp=1e-3, x1c=0.5 * (p["xmin"][0] + p["xmax"][0]),
@@ -704,20 +736,36 @@ def test_fuzz_one_step_random_configurations(kh, kho, seed):
         if not curved and any(b != kp.BC_PERIODIC for b in p["bc"]):
             pot = [np.zeros_like(pot[0]), np.zeros_like(pot[0]), pot[2] * 0 + 1e-3 * np.cos(np.linspace(0, 1, pot[2].shape[2]))[None, None, :]]
         faces = facefield.face_from_potential(p, *pot)
-        for g in (gg, go):
-            g.set_face_B(*faces)
     label = "fuzz %d %s n=%s bc=%s" % (seed, opts, n, p["bc"])
+    return p, P0, faces, opts, label
+
+
+@pytest.mark.parametrize("seed", list(range(int(__import__("os").environ.get("KH_FUZZ_SEEDS", "48")))) + [432])
+def test_fuzz_one_step_random_configurations(kh, kho, seed):
+    """Random small blocks: ragged sizes (down to 3 zones), every boundary kind that is legal for the coordinate system,
+    and random choices of reconstruction, inverter, floor frame, FOFC, transport and EMF kind.  One step (plus one more
+    for the odd seeds), the usual bars.  Seed 432 is the one seed of 0..999 that was outside the bar at the end of round 1
+    (named here so that it runs every time)."""
+    p, P0, faces, opts, label = _fuzz_case(seed)
+    gg, go = kh.Grid(p), kho.Grid(p, omp=True)
+    for g in (gg, go):
+        g.set_prims(P0)
+        if faces is not None:
+            g.set_face_B(*faces)
     dt = go.estimate_dt()
     assert abs(gg.estimate_dt() / dt - 1) < 1e-12, label
+    dts = []
     for _ in range(1 + seed % 2):
         n_g, n_o = gg.step(dt), go.step(dt)
         assert abs(n_g / n_o - 1) < 1e-10, label
+        dts.append(dt)
         dt = n_o
     pf_g, ff_g = gg.get_flags()
     pf_o, ff_o = go.get_flags()
-    # two steps double the bar; the normal-frame floors invert twice per zone, which squares the conditioning of u
-    tol = TOL_ONE_STEP * (2 if seed % 2 else 1) * (4 if opts["floor_frame"] == kp.FRAME_NORMAL else 1)
-    _assert_step_parity(p, gg.get_prims(), go.get_prims(), pf_g, pf_o, label, tol=tol)
+    # the flat bar for one step and for two, for every floor frame: what exceeds it must be explained by the oracle's own
+    # measured sensitivity to 1-ulp input noise (S23c), not by a looser number
+    sens = oracle_sensitivity(kho, p, P0, faces, dts)
+    _assert_step_parity(p, gg.get_prims(), go.get_prims(), pf_g, pf_o, label, tol=TOL_ONE_STEP, sens=sens)
     if opts["floor_frame"] != kp.FRAME_NORMAL:      # (after a normal-frame injection rho sits AT its floor: the second-pass bit is a coin flip)
         assert (ff_g != ff_o).sum() <= max(2, (1e-2 if opts["fofc"] else 5e-3) * ff_o.size), label    # marginal floor decisions may flip
 
