@@ -40,7 +40,8 @@ extern "C" {
 
 enum { KH_OK = 0, KH_EINVAL = -1, KH_ENOMEM = -2, KH_ECUDA = -3, KH_ENAN = -4 };
 enum { KH_MINKOWSKI = 0, KH_KS = 1, KH_FMKS = 2 };                            /* coords          */
-enum { KH_BC_PERIODIC = 0, KH_BC_OUTFLOW = 1, KH_BC_POLAR = 2, KH_BC_FIXED = 3 };
+enum { KH_BC_PERIODIC = 0, KH_BC_OUTFLOW = 1, KH_BC_POLAR = 2, KH_BC_FIXED = 3,
+       KH_BC_BLOCK = 4 /* ghost layers owned by a neighbouring block: kh_link_blocks, kh_step_blocks */ };
 enum { KH_RECON_MC = 0, KH_RECON_WENO5 = 1 };
 enum { KH_INV_1DW = 0, KH_INV_KASTAUN = 1 };
 enum { KH_FRAME_FLUID = 0, KH_FRAME_DRIFT = 1, KH_FRAME_NORMAL = 2 };
@@ -56,7 +57,7 @@ typedef struct {
   int n1, n2, n3;             /* interior zones; n3 == 1 runs a 2-D problem as a one-zone-thick block      */
   double xmin[3], xmax[3];    /* native-coordinate bounds of the interior                                  */
   int bc[6];                  /* x1lo x1hi x2lo x2hi x3lo x3hi; periodic must be set on both sides;
-                                 KH_BC_POLAR only in x2 (needs n2 >= 3)                                     */
+                                 KH_BC_POLAR only in x2 (needs n2 >= 3); KH_BC_BLOCK needs N_d >= 3          */
   double gamma, cfl;          /* adiabatic index; Courant factor                                           */
   int recon;                  /* KH_RECON_MC | KH_RECON_WENO5                                              */
   double rho_min, u_min, r_char, bsq_over_rho_max, bsq_over_u_max, u_over_rho_max, gamma_max; /* floors */
@@ -130,6 +131,24 @@ int kh_divB(kh_grid* g, double* max_abs);
 
 /* Number of zones with pflag != 0 and with fflag != 0 in the last sub-step (HOST ints; may be NULL). */
 int kh_count_flags(kh_grid* g, long long* n_pflag, long long* n_fflag);
+
+/* ---- several blocks on one device ("HARM requires two synchronizations") ----
+ * A mesh block may be cut into several kh_grids along any direction.  A side whose neighbour is another block is created
+ * with KH_BC_BLOCK; kh_link_blocks(lo, hi, dir) declares that `hi` continues `lo` across lo's upper dir-side (dir = 1..3;
+ * both sides must be KH_BC_BLOCK, the transverse sizes, zone sizes, the stream and every option must agree; a periodic
+ * direction cut in two is closed by a second link (hi, lo)).  Restrictions: fofc = 0, KH_B_FLUX_CT, KH_EMF_ARITHMETIC;
+ * in FMKS cut along x2 or x3 (the map's x1 origin is a block's own xmin[0]).
+ * kh_exchange_halos(blocks, n) packs the 3 layers next to every linked side (8 primitives + the inversion flag, over the full
+ * padded transverse extent) into that side's message buffer and unpacks it into the neighbour's ghost layers -- on one
+ * device the neighbour reads the buffer directly; the buffer is what an inter-GPU transport would send.  Call it after
+ * loading primitives into linked blocks.
+ * kh_step_blocks steps all n blocks (n <= 16) by dt together: per sub-step every block computes fluxes, EMFs, update and its
+ * own boundary fills; halos are exchanged; every block repairs its failed zones (reading the neighbour's flags and values
+ * through the halo); halos are exchanged again -- the two synchronisations of P:317 -- and dt_next is the minimum over the
+ * blocks (one scalar reduction).  dt <= 0 and dt_next as for kh_step.  The result equals the single-block step bit for bit. */
+int kh_link_blocks(kh_grid* lo, kh_grid* hi, int dir);
+int kh_exchange_halos(kh_grid* const* blocks, int n);
+int kh_step_blocks(kh_grid* const* blocks, int n, double dt, double* dt_next);
 
 /* ---- stage access (tests / debugging) ---- */
 /* Geometry tables over (j,i) with ghosts, [(n2+6)*(n1+6)] points: gcov/gcon as 16 doubles per point

@@ -10,6 +10,7 @@ PRIM_NAMES = ("rho", "u", "ut1", "ut2", "ut3", "B1", "B2", "B3")
 
 MINKOWSKI, KS, FMKS = 0, 1, 2
 BC_PERIODIC, BC_OUTFLOW, BC_POLAR, BC_FIXED = 0, 1, 2, 3
+BC_BLOCK = 4            # ghost layers owned by a neighbouring block (libkharm only: kh_link_blocks / kh_step_blocks)
 RECON_MC, RECON_WENO5 = 0, 1
 INV_1DW, INV_KASTAUN = 0, 1
 FRAME_FLUID, FRAME_DRIFT, FRAME_NORMAL = 0, 1, 2

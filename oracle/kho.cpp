@@ -803,7 +803,7 @@ void compute_flux(kho_grid& g, const double* Ps, int d) {
   double* F = g.F[d].data();
   double* ct = g.ctop[d].data();
 #ifdef _OPENMP
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for collapse(2) schedule(static)
 #endif
   for (int k = lo[2]; k < hi[2]; k++)
     for (int j = lo[1]; j < hi[1]; j++)
@@ -964,7 +964,7 @@ void update_zones(kho_grid& g, const double* Pi, const double* Ps, double* Pf, d
   std::fill(g.pflag.begin(), g.pflag.end(), 0);
   std::fill(g.fflag.begin(), g.fflag.end(), 0);
 #ifdef _OPENMP
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for collapse(2) schedule(static)
 #endif
   for (int k = 0; k < g.n[2]; k++) for (int j = 0; j < g.n[1]; j++) for (int i = 0; i < g.n[0]; i++) {
     long n = g.idx(i, j, k), n2 = g.idx2(i, j);

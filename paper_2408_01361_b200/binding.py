@@ -9,7 +9,7 @@ import os
 import numpy as np
 
 MINKOWSKI, KS, FMKS = 0, 1, 2
-BC_PERIODIC, BC_OUTFLOW, BC_POLAR, BC_FIXED = 0, 1, 2, 3
+BC_PERIODIC, BC_OUTFLOW, BC_POLAR, BC_FIXED, BC_BLOCK = 0, 1, 2, 3, 4
 RECON_MC, RECON_WENO5 = 0, 1
 INV_1DW, INV_KASTAUN = 0, 1
 LOC_CENT, LOC_FACE1, LOC_FACE2, LOC_FACE3 = 0, 1, 2, 3
@@ -21,7 +21,7 @@ EXPORTED_SYMBOLS = (
     "kh_grid_create", "kh_grid_destroy", "kh_set_prims", "kh_get_prims", "kh_get_cons", "kh_get_flags",
     "kh_estimate_dt", "kh_step", "kh_divB", "kh_set_face_B", "kh_get_face_B", "kh_divB_face", "kh_count_flags", "kh_get_geom", "kh_get_conn", "kh_get_flux",
     "kh_get_emf", "kh_debug_fixup", "kh_debug_predictor", "kh_launch_count", "kh_set_graph", "kh_set_profile", "kh_get_profile", "kh_measure_fp64_peak", "kh_strerror",
-    "kh_last_cuda_error", "kh_get_stream", "kh_sync",
+    "kh_last_cuda_error", "kh_get_stream", "kh_sync", "kh_link_blocks", "kh_exchange_halos", "kh_step_blocks",
 )
 
 
@@ -97,6 +97,9 @@ def lib():
         L.kh_measure_fp64_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.kh_get_stream.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
         L.kh_sync.argtypes = [C.c_void_p]
+        L.kh_link_blocks.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        L.kh_exchange_halos.argtypes = [C.POINTER(C.c_void_p), C.c_int]
+        L.kh_step_blocks.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_double, C.POINTER(C.c_double)]
         _LIB = L
     return _LIB
 
@@ -116,6 +119,29 @@ def measure_fp64_peak():
     tf, mhz = C.c_double(), C.c_double()
     _chk(lib().kh_measure_fp64_peak(C.byref(tf), C.byref(mhz)))
     return tf.value, mhz.value
+
+
+def _handles(blocks):
+    return (C.c_void_p * len(blocks))(*[b.h for b in blocks])
+
+
+def link_blocks(lo, hi, direction):
+    """`hi` continues `lo` across lo's upper side in direction 1..3 (both sides KH_BC_BLOCK)."""
+    _chk(lib().kh_link_blocks(lo.h, hi.h, int(direction)))
+
+
+def exchange_halos(blocks):
+    _chk(lib().kh_exchange_halos(_handles(blocks), len(blocks)))
+
+
+def step_blocks(blocks, dt, sync=True):
+    """One predictor-corrector step of several linked blocks together; returns the common dt_next (sync=True)."""
+    if sync:
+        nxt = C.c_double()
+        _chk(lib().kh_step_blocks(_handles(blocks), len(blocks), C.c_double(dt), C.byref(nxt)))
+        return nxt.value
+    _chk(lib().kh_step_blocks(_handles(blocks), len(blocks), C.c_double(dt), None))
+    return None
 
 
 class Grid:

@@ -362,7 +362,7 @@ __device__ __forceinline__ int ghost_map(int gi, int N, int bc_lo, int bc_hi, in
   if (gi >= 0 && gi < N) return gi;
   const int side = gi >= N;
   const int bc = side ? bc_hi : bc_lo;
-  if (bc == 3) return gi;                                   // fixed: the ghost keeps its content
+  if (bc >= 3) return gi;                                   // fixed (3) or owned by a neighbouring block (4): the ghost keeps its content
   if (bc == 0) {                                            // periodic wrap (a block thinner than the ghost layer wraps more than once)
     kind = KH_MAP_COPY;
     return N >= KH_NGH ? (side ? gi - N : gi + N) : ((gi % N) + N) % N;
@@ -994,6 +994,65 @@ fixup_apply_kernel(GV g, double* __restrict__ Pf, const unsigned* __restrict__ l
     for (int v = 0; v < 5; v++) Pf[v * nt + n] = P[v];
     store_ghost_images<5>(g, Pf, nullptr, i, j, k, P, 0);
   }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Multi-block halo exchange ("two synchronizations").  A side with KH_BC_BLOCK has its
+// 3 ghost layers owned by the neighbouring block.  halo_pack_kernel gathers the 3 interior layers next to that side -- over the
+// FULL padded extent of the two transverse directions, whose own ghosts the block's fill has already set, so that edges and
+// corners arrive composed exactly as the single-block fill composes them -- 8 primitives and the inversion flag, into one
+// contiguous message [9][3][t2][t1] (the flag as a double: one message per side and synchronisation).  halo_unpack_kernel
+// scatters a message into the ghost layers of the receiving side.  Between the two sits the transport: on one GPU the
+// receiver reads the sender's buffer directly; across GPUs it is one ncclSend / ncclRecv (or peer copy) of the same buffer.
+// dir 1..3; side 0 = lower, 1 = upper.  Layer l = 0..2 counts away from the lower end of the packed / unpacked slab.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void halo_index(const GV& g, int dir, long t, int& l, int& a, int& b, long& count) {
+  // transverse padded extents (t1 fastest): dir 1 -> (nt2, nt3), dir 2 -> (nt1, nt3), dir 3 -> (nt1, nt2)
+  const int e1 = dir == 1 ? g.nt2 : g.nt1, e2 = dir == 3 ? g.nt2 : g.nt3;
+  count = (long)KH_NGH * e1 * e2;
+  a = (int)(t % e1);
+  const long r = t / e1;
+  b = (int)(r % e2);
+  l = (int)(r / e2);
+}
+__device__ __forceinline__ long halo_zone(const GV& g, int dir, int first, int l, int a, int b) {
+  // padded indices (0-based with ghosts) of layer first + l along dir and transverse position (a, b)
+  const int i = dir == 1 ? first + l : a, j = dir == 2 ? first + l : (dir == 1 ? a : b), k = dir == 3 ? first + l : b;
+  return (long)k * g.s3 + (long)j * g.s2 + i;
+}
+__global__ void __launch_bounds__(128)
+halo_pack_kernel(GV g, const double* __restrict__ P, const unsigned char* __restrict__ flag, int dir, int side, double* __restrict__ buf) {
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  int l, a, b; long count;
+  halo_index(g, dir, t, l, a, b, count);
+  if (t >= count) return;
+  const int N = dir == 1 ? g.n1 : (dir == 2 ? g.n2 : g.n3);
+  const long n = halo_zone(g, dir, side ? N : KH_NGH, l, a, b);      // interior layers next to the side: padded [NG, 2NG) or [N, N+NG)
+#pragma unroll
+  for (int v = 0; v < KH_NP; v++) buf[v * count + t] = P[v * g.ntot + n];
+  buf[KH_NP * count + t] = (double)flag[n];
+}
+__global__ void __launch_bounds__(128)
+halo_unpack_kernel(GV g, double* __restrict__ P, unsigned char* __restrict__ flag, int dir, int side, const double* __restrict__ buf) {
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  int l, a, b; long count;
+  halo_index(g, dir, t, l, a, b, count);
+  if (t >= count) return;
+  const int N = dir == 1 ? g.n1 : (dir == 2 ? g.n2 : g.n3);
+  const long n = halo_zone(g, dir, side ? N + KH_NGH : 0, l, a, b);  // ghost layers of the side: padded [0, NG) or [N+NG, N+2NG)
+#pragma unroll
+  for (int v = 0; v < KH_NP; v++) P[v * g.ntot + n] = buf[v * count + t];
+  flag[n] = (unsigned char)buf[KH_NP * count + t];
+}
+
+// dt_next of a set of linked blocks: the CFL maximum over all of them (the "one scalar min all-reduce" of SURVEY 8(e))
+struct BlockScalars { StepScalars* sc[16]; int n; };
+__global__ void finalize_dt_blocks_kernel(BlockScalars bs, double cfl, double growth) {
+  unsigned long long m = 0ULL, bad = 0ULL;
+  for (int b = 0; b < bs.n; b++) { m = bs.sc[b]->rate_bits > m ? bs.sc[b]->rate_bits : m; bad |= bs.sc[b]->nonfinite; }
+  const double d = cfl * (1.0 / __longlong_as_double((long long)m)), cap = growth * bs.sc[0]->dt;
+  const double nxt = bad ? __longlong_as_double(0x7ff8000000000000LL) : (d < cap ? d : cap);
+  for (int b = 0; b < bs.n; b++) { bs.sc[b]->dt_next = nxt; bs.sc[b]->rate_bits = 0ULL; bs.sc[b]->nonfinite = bad; }
 }
 
 // ---------------------------------------------------------------------------------------------

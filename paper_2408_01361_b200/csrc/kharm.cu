@@ -5,6 +5,7 @@
 
 #include <cstdio>
 #include <cstdlib>
+#include <cmath>
 #include <cstring>
 #include <new>
 
@@ -46,6 +47,9 @@ struct kh_grid {
   bool fixed_ghosts_set; // ... and a with_ghosts = 1 load has supplied the ghost layers
   bool have_dt_next;     // a completed step has left a dt_next on the device (kh_step(dt <= 0) is legal)
   int device;            // the CUDA device the grid lives on
+  bool has_block;        // some side is KH_BC_BLOCK: stepped by kh_step_blocks only
+  kh_grid* nb[3][2];     // neighbouring block across [dir - 1][side] (kh_link_blocks)
+  double* halo_buf[3][2];// message buffer of the 3 layers next to that side: [9][3][t2][t1] doubles (8 primitives + flag)
   double* Bf[3][3];      // face-centred CT: Phi^d per rotation state [state][d], [ntot] each (allocated on demand)
   unsigned char* mask;   // FOFC: troubled zones of the speculative update (with ghost images)
   unsigned* faillist;    // zones (device-layout index) whose inversion failed in the current sub-step
@@ -231,7 +235,7 @@ static int do_fixup(kh_grid* g, double* Pf) {
 
 // One sub-step (S22): fluxes from Ps, update of U(Pi), inversion with guess Pi, floors, fill, fix-up, fill.
 static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, double dt_factor, bool corrector,
-                   double* const* Bfi = nullptr, double* const* Bff = nullptr) {
+                   double* const* Bfi = nullptr, double* const* Bff = nullptr, bool with_fixup = true) {
   const GV& v = g->gv;
   reset_counters_kernel<<<1, 1, 0, g->stream>>>(g->sc, 0);
   g->launches++;
@@ -325,6 +329,7 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
       CK(cudaGetLastError());
     }
   }
+  if (!with_fixup) return fill_ghosts(g, Pf, g->pflag);          // linked blocks: halo exchange, fix-up, halo exchange follow (kh_step_blocks)
   int rc = fill_ghosts(g, Pf, g->pflag);
   if (rc) return rc;
   return do_fixup(g, Pf);      // also refreshes the ghost images of the fixed zones (the second fill of S22)
@@ -391,6 +396,10 @@ int kh_grid_destroy(kh_grid* g) {
   for (int b = 0; b < 3; b++) { free_shifted(g->P[b]); free_shifted(g->F[b]); free_shifted(g->ctop[b]); free_shifted(g->emf[b]); }
   cudaFree(g->pflag); cudaFree(g->fflag); cudaFree(g->mask);
   for (int b = 0; b < 3; b++) for (int d = 0; d < 3; d++) free_shifted(g->Bf[b][d]);
+  for (int d = 0; d < 3; d++) for (int sd = 0; sd < 2; sd++) {
+    cudaFree(g->halo_buf[d][sd]);
+    if (g->nb[d][sd] && g->nb[d][sd]->nb[d][1 - sd] == g) g->nb[d][sd]->nb[d][1 - sd] = nullptr;    // unlink the neighbour
+  }
   for (int d = 0; d < 4; d++) cudaFree(g->ecent[d]); cudaFree(g->faillist); cudaFree(g->sc); cudaFree(g->fix); cudaFree(g->stage);
   if (g->sc_host) cudaFreeHost(g->sc_host);
   if (g->pev) { for (int e = 0; e < 2 * KH_PROF_POOL; e++) if (g->pev[e]) cudaEventDestroy(g->pev[e]); delete[] g->pev; }
@@ -412,8 +421,9 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
     if (!(p->xmax[d] > p->xmin[d])) return KH_EINVAL;
     for (int s = 0; s < 2; s++) {
       int bc = p->bc[2 * d + s];
-      if (bc < 0 || bc > 3) return KH_EINVAL;
+      if (bc < 0 || bc > 4) return KH_EINVAL;
       if (bc == KH_BC_POLAR && (d != 1 || N[d] < KH_NGH)) return KH_EINVAL;
+      if (bc == KH_BC_BLOCK && (N[d] < KH_NGH || p->fofc || p->transport != KH_B_FLUX_CT || p->emf != KH_EMF_ARITHMETIC)) return KH_EINVAL;
     }
     if ((p->bc[2 * d] == KH_BC_PERIODIC) != (p->bc[2 * d + 1] == KH_BC_PERIODIC)) return KH_EINVAL;
   }
@@ -433,7 +443,7 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
     g->own_stream = true;
   }
   g->flat = (p->coords == KH_MINKOWSKI);
-  for (int b = 0; b < 6; b++) g->has_fixed = g->has_fixed || p->bc[b] == KH_BC_FIXED;
+  for (int b = 0; b < 6; b++) { g->has_fixed = g->has_fixed || p->bc[b] == KH_BC_FIXED; g->has_block = g->has_block || p->bc[b] == KH_BC_BLOCK; }
   {
     int dev = 0;
     cudaGetDevice(&dev);
@@ -674,6 +684,7 @@ int kh_step(kh_grid* g, double dt, double* dt_next) {
   if (!g || dt != dt) return KH_EINVAL;
   if (g->p.transport == KH_B_FACE_CT && !g->faces_set) return KH_EINVAL;   // the face field is the magnetic state: set it first
   if (g->has_fixed && !g->fixed_ghosts_set) return KH_EINVAL;               // FIXED ghost layers were never supplied
+  if (g->has_block) return KH_EINVAL;                                       // a block with KH_BC_BLOCK sides steps with its neighbours: kh_step_blocks
   if (!(dt > 0.0) && !g->have_dt_next) return KH_EINVAL;                    // no dt_next on the device yet
   ENTER(g);
   set_dt_kernel<<<1, 1, 0, g->stream>>>(g->sc, dt, dt > 0.0 ? 0 : 1);
@@ -737,13 +748,125 @@ int kh_sync(kh_grid* g) {
   return KH_OK;
 }
 
+// ---- several blocks on one device ----
+static long halo_count(const GV& v, int dir) {
+  const long e1 = dir == 1 ? v.nt2 : v.nt1, e2 = dir == 3 ? v.nt2 : v.nt3;
+  return (long)KH_NGH * e1 * e2;
+}
+
+int kh_link_blocks(kh_grid* lo, kh_grid* hi, int dir) {
+  if (!lo || !hi || dir < 1 || dir > 3) return KH_EINVAL;
+  const int d = dir - 1;
+  if (lo->p.bc[2 * d + 1] != KH_BC_BLOCK || hi->p.bc[2 * d] != KH_BC_BLOCK) return KH_EINVAL;
+  if (lo->stream != hi->stream || lo->device != hi->device) return KH_EINVAL;
+  const int nl[3] = {lo->p.n1, lo->p.n2, lo->p.n3}, nh[3] = {hi->p.n1, hi->p.n2, hi->p.n3};
+  for (int e = 0; e < 3; e++) {
+    if (e != d && nl[e] != nh[e]) return KH_EINVAL;                                             // same transverse shape
+    const double dl = (lo->p.xmax[e] - lo->p.xmin[e]) / nl[e], dh = (hi->p.xmax[e] - hi->p.xmin[e]) / nh[e];
+    if (!(fabs(dl - dh) <= 1e-12 * fabs(dl))) return KH_EINVAL;                                 // same zone size
+  }
+  if (lo->p.coords != hi->p.coords || lo->p.recon != hi->p.recon || lo->p.inverter != hi->p.inverter || lo->p.floor_frame != hi->p.floor_frame ||
+      lo->p.gamma != hi->p.gamma || lo->p.cfl != hi->p.cfl) return KH_EINVAL;
+  ENTER(lo);
+  const size_t bytes = sizeof(double) * (KH_NP + 1) * (size_t)halo_count(lo->gv, dir);
+  if (!lo->halo_buf[d][1]) CK(cudaMalloc((void**)&lo->halo_buf[d][1], bytes));
+  if (!hi->halo_buf[d][0]) CK(cudaMalloc((void**)&hi->halo_buf[d][0], bytes));
+  lo->nb[d][1] = hi;
+  hi->nb[d][0] = lo;
+  return KH_OK;
+}
+
+// every linked side: pack the sender's 3 layers, then unpack into the receiver's ghosts (all packs first: a block thinner than
+// 6 zones would otherwise send layers its own unpack has just overwritten -- not possible here, ghosts are not interior, but
+// the order also is what a two-sided transport needs)
+static int exchange(kh_grid* const* blocks, int n, int which /* offset of the P buffer from cur */) {
+  for (int pass = 0; pass < 2; pass++)
+    for (int b = 0; b < n; b++) {
+      kh_grid* g = blocks[b];
+      for (int d = 0; d < 3; d++) for (int sd = 0; sd < 2; sd++) {
+        if (g->p.bc[2 * d + sd] != KH_BC_BLOCK) continue;
+        kh_grid* nbr = g->nb[d][sd];
+        if (!nbr) return KH_EINVAL;                                                              // a KH_BC_BLOCK side that was never linked
+        const long cnt = halo_count(g->gv, d + 1);
+        const unsigned grid = (unsigned)((cnt + 127) / 128);
+        if (pass == 0) halo_pack_kernel<<<grid, 128, 0, g->stream>>>(g->gv, g->P[(g->cur + which) % 3], g->pflag, d + 1, sd, g->halo_buf[d][sd]);
+        else halo_unpack_kernel<<<grid, 128, 0, g->stream>>>(g->gv, g->P[(g->cur + which) % 3], g->pflag, d + 1, sd, nbr->halo_buf[d][1 - sd]);
+        g->launches++;
+      }
+    }
+  CK(cudaGetLastError());
+  return KH_OK;
+}
+
+static int check_blocks(kh_grid* const* blocks, int n) {
+  if (!blocks || n < 1 || n > 16) return KH_EINVAL;
+  for (int b = 0; b < n; b++) {
+    if (!blocks[b] || blocks[b]->stream != blocks[0]->stream || blocks[b]->cur != blocks[0]->cur) return KH_EINVAL;
+    if (blocks[b]->has_fixed && !blocks[b]->fixed_ghosts_set) return KH_EINVAL;
+  }
+  return KH_OK;
+}
+
+int kh_exchange_halos(kh_grid* const* blocks, int n) {
+  int rc = check_blocks(blocks, n);
+  if (rc) return rc;
+  ENTER(blocks[0]);
+  return exchange(blocks, n, 0);
+}
+
+int kh_step_blocks(kh_grid* const* blocks, int n, double dt, double* dt_next) {
+  int rc = check_blocks(blocks, n);
+  if (rc) return rc;
+  if (dt != dt) return KH_EINVAL;
+  for (int b = 0; b < n; b++) if (!(dt > 0.0) && !blocks[b]->have_dt_next) return KH_EINVAL;
+  ENTER(blocks[0]);
+  for (int b = 0; b < n; b++) {
+    kh_grid* g = blocks[b];
+    set_dt_kernel<<<1, 1, 0, g->stream>>>(g->sc, dt, dt > 0.0 ? 0 : 1);
+    g->launches++;
+  }
+  const int cur = blocks[0]->cur;
+  for (int sub = 0; sub < 2; sub++) {
+    const int out = sub == 0 ? 1 : 2;                      // P* = P[cur + 1], P^{n+1} = P[cur + 2]
+    for (int b = 0; b < n; b++) {                          // K2, K3, K4/K5 and the block's own boundary fills
+      kh_grid* g = blocks[b];
+      rc = substep(g, g->P[cur], sub == 0 ? g->P[cur] : g->P[(cur + 1) % 3], g->P[(cur + out) % 3], sub == 0 ? 0.5 : 1.0, sub == 1,
+                   nullptr, nullptr, false);
+      if (rc) return rc;
+    }
+    rc = exchange(blocks, n, out);                         // first synchronisation: primitives and inversion flags
+    if (rc) return rc;
+    for (int b = 0; b < n; b++) {                          // K5b: failed zones read their neighbours through the halo
+      rc = do_fixup(blocks[b], blocks[b]->P[(cur + out) % 3]);
+      if (rc) return rc;
+    }
+    rc = exchange(blocks, n, out);                         // second synchronisation: the repaired zones reach the neighbours' ghosts
+    if (rc) return rc;
+  }
+  BlockScalars bs;
+  bs.n = n;
+  for (int b = 0; b < n; b++) bs.sc[b] = blocks[b]->sc;
+  finalize_dt_blocks_kernel<<<1, 1, 0, blocks[0]->stream>>>(bs, blocks[0]->p.cfl, blocks[0]->p.dt_growth_max);
+  blocks[0]->launches++;
+  CK(cudaGetLastError());
+  for (int b = 0; b < n; b++) { blocks[b]->cur = (cur + 2) % 3; blocks[b]->have_dt_next = true; }
+  if (dt_next) {
+    rc = read_scalars(blocks[0]);
+    if (rc) return rc;
+    if (blocks[0]->sc_host->nonfinite || !(blocks[0]->sc_host->dt_next == blocks[0]->sc_host->dt_next)) return KH_ENAN;
+    *dt_next = blocks[0]->sc_host->dt_next;
+  }
+  return KH_OK;
+}
+
 int kh_divB(kh_grid* g, double* max_abs) {
   if (!g || !max_abs) return KH_EINVAL;
   ENTER(g);
   const GV& v = g->gv;
   int lo[3], cnt[3];
   const int N[3] = {v.n1, v.n2, v.n3};
-  for (int d = 0; d < 3; d++) { lo[d] = (g->p.bc[2 * d] == KH_BC_PERIODIC) ? 0 : 1; cnt[d] = N[d] - lo[d]; }
+  // corners on a lower boundary plane involve ghost zones: valid where those are periodic images or a neighbouring block's zones
+  for (int d = 0; d < 3; d++) { lo[d] = (g->p.bc[2 * d] == KH_BC_PERIODIC || g->p.bc[2 * d] == KH_BC_BLOCK) ? 0 : 1; cnt[d] = N[d] - lo[d]; }
   unsigned long long zero = 0;
   CK(cudaMemcpyAsync(&g->sc->max_bits, &zero, sizeof(zero), cudaMemcpyHostToDevice, g->stream));
   if (cnt[0] > 0 && cnt[1] > 0 && cnt[2] > 0) {

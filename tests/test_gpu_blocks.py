@@ -1,0 +1,164 @@
+"""GPU: a mesh block cut into linked blocks with halo exchange (SURVEY 8(e), 8(f) NEXT-4 second half; "two
+synchronizations") reproduces the single-block step: bit for bit against the single-block CUDA result, to the usual
+bars against the single-block oracle, identical flags, identical dt_next, div B at round-off across the seam."""
+import numpy as np
+import pytest
+
+import kharm_inputs as ki
+from kharm_inputs import modes, torus
+from kharm_inputs import params as kp
+from parity_util import rel_diff
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def kh():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2408_01361_b200 as m
+    m.lib()
+    return m
+
+
+def _cut(p, d, sizes):
+    """Parameter sets of the pieces of block p cut along direction d (0..2) into consecutive pieces of the given sizes."""
+    key = ("n1", "n2", "n3")[d]
+    assert sum(sizes) == p[key]
+    dx = (p["xmax"][d] - p["xmin"][d]) / p[key]
+    periodic = p["bc"][2 * d] == kp.BC_PERIODIC
+    out, start = [], 0
+    for m, sz in enumerate(sizes):
+        q = dict(p, xmin=list(p["xmin"]), xmax=list(p["xmax"]), bc=list(p["bc"]))
+        q[key] = sz
+        q["xmin"][d] = p["xmin"][d] + start * dx
+        q["xmax"][d] = p["xmin"][d] + (start + sz) * dx
+        if m > 0 or periodic:
+            q["bc"][2 * d] = kp.BC_BLOCK
+        if m < len(sizes) - 1 or periodic:
+            q["bc"][2 * d + 1] = kp.BC_BLOCK
+        out.append(q)
+        start += sz
+    return out, periodic
+
+
+def _make_blocks(kh, p, d, sizes, P0):
+    import torch
+    parts, periodic = _cut(p, d, sizes)
+    stream = torch.cuda.Stream()              # linked blocks share ONE stream (NULL would give every grid a stream of its own)
+    blocks = [kh.Grid(q, stream=stream.cuda_stream) for q in parts]
+    blocks[0]._keep_stream = stream
+    for a, b in zip(blocks[:-1], blocks[1:]):
+        kh.link_blocks(a, b, d + 1)
+    if periodic:
+        kh.link_blocks(blocks[-1], blocks[0], d + 1)
+    pieces = np.split(P0, np.cumsum(sizes)[:-1], axis=3 - d)
+    for g, piece in zip(blocks, pieces):
+        g.set_prims(np.ascontiguousarray(piece))
+    kh.exchange_halos(blocks)
+    return blocks
+
+
+def _merge(arrs, d, axis0):
+    return np.concatenate(arrs, axis=axis0 + 2 - d)
+
+
+# The cuts sit where the pieces' zone size (xmax - xmin) / N is the parent's to the last bit (power-of-two fractions of the
+# extent): 1 / dx enters every flux difference, and "bit for bit" below means exactly that.
+CASES = [
+    ("cfg5 x3 halves", lambda: ki.config_params(5, n=(24, 20, 16), recon=kp.RECON_WENO5), lambda p: modes.config5(p, seed=3, amp=1e-2), 2, (8, 8)),
+    ("cfg5 x1 ragged", lambda: ki.config_params(5, n=(32, 20, 6), recon=kp.RECON_MC), lambda p: modes.config5(p, seed=4, amp=1e-2), 0, (12, 20)),
+    ("cfg5 x2 three pieces", lambda: ki.config_params(5, n=(16, 32, 5), recon=kp.RECON_WENO5), lambda p: modes.config5(p, seed=5, amp=1e-2), 1, (8, 12, 12)),
+    ("cfg3 torus x3 halves", lambda: ki.config_params(3, n=(48, 32, 16)), lambda p: torus.torus_state(p, seed=1), 2, (8, 8)),
+    ("cfg4 MAD stress x3, failures at the seam", lambda: ki.config_params(4, n=(48, 24, 16)),
+     lambda p: torus.torus_state(p, mad=True, seed=2, stress=True, stress_fraction=0.04), 2, (4, 12)),
+    ("cfg3 torus x2 (polar ends, cut at the equator)", lambda: ki.config_params(3, n=(40, 24, 6)), lambda p: torus.torus_state(p, seed=3), 1, (12, 12)),
+]
+
+
+@pytest.mark.parametrize("label,mkp,mkP,d,sizes", CASES, ids=[c[0] for c in CASES])
+def test_linked_blocks_reproduce_the_single_block(kh, kho, label, mkp, mkP, d, sizes):
+    from test_gpu_parity import _assert_step_parity
+    p = mkp()
+    P0 = mkP(p)
+    single = kh.Grid(p)
+    single.set_prims(P0)
+    go = kho.Grid(p, omp=True)
+    go.set_prims(P0)
+    blocks = _make_blocks(kh, p, d, sizes, P0)
+    # ghosts after the first exchange equal the single block's ghosts (full padded extent of the transverse directions)
+    full = single.get_prims(with_ghosts=True)
+    start = 0
+    for g, sz in zip(blocks, sizes):
+        sl = [slice(None)] * 4
+        sl[3 - d] = slice(start, start + sz + 6)
+        if "x2 (polar" not in label:
+            assert np.array_equal(g.get_prims(with_ghosts=True), full[tuple(sl)]), label
+        else:            # outflow ghosts carry the ratio of tabulated sqrt(-g)
+            assert np.allclose(g.get_prims(with_ghosts=True), full[tuple(sl)], rtol=1e-13, atol=0), label
+        start += sz
+    bitwise = "x2 (polar" not in label      # a cut in x2 of a curved block: the pieces tabulate the metric at xmin2' + (j + 1/2) dx2,
+    dt = min(g.estimate_dt() for g in blocks)   # the parent at xmin2 + (j' + 1/2) dx2 -- the same points to an ulp, not to the bit
+    assert dt == single.estimate_dt() if bitwise else abs(dt / single.estimate_dt() - 1) < 1e-13
+    failures = 0
+    for step in range(3):
+        n_s = single.step(dt)
+        n_b = kh.step_blocks(blocks, dt)
+        assert n_b == n_s if bitwise else abs(n_b / n_s - 1) < 1e-13, (label, step)    # the same dt_next, bit for bit
+        merged = _merge([g.get_prims() for g in blocks], d, 1)
+        if bitwise:
+            assert np.array_equal(merged, single.get_prims()), (label, step)        # the same state, bit for bit
+        else:
+            assert rel_diff(p, merged, single.get_prims()).max() < 1e-11, (label, step)
+        pf = _merge([g.get_flags()[0] for g in blocks], d, 0)
+        ff = _merge([g.get_flags()[1] for g in blocks], d, 0)
+        pf_s, ff_s = single.get_flags()
+        assert np.array_equal(pf, pf_s) and np.array_equal(ff, ff_s), (label, step)
+        failures += int((pf != 0).sum())
+        if step == 0:
+            n_o = go.step(dt)
+            assert abs(n_b / n_o - 1) < 1e-11
+            _assert_step_parity(p, merged, go.get_prims(), pf, go.get_flags()[0], "blocks " + label)
+        # div B of the corner-centred divergence, seam corners included (they read the exchanged ghosts)
+        assert max(g.divB() for g in blocks) <= max(single.divB() * 1.0000001, 1e-13), label
+        dt = n_s
+    if "stress" in label:
+        assert failures > 0                     # the fix-up did run, also next to the seam
+    # a block with linked sides cannot be stepped on its own
+    with pytest.raises(kh.KharmError):
+        blocks[0].step(dt)
+
+
+def test_device_resident_dt_over_linked_blocks(kh):
+    p = ki.config_params(5, n=(20, 12, 12), recon=kp.RECON_MC)
+    P0 = modes.config5(p, seed=7, amp=1e-2)
+    single = kh.Grid(p)
+    single.set_prims(P0)
+    blocks = _make_blocks(kh, p, 2, (6, 6), P0)
+    dt = single.estimate_dt()
+    single.step(dt, sync=False)
+    kh.step_blocks(blocks, dt, sync=False)
+    for _ in range(4):
+        single.step(-1.0, sync=False)
+        kh.step_blocks(blocks, -1.0, sync=False)
+    assert np.array_equal(_merge([g.get_prims() for g in blocks], 2, 1), single.get_prims())
+
+
+def test_link_validation(kh):
+    p = ki.config_params(5, n=(12, 12, 12))
+    parts, _ = _cut(p, 2, (6, 6))
+    import torch
+    stream = torch.cuda.Stream()
+    a, b = kh.Grid(parts[0], stream=stream.cuda_stream), kh.Grid(parts[1], stream=stream.cuda_stream)
+    with pytest.raises(kh.KharmError):
+        kh.link_blocks(a, b, 1)                              # not a KH_BC_BLOCK side
+    with pytest.raises(kh.KharmError):
+        kh.link_blocks(a, kh.Grid(parts[1]), 3)              # not on the same stream
+    kh.link_blocks(a, b, 3)
+    with pytest.raises(kh.KharmError):
+        kh.exchange_halos([a, b])                            # the periodic wrap (b, a) was never linked
+    with pytest.raises(kh.KharmError):
+        kh.Grid(dict(parts[0], fofc=1))                      # restrictions of linked blocks
+    c = kh.Grid(dict(parts[1], n1=10), stream=stream.cuda_stream)
+    with pytest.raises(kh.KharmError):
+        kh.link_blocks(a, c, 3)                              # transverse shapes differ
