@@ -45,6 +45,10 @@ WORKLOADS = {
     "torus_sane_192x128x128_weno5_drift": (3, None, None),        # same block, kh_params.floor_frame = KH_FRAME_DRIFT
     "torus_sane_192x128x128_weno5_facect": (3, None, None),       # same block, kh_params.transport = KH_B_FACE_CT
     "torus_sane_192x128x128_weno5_facect_upwind": (3, None, None),  # ... and kh_params.emf = KH_EMF_UPWIND
+    # the same block cut in x3 into two linked blocks of 192 x 128 x 64 with halo exchange (kh_step_blocks)
+    "torus_sane_192x128x128_weno5_2blocks": (3, None, None),
+    # two of the paper's weak-scaling units (128^3 per GPU) as linked blocks on one GPU: a 128 x 128 x 256 periodic box
+    "minkowski_2x128cubed_weno5_2blocks": (5, (128, 128, 256), 1),
     "minkowski_128_mc": (5, 128, 0), "minkowski_128_weno5": (5, 128, 1),
     "minkowski_256_mc": (5, 256, 0), "minkowski_256_weno5": (5, 256, 1),
     "minkowski_64_mc": (5, 64, 0), "minkowski_192_mc": (5, 192, 0), "minkowski_320_mc": (5, 320, 0),
@@ -345,6 +349,68 @@ class Ranks:
             self.dist = None
 
 
+def run_blocks(args, kh, p, P0, stream, R, cfg):
+    """`..._2blocks` workloads: the block cut in x3 into two linked blocks stepped by kh_step_blocks (halo exchange after
+    U -> P and after the fix-up, dt_next = minimum over the blocks).  Device-resident timing only (direct launches)."""
+    import torch
+    K, W = args.steps, max(args.warmup, 3)
+    n3 = p["n3"] // 2
+    dx3 = (p["xmax"][2] - p["xmin"][2]) / p["n3"]
+    parts = []
+    for m in range(2):
+        q = dict(p, n3=n3, xmin=list(p["xmin"]), xmax=list(p["xmax"]), bc=list(p["bc"]))
+        q["xmin"][2] = p["xmin"][2] + m * n3 * dx3
+        q["xmax"][2] = p["xmin"][2] + (m + 1) * n3 * dx3
+        q["bc"][4] = q["bc"][5] = kh.BC_BLOCK             # x3 is periodic in every bench workload: both sides are linked
+        parts.append(q)
+    with torch.cuda.stream(stream):
+        blocks = [kh.Grid(q, stream=stream.cuda_stream) for q in parts]
+        kh.link_blocks(blocks[0], blocks[1], 3)
+        kh.link_blocks(blocks[1], blocks[0], 3)
+        for m, g in enumerate(blocks):
+            g.set_prims(np.ascontiguousarray(P0[:, m * n3:(m + 1) * n3]))
+        kh.exchange_halos(blocks)
+        dt0 = min(g.estimate_dt() for g in blocks)
+        clocks = ClockSampler(R.local)
+        clocks.start()
+        kh.step_blocks(blocks, dt0, sync=False)
+        for _ in range(W - 1):
+            kh.step_blocks(blocks, -1.0, sync=False)
+        R.barrier()
+        l0 = sum(g.launch_count() for g in blocks)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(K):
+            kh.step_blocks(blocks, -1.0, sync=False)
+        e1.record(stream)
+        R.barrier()
+        ms_total = R.max(e0.elapsed_time(e1))
+        launches = sum(g.launch_count() for g in blocks) - l0
+        clk = clocks.stop()
+        assert all(np.isfinite(g.get_prims()).all() for g in blocks)
+        divb = max(g.divB() for g in blocks)
+    if R.rank != 0:
+        R.close()
+        return 0
+    zones = p["n1"] * p["n2"] * p["n3"]
+    hbm_peak, hbm_src, _ = load_peaks()
+    ms_step = ms_total / K
+    halo = 2 * 2 * 2 * 9 * 8 * 3 * (p["n1"] + 6) * (p["n2"] + 6)        # 2 sub-steps x 2 exchanges x 2 sides x (8 + flag) doubles x 3 layers
+    line = {"metric": "zone-cycles/sec (fp64 HARM step)", "value": R.world * zones * K / (ms_total * 1e-3), "unit": "zone-cycles/s",
+            "n_gpus": R.world, "steps": K, "warmup": W, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "baseline_config": cfg, "n1": p["n1"], "n2": p["n2"], "n3": p["n3"],
+                       "blocks": "2 linked blocks of %dx%dx%d on one GPU, cut in x3 (periodic: both sides exchange)" % (p["n1"], p["n2"], n3),
+                       "halo_bytes_per_block_step": halo, "launch": "direct launches (kh_step_blocks), device-resident dt"},
+            "clocks": clk, "gpu_launches": int(launches), "e2e": None,
+            "roofline_step": {"alg_bytes_per_zone_cycle": ALG_BYTES_PER_ZONE_STEP, "hbm_peak_gbs": hbm_peak,
+                              "frac_hbm": ALG_BYTES_PER_ZONE_STEP * zones / (ms_step * 1e-3) / 1e9 / hbm_peak},
+            "state": {"divB_max": divb}}
+    print(json.dumps(line))
+    R.close()
+    return 0
+
+
 def run_ours(args):
     import torch
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
@@ -361,6 +427,8 @@ def run_ours(args):
     K, W = args.steps, max(args.warmup, 3)
     barrier, max_over_ranks = R.barrier, R.max
 
+    if args.workload.endswith("_2blocks"):
+        return run_blocks(args, kh, p, P0, stream, R, cfg)
     with torch.cuda.stream(stream):
         g = kh.Grid(p, stream=stream.cuda_stream)
         g.set_prims(P0)

@@ -46,7 +46,7 @@ enum { KH_RECON_MC = 0, KH_RECON_WENO5 = 1 };                                 /*
 enum { KH_INV_1DW = 0, KH_INV_KASTAUN = 1 };
 enum { KH_FRAME_FLUID = 0, KH_FRAME_DRIFT = 1, KH_FRAME_NORMAL = 2 };
 enum { KH_B_FLUX_CT = 0, KH_B_FACE_CT = 1 };
-enum { KH_EMF_ARITHMETIC = 0, KH_EMF_UPWIND = 1 };
+enum { KH_EMF_ARITHMETIC = 0, KH_EMF_UPWIND = 1, KH_EMF_CENTRED = 2 };
 enum { KH_MEM_DEVICE = 0, KH_MEM_HOST = 1 };
 enum { KH_LOC_CENT = 0, KH_LOC_FACE1 = 1, KH_LOC_FACE2 = 2, KH_LOC_FACE3 = 3 };
 
@@ -72,8 +72,10 @@ typedef struct {
   int transport;              /* magnetic field transport: KH_B_FLUX_CT (zone-centred field, Toth's Flux-CT) |
                                  KH_B_FACE_CT (face-centred field advanced by the circulation of the edge EMFs;
                                  needs kh_set_face_B)                                                          */
-  int emf;                    /* edge EMFs of either transport ("with and without upwinding"): KH_EMF_ARITHMETIC
-                                 (four-point average of the face fluxes) | KH_EMF_UPWIND (contact-upwinded)     */
+  int emf;                    /* edge EMFs of either transport ("a number of schemes ... with and without upwinding"):
+                                 KH_EMF_ARITHMETIC (four-point average of the face fluxes) | KH_EMF_UPWIND (Gardiner & Stone,
+                                 contact-upwinded) | KH_EMF_CENTRED (Gardiner & Stone without upwinding: half the sum of the
+                                 four face values minus a quarter of the sum of the four zone-centred values)    */
 } kh_params;
 
 typedef struct kh_grid kh_grid;   /* opaque */
@@ -181,12 +183,14 @@ int kh_debug_predictor(kh_grid* g, double dt);
 long long kh_launch_count(const kh_grid* g);
 /* Enable/disable CUDA-graph replay of kh_step (default on); the first step after a change captures. */
 int kh_set_graph(kh_grid* g, int enable);
-/* Per-kernel device timing.  While enabled, kh_step enqueues its kernels directly (no graph replay) and
- * brackets every launch group with a CUDA-event pair on the grid's stream; kh_get_profile synchronises and
- * returns, per kernel kind (KH_K_*), the summed device milliseconds and the number of bracketed groups since
- * kh_set_profile(g, 1).  ms and count are HOST arrays of KH_K_COUNT entries.  Used by bench.py for the
- * per-kernel roofline; the bracketing serialises nothing (one stream) but adds two event records per launch,
- * so headline throughput is always measured with profiling off. */
+/* Per-kernel device timing.  While enabled, kh_step replays a second, instrumented CUDA graph of the step whose launch
+ * groups are bracketed by event-record nodes, and reads them out (synchronising) after every step, so the kernels are
+ * timed running exactly as in the product path; with graph replay off (kh_set_graph(g, 0)) the kernels are enqueued
+ * directly between event pairs.  A launch group is one kernel, except: the three flux directions of a sub-step, which run
+ * concurrently, are ONE group reported under KH_K_FLUX1 (KH_K_FLUX2 / 3 then stay empty); the fix-up's two kernels are one
+ * group.  kh_get_profile returns, per kind (KH_K_*), the summed device milliseconds and the number of groups since
+ * kh_set_profile(g, 1).  ms and count are HOST arrays of KH_K_COUNT entries.  Used by bench.py for the per-kernel roofline;
+ * headline throughput is always measured with profiling off. */
 enum { KH_K_FLUX1 = 0, KH_K_FLUX2 = 1, KH_K_FLUX3 = 2, KH_K_EMF = 3, KH_K_UPDATE = 4, KH_K_FILL = 5, KH_K_FIXUP = 6,
        KH_K_FOFC = 7 /* mask + re-flux of the first-order flux correction */, KH_K_COUNT = 8 };
 int kh_set_profile(kh_grid* g, int enable);

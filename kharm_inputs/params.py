@@ -15,7 +15,7 @@ RECON_MC, RECON_WENO5 = 0, 1
 INV_1DW, INV_KASTAUN = 0, 1
 FRAME_FLUID, FRAME_DRIFT, FRAME_NORMAL = 0, 1, 2
 B_FLUX_CT, B_FACE_CT = 0, 1
-EMF_ARITHMETIC, EMF_UPWIND = 0, 1
+EMF_ARITHMETIC, EMF_UPWIND, EMF_CENTRED = 0, 1, 2
 
 FLOOR_DEFAULTS = dict(rho_min=1e-6, u_min=1e-8, r_char=10.0, bsq_over_rho_max=100.0, bsq_over_u_max=1e4,
                       u_over_rho_max=100.0, gamma_max=50.0, dt_growth_max=1.3)

@@ -1,6 +1,10 @@
 """Build the CPU oracle (test infrastructure; see kho.h).
 
     python oracle/build.py            -> oracle/libkho.so (single thread) and oracle/libkho_omp.so
+    python oracle/build.py --sanitize -> also oracle/libkho_san.so (-fsanitize=address,undefined -O1 -g); the oracle tests
+                                         run against it with
+        KHO_SANITIZE=1 LD_PRELOAD=$(gcc -print-file-name=libasan.so):$(gcc -print-file-name=libubsan.so) \
+            ASAN_OPTIONS=detect_leaks=0 python -m pytest tests -m "not gpu" -q -k oracle
 
 Flags: -O2 -ffp-contract=off (no FMA contraction: the oracle's rounding is the plain IEEE one).
 The OpenMP build only parallelises zone-independent outer loops; results are bit-identical.
@@ -19,11 +23,14 @@ def _stale(target, sources):
     return any(os.path.getmtime(s) > t for s in sources)
 
 
-def build(verbose=False):
+def build(verbose=False, sanitize=False):
     src = [os.path.join(HERE, "kho.cpp"), os.path.join(HERE, "kho.h")]
     base = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-Wall", "-Wno-unused-variable"]
     outs = []
-    for name, extra in (("libkho.so", []), ("libkho_omp.so", ["-fopenmp"])):
+    variants = [("libkho.so", []), ("libkho_omp.so", ["-fopenmp"])]
+    if sanitize:
+        variants.append(("libkho_san.so", ["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"]))
+    for name, extra in variants:
         out = os.path.join(HERE, name)
         if _stale(out, src):
             cmd = base + extra + ["-o", out, src[0]]
@@ -35,5 +42,5 @@ def build(verbose=False):
 
 
 if __name__ == "__main__":
-    build(verbose=True)
+    build(verbose=True, sanitize="--sanitize" in sys.argv)
     sys.exit(0)

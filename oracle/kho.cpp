@@ -930,6 +930,46 @@ void emf_upwind(const kho_grid& g, const double* Ps, const double* F1, const dou
 }
 
 // C9. Fix-up of failed inversions (S19) followed by floors.
+// Edge EMFs of Gardiner & Stone's un-upwinded scheme (their "E-circle"; "a number of schemes for
+// determining the EMFs along zone edges with and without upwinding"; S30): the four-point face average corrected by
+// the zone-centred reference values,
+//   eps_c(edge) = 1/2 (sum of the four face values) - 1/4 (sum of the four zone-centred values around the edge),
+// with the face values eps_c = F^a[B^b] = -F^b[B^a] and the centred ones sqrt(-g) (B^b v^a - B^a v^b), v^i = u^i / u^t, (c, a, b)
+// cyclic.  It is what the upwinded scheme's general form gives when both candidate gradients are averaged at every face; it
+// has the correct limit for plane-parallel, grid-aligned flow (the edge sees the one-dimensional face value), which the plain
+// arithmetic average lacks, and no dependence on the direction of the flow.  Written out from this closed form, not through
+// emf_upwind().
+void emf_centred(const kho_grid& g, const double* Ps, const double* F1, const double* F2, const double* F3, double* e1, double* e2, double* e3) {
+  const long nt = g.ntot;
+  const long st[3] = {1, g.nt[0], (long)g.nt[0] * g.nt[1]};
+  const double* F[3] = {F1, F2, F3};
+  double* E[3] = {e1, e2, e3};
+  for (int c = 0; c < 3; c++) {
+    const int a = (c + 1) % 3, b = (c + 2) % 3;
+    const long sa = st[a], sb = st[b];
+    std::vector<double> ec(nt, 0.0);
+    for (int k = -1; k <= g.n[2]; k++) for (int j = -1; j <= g.n[1]; j++) for (int i = -1; i <= g.n[0]; i++) {
+      long n = g.idx(i, j, k);
+      const Geom& G = g.G[0][g.idx2(i, j)];
+      double P[NP];
+      get_prim(g, Ps, n, P);
+      FourVec D;
+      four_vectors(G.gcov, G.gcon, P, D);
+      ec[n] = G.gdet * (P[B1 + b] * D.ucon[1 + a] - P[B1 + a] * D.ucon[1 + b]) / D.ucon[0];
+    }
+    int hi[3] = {g.n[0] + 1, g.n[1] + 1, g.n[2] + 1};
+    hi[c] = g.n[c];
+    for (int k = 0; k < hi[2]; k++) for (int j = 0; j < hi[1]; j++) for (int i = 0; i < hi[0]; i++) {
+      long n = g.idx(i, j, k);
+      double faces = F[a][(B1 + b) * nt + n] + F[a][(B1 + b) * nt + n - sb] - F[b][(B1 + a) * nt + n] - F[b][(B1 + a) * nt + n - sa];
+      double centres = ec[n] + ec[n - sa] + ec[n - sb] + ec[n - sa - sb];
+      double v = 0.5 * faces - 0.25 * centres;
+      if (c != 1 && polar_face(g, j)) v = 0.0;             // S10
+      E[c][n] = v;
+    }
+  }
+}
+
 void fixup(kho_grid& g, double* Pf) {
   std::vector<double> snap(Pf, Pf + 5 * g.ntot);   // hydro primitives, pre-fix-up snapshot
   for (int k = 0; k < g.n[2]; k++) for (int j = 0; j < g.n[1]; j++) for (int i = 0; i < g.n[0]; i++) {
@@ -1041,7 +1081,8 @@ void substep(kho_grid& g, const double* Pi, const double* Ps, double* Pf, double
     // speculative update with the high-order fluxes: which zones would fail the inversion or hit a floor?
     std::vector<double> raw[3] = {g.F[0], g.F[1], g.F[2]};                      // flux_ct rewrites the B components in place
     if (g.p.emf == KHO_EMF_UPWIND) emf_upwind(g, Ps, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data());
-    flux_ct(g, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data(), g.p.emf == KHO_EMF_UPWIND);
+    if (g.p.emf == KHO_EMF_CENTRED) emf_centred(g, Ps, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data());
+    flux_ct(g, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data(), g.p.emf != KHO_EMF_ARITHMETIC);
     if (Pf != Pi) std::memcpy(Pf, Pi, sizeof(double) * NP * nt);
     update_zones(g, Pi, Ps, Pf, Dt);
     std::vector<int> mask(nt, 0);
@@ -1051,7 +1092,8 @@ void substep(kho_grid& g, const double* Pi, const double* Ps, double* Pf, double
     fofc_reflux(g, Ps, mask);
   }
   if (g.p.emf == KHO_EMF_UPWIND) emf_upwind(g, Ps, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data());
-  flux_ct(g, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data(), g.p.emf == KHO_EMF_UPWIND);
+  if (g.p.emf == KHO_EMF_CENTRED) emf_centred(g, Ps, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data());
+  flux_ct(g, g.F[0].data(), g.F[1].data(), g.F[2].data(), g.emf[0].data(), g.emf[1].data(), g.emf[2].data(), g.p.emf != KHO_EMF_ARITHMETIC);
   if (Pf != Pi) std::memcpy(Pf, Pi, sizeof(double) * NP * nt);   // ghosts of Pf start from Pi (matters for FIXED)
   if (Bfi) face_ct_update(g, Bfi, Bff, Dt);
   update_zones(g, Pi, Ps, Pf, Dt, Bfi ? Bff : nullptr);
@@ -1346,6 +1388,8 @@ int kho_debug_emf(kho_grid* g) {
   for (int d = 0; d < 3; d++) compute_flux(*g, P, d);
   if (g->p.emf == KHO_EMF_UPWIND) {
     emf_upwind(*g, P, g->F[0].data(), g->F[1].data(), g->F[2].data(), g->emf[0].data(), g->emf[1].data(), g->emf[2].data());
+  } else if (g->p.emf == KHO_EMF_CENTRED) {
+    emf_centred(*g, P, g->F[0].data(), g->F[1].data(), g->F[2].data(), g->emf[0].data(), g->emf[1].data(), g->emf[2].data());
   } else {
     std::vector<double> raw[3] = {g->F[0], g->F[1], g->F[2]};
     flux_ct(*g, g->F[0].data(), g->F[1].data(), g->F[2].data(), g->emf[0].data(), g->emf[1].data(), g->emf[2].data());

@@ -27,7 +27,7 @@ enum { KHO_RECON_MC = 0, KHO_RECON_WENO5 = 1 };
 enum { KHO_INV_1DW = 0, KHO_INV_KASTAUN = 1 };
 enum { KHO_FRAME_FLUID = 0, KHO_FRAME_DRIFT = 1, KHO_FRAME_NORMAL = 2 };
 enum { KHO_B_FLUX_CT = 0, KHO_B_FACE_CT = 1 };
-enum { KHO_EMF_ARITHMETIC = 0, KHO_EMF_UPWIND = 1 };
+enum { KHO_EMF_ARITHMETIC = 0, KHO_EMF_UPWIND = 1, KHO_EMF_CENTRED = 2 };
 enum { KHO_LOC_CENT = 0, KHO_LOC_FACE1 = 1, KHO_LOC_FACE2 = 2, KHO_LOC_FACE3 = 3 };
 
 typedef struct {
@@ -45,7 +45,7 @@ typedef struct {
   int fofc;                                        /* 1: first-order flux correction (NEXT-3) */
   int floor_frame;                                 /* KHO_FRAME_FLUID | _DRIFT | _NORMAL (NEXT-4) */
   int transport;                                   /* KHO_B_FLUX_CT | KHO_B_FACE_CT (NEXT-1) */
-  int emf;                                         /* KHO_EMF_ARITHMETIC | KHO_EMF_UPWIND (NEXT-1) */
+  int emf;                                         /* KHO_EMF_ARITHMETIC | KHO_EMF_UPWIND | KHO_EMF_CENTRED (NEXT-1) */
 } kho_params;
 
 typedef struct kho_grid kho_grid;

@@ -56,8 +56,9 @@ def _ptr(a):
 def lib(omp=False):
     key = "omp" if omp else "st"
     if key not in _libs:
-        paths = _build.build()
-        L = C.CDLL(paths[1] if omp else paths[0])
+        san = os.environ.get("KHO_SANITIZE") == "1"        # the ASan / UBSan build of the same source (oracle/build.py --sanitize)
+        paths = _build.build(sanitize=san)
+        L = C.CDLL(paths[2] if san else (paths[1] if omp else paths[0]))
         L.kho_strerror.restype = C.c_char_p
         for name in ("kho_embed", "kho_metric", "kho_conn", "kho_conn_fd", "kho_fourvec", "kho_prim_to_flux",
                      "kho_stress", "kho_vchar", "kho_recon", "kho_llf", "kho_source"):

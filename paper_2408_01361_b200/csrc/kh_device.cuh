@@ -589,7 +589,7 @@ __device__ __forceinline__ bool kastaun_root(const KastaunC& c, double a, double
 }
 
 template <bool FLAT>
-__device__ __forceinline__ int u_to_p_kastaun_floors(const Geo& G, const double Uh[KH_NP], double gam, const FloorPar& fp, int frame,
+__device__ __forceinline__ int u_to_p_kastaun_floors(const Geo& G, const double Uh[KH_NP], double mu0, double gam, const FloorPar& fp, int frame,
                                                      double rho_g, double u_g, double Pout[KH_NP], int& fflag, double inj[2]) {
   fflag = 0;
   Pout[B1] = Uh[B1]; Pout[B2] = Uh[B2]; Pout[B3] = Uh[B3];
@@ -637,14 +637,31 @@ __device__ __forceinline__ int u_to_p_kastaun_floors(const Geo& G, const double 
     }
   }
   double vr, W, er, omv;
-  const double f0 = kastaun_f(c, 0.0, vr, W, er, omv);
-  const double f1 = kastaun_f(c, mu_hi, vr, W, er, omv);
   double mu;
-  if (!(f0 < 0.0) || !isfinite(f1)) return 2;
-  if (f1 <= 0.0) mu = mu_hi;
-  else {
-    if (!kastaun_root<false>(c, 0.0, f0, mu_hi, f1, lo, hi)) return 2;
-    mu = 0.5 * (lo + hi);
+  // A bracket around the guess first (mu0 = 1/(W h) of the guess primitives): the master function has exactly one root in
+  // (0, mu_+] and is negative below it, positive above, so f(a) < 0 < f(b) with 0 < a < b <= mu_+ encloses THE root and the
+  // end-point evaluations f(0), f(mu_+) (with their flag semantics) are implied.  The root find converges to the same
+  // 4e-16 bracket from any start (S24): the result does not depend on the guess; only the number of evaluations does.
+  bool bracketed = false;
+  if (mu0 > 0.0 && mu0 < mu_hi) {
+    double a = mu0 * (1.0 - 4e-3), b = mu0 * (1.0 + 4e-3);
+    if (b > mu_hi) b = mu_hi;
+    const double fa = kastaun_f(c, a, vr, W, er, omv), fb = kastaun_f(c, b, vr, W, er, omv);
+    if (fa < 0.0 && fb > 0.0) {
+      if (!kastaun_root<false>(c, a, fa, b, fb, lo, hi)) return 2;
+      mu = 0.5 * (lo + hi);
+      bracketed = true;
+    }
+  }
+  if (!bracketed) {
+    const double f0 = kastaun_f(c, 0.0, vr, W, er, omv);
+    const double f1 = kastaun_f(c, mu_hi, vr, W, er, omv);
+    if (!(f0 < 0.0) || !isfinite(f1)) return 2;
+    if (f1 <= 0.0) mu = mu_hi;
+    else {
+      if (!kastaun_root<false>(c, 0.0, f0, mu_hi, f1, lo, hi)) return 2;
+      mu = 0.5 * (lo + hi);
+    }
   }
   double vsq_raw, eps_raw;
   kastaun_f(c, mu, vsq_raw, W, eps_raw, omv);
@@ -667,7 +684,8 @@ __device__ __forceinline__ int u_to_p_kastaun_floors(const Geo& G, const double 
 }
 
 // ---------------------------------------------------------------------------------------------
-// Inversion + floors with the injection frame resolved.  INVERTER: 0 1D_W, 1 Kastaun.  Frame 2 (normal observer, S27):
+// Inversion + floors with the injection frame resolved.  INVERTER: 0 1D_W, 1 Kastaun.  W0: the guess -- for 1D_W
+// W0 = (rho + Gamma u) gamma^2 of the guess primitives, for Kastaun mu0 = 1/(W h) = rho / ((rho + Gamma u) gamma) (<= 0: none).  Frame 2 (normal observer, S27):
 // the floor material enters as conserved variables of a gas at rest for the normal observer,
 //   U_add/sqrt(-g) = (rho_inj/alpha, -(rho_inj + u_inj) + rho_inj/alpha, 0, 0, 0), and the sum is inverted again (guess: the
 // fluid-frame result; the fluid-frame limits and ceilings act on the new state).  A failed re-inversion keeps the
@@ -677,7 +695,7 @@ template <bool FLAT, int INVERTER>
 __device__ __forceinline__ int invert_any(const Geo& G, const double Uh[KH_NP], double W0, double gam, const FloorPar& fp, int frame,
                                           double rho_g, double u_g, double Pout[KH_NP], int& fflag, double inj[2]) {
   if (INVERTER == 0) return u_to_p_floors<FLAT>(G, Uh, W0, gam, fp, frame, rho_g, u_g, Pout, fflag, inj);
-  return u_to_p_kastaun_floors<FLAT>(G, Uh, gam, fp, frame, rho_g, u_g, Pout, fflag, inj);
+  return u_to_p_kastaun_floors<FLAT>(G, Uh, W0, gam, fp, frame, rho_g, u_g, Pout, fflag, inj);     // W0 carries mu0 for this inverter
 }
 
 template <bool FLAT, int INVERTER>
@@ -692,7 +710,8 @@ __device__ __forceinline__ int invert_with_floors(const Geo& G, const double Uh[
   for (int v = 0; v < KH_NP; v++) Ub[v] = Uh[v];
   Ub[RHO] = fma(inj[0], ialpha, Ub[RHO]);
   Ub[UU] += fma(inj[0], ialpha, -(inj[0] + inj[1]));
-  const double W0b = fma(gam, Pout[UU], Pout[RHO]) * (1.0 + spatial_norm2<FLAT>(G, Pout[U1], Pout[U2], Pout[U3]));
+  const double xb = 1.0 + spatial_norm2<FLAT>(G, Pout[U1], Pout[U2], Pout[U3]), efb = fma(gam, Pout[UU], Pout[RHO]);
+  const double W0b = INVERTER == 0 ? efb * xb : Pout[RHO] / (efb * sqrt(xb));
   int ff2;
   const int p2 = invert_any<FLAT, INVERTER>(G, Ub, W0b, gam, fp, 0, rho_g, u_g, Pb, ff2, inj2);
   if (p2 != 0) { fflag |= 64; return 0; }

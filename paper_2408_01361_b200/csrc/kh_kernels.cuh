@@ -298,20 +298,24 @@ ecent_kernel(GV g, const double* __restrict__ P, double* __restrict__ c1, double
 }
 
 // upwind choice by the mass flux M through the face between the two candidates; |M| <= 1e-10 of the two zones' conserved
-// densities is "no flow" (often an exact zero by symmetry, whose computed sign would be round-off noise): the mean
+// densities is "no flow" (often an exact zero by symmetry, whose computed sign would be round-off noise): the mean.
+// CENTRED (KH_EMF_CENTRED, Gardiner & Stone's un-upwinded scheme, S30): always the mean -- the edge value then is
+// 1/2 (sum of the four face values) - 1/4 (sum of the four zone-centred values).
+template <bool CENTRED>
 __device__ __forceinline__ double upw(double lo, double hi, double M, double Dsum) {
+  if (CENTRED) return 0.5 * (lo + hi);
   const double t = 1e-10 * Dsum;
   return M > t ? lo : (M < -t ? hi : 0.5 * (lo + hi));
 }
 
 // one edge value: Fa = F^a (component B^b is +eps), Fb = F^b (component B^a is -eps), ec the zone-centred table
+template <bool CENTRED>
 __device__ __forceinline__ double edge_emf_upwind(const double* __restrict__ Fa, const double* __restrict__ Fb, const double* __restrict__ ec,
                                                   const double* __restrict__ dc, long nt, long n, long sa, long sb, int vb /* B^b slot */,
                                                   int va /* B^a slot */) {
   const double* fa = Fa + (long)vb * nt;
   const double* fb = Fb + (long)va * nt;
-  const double efa0 = fa[n], efa_b = fa[n - sb], efa_ab = 0.0;
-  (void)efa_ab;
+  const double efa0 = fa[n], efa_b = fa[n - sb];
   const double efb0 = -fb[n], efb_a = -fb[n - sa];
   const double ec0 = ec[n], ec_a = ec[n - sa], ec_b = ec[n - sb], ec_ab = ec[n - sa - sb];
   // gradients along b (at columns n - sa and n), below (m) and above (p) the b-faces
@@ -320,12 +324,17 @@ __device__ __forceinline__ double edge_emf_upwind(const double* __restrict__ Fa,
   // gradients along a (at rows n - sb and n)
   const double dam_lo = 2.0 * (efa_b - ec_ab), dam_hi = 2.0 * (efa0 - ec_a);
   const double dap_lo = 2.0 * (ec_b - efa_b), dap_hi = 2.0 * (ec0 - efa0);
-  const double Ma0 = Fa[n], Ma1 = Fa[n - sb], Mb0 = Fb[n], Mb1 = Fb[n - sa];            // mass fluxes (slot RHO = 0)
-  const double d0 = dc[n], d_a = dc[n - sa], d_b = dc[n - sb], d_ab = dc[n - sa - sb];
-  return 0.25 * (efa0 + efa_b + efb0 + efb_a) + 0.125 * (upw(dbm_lo, dbm_hi, Ma1, d_ab + d_b) - upw(dbp_lo, dbp_hi, Ma0, d_a + d0)) +
-         0.125 * (upw(dam_lo, dam_hi, Mb1, d_ab + d_a) - upw(dap_lo, dap_hi, Mb0, d_b + d0));
+  double Ma0 = 0.0, Ma1 = 0.0, Mb0 = 0.0, Mb1 = 0.0, d0 = 0.0, d_a = 0.0, d_b = 0.0, d_ab = 0.0;
+  if (!CENTRED) {
+    Ma0 = Fa[n]; Ma1 = Fa[n - sb]; Mb0 = Fb[n]; Mb1 = Fb[n - sa];                        // mass fluxes (slot RHO = 0)
+    d0 = dc[n]; d_a = dc[n - sa]; d_b = dc[n - sb]; d_ab = dc[n - sa - sb];
+  }
+  return 0.25 * (efa0 + efa_b + efb0 + efb_a) +
+         0.125 * (upw<CENTRED>(dbm_lo, dbm_hi, Ma1, d_ab + d_b) - upw<CENTRED>(dbp_lo, dbp_hi, Ma0, d_a + d0)) +
+         0.125 * (upw<CENTRED>(dam_lo, dam_hi, Mb1, d_ab + d_a) - upw<CENTRED>(dap_lo, dap_hi, Mb0, d_b + d0));
 }
 
+template <bool CENTRED>
 __global__ void __launch_bounds__(128)
 emf_upwind_kernel(GV g, const double* __restrict__ F1, const double* __restrict__ F2, const double* __restrict__ F3,
                   const double* __restrict__ c1, const double* __restrict__ c2, const double* __restrict__ c3, const double* __restrict__ dc,
@@ -336,9 +345,9 @@ emf_upwind_kernel(GV g, const double* __restrict__ F1, const double* __restrict_
   const long n = zidx(g, i, j, k), nt = g.ntot;
   const bool axis = polar_face(g, j);
   // (c; a, b) cyclic: eps_3 = F^1[B^2] = -F^2[B^1];  eps_1 = F^2[B^3] = -F^3[B^2];  eps_2 = F^3[B^1] = -F^1[B^3]
-  if (k < g.n3) { double v = edge_emf_upwind(F1, F2, c3, dc, nt, n, 1, g.s2, B2, B1); e3[n] = axis ? 0.0 : v; }
-  if (j < g.n2) { double v = edge_emf_upwind(F3, F1, c2, dc, nt, n, g.s3, 1, B1, B3); e2[n] = v; }
-  if (i < g.n1) { double v = edge_emf_upwind(F2, F3, c1, dc, nt, n, g.s2, g.s3, B3, B2); e1[n] = axis ? 0.0 : v; }
+  if (k < g.n3) { double v = edge_emf_upwind<CENTRED>(F1, F2, c3, dc, nt, n, 1, g.s2, B2, B1); e3[n] = axis ? 0.0 : v; }
+  if (j < g.n2) { double v = edge_emf_upwind<CENTRED>(F3, F1, c2, dc, nt, n, g.s3, 1, B1, B3); e2[n] = v; }
+  if (i < g.n1) { double v = edge_emf_upwind<CENTRED>(F2, F3, c1, dc, nt, n, g.s2, g.s3, B3, B2); e1[n] = axis ? 0.0 : v; }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -507,7 +516,7 @@ __device__ __forceinline__ void update_zone_a(const GV& g, const ACC& A, const G
     double ee = ef + D.bsq, ptot = fma(0.5, D.bsq, pg);
     double eu[4] = {ee * D.ucov[0], ee * D.ucov[1], ee * D.ucov[2], ee * D.ucov[3]};
     flux_row(pi, D, eu, ptot, 0, Uh);
-    W0 = ef * D.x;
+    W0 = (MODE & 1) ? pi[RHO] * fast_rsqrt(D.x) * fast_rcp(ef) : ef * D.x;      // the inverter's guess: mu0 = 1/(W h) (Kastaun) or W0 (1D_W)
     if (!FLAT) {
       double ps[KH_NP];
       if (CORR) {
@@ -977,10 +986,10 @@ fixup_apply_kernel(GV g, double* __restrict__ Pf, const unsigned* __restrict__ l
       flux_row(P0, D, eu, ptot, 0, Uh);
       Uh[RHO] = fma(inj[0], ialpha, Uh[RHO]);
       Uh[UU] += fma(inj[0], ialpha, -(inj[0] + inj[1]));
-      const double W0b = fma(g.gam, P[UU], P[RHO]) * (1.0 + spatial_norm2<FLAT>(G, P[U1], P[U2], P[U3]));
+      const double xb = 1.0 + spatial_norm2<FLAT>(G, P[U1], P[U2], P[U3]), efb = fma(g.gam, P[UU], P[RHO]);
       int ff2;
-      const int p2 = g.inverter ? invert_any<FLAT, 1>(G, Uh, W0b, g.gam, g.fp, 0, rho_g, u_g, Pb, ff2, inj2)
-                                : invert_any<FLAT, 0>(G, Uh, W0b, g.gam, g.fp, 0, rho_g, u_g, Pb, ff2, inj2);
+      const int p2 = g.inverter ? invert_any<FLAT, 1>(G, Uh, P[RHO] / (efb * sqrt(xb)), g.gam, g.fp, 0, rho_g, u_g, Pb, ff2, inj2)
+                                : invert_any<FLAT, 0>(G, Uh, efb * xb, g.gam, g.fp, 0, rho_g, u_g, Pb, ff2, inj2);
       if (p2 != 0) ff |= 64;
       else {
 #pragma unroll

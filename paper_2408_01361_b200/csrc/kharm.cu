@@ -25,6 +25,8 @@ static thread_local char g_cuda_err[256] = "";
     }                                                                                              \
   } while (0)
 
+enum { KH_GP_MAX = 64 };
+
 struct kh_grid {
   kh_params p;
   GV gv;
@@ -78,6 +80,14 @@ struct kh_grid {
   int march_J;                // 0 = chosen by march_chunk()
   double prof_ms[KH_K_COUNT];
   long long prof_n[KH_K_COUNT];
+  // profiling INSIDE the step's graph: event-record nodes (cudaEventRecordExternal) around every launch group of a second,
+  // instrumented graph per rotation state, read out after each replay -- the timed kernels then run exactly as in the product
+  // path (the concurrent flux directions overlap as they do there; direct launches bracketed by events do not reproduce that)
+  cudaGraphExec_t gexec_prof[3];
+  cudaEvent_t gpev[3][KH_GP_MAX][2];
+  int gpkind[3][KH_GP_MAX];
+  int gpn[3];
+  int gp_capture;             // rotation state + 1 while an instrumented graph is being captured, else 0
 };
 
 enum { KH_PROF_POOL = 2048 };
@@ -97,12 +107,27 @@ static void prof_flush(kh_grid* g) {
 // bracket one launch: PROF_BEGIN(kind); kernel<<<...>>>(...); PROF_END();
 static inline void prof_begin(kh_grid* g, int kind) {
   if (!g->profile) return;
+  if (g->gp_capture) {
+    const int c = g->gp_capture - 1, r = g->gpn[c];
+    if (r >= KH_GP_MAX) return;
+    if (!g->gpev[c][r][0]) { cudaEventCreate(&g->gpev[c][r][0]); cudaEventCreate(&g->gpev[c][r][1]); }
+    g->gpkind[c][r] = kind;
+    cudaEventRecordWithFlags(g->gpev[c][r][0], g->stream, cudaEventRecordExternal);
+    return;
+  }
   if (g->npev == KH_PROF_POOL) prof_flush(g);
   g->pkind[g->npev] = kind;
   cudaEventRecord(g->pev[2 * g->npev], g->stream);
 }
 static inline void prof_end(kh_grid* g) {
   if (!g->profile) return;
+  if (g->gp_capture) {
+    const int c = g->gp_capture - 1, r = g->gpn[c];
+    if (r >= KH_GP_MAX) return;
+    cudaEventRecordWithFlags(g->gpev[c][r][1], g->stream, cudaEventRecordExternal);
+    g->gpn[c]++;
+    return;
+  }
   cudaEventRecord(g->pev[2 * g->npev + 1], g->stream);
   g->npev++;
 }
@@ -261,11 +286,15 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
   const int passes = g->p.fofc ? 2 : 1;       // FOFC: a speculative update first, then the re-flux, then the real one
   for (int pass = 0; pass < passes; pass++) {
     prof_begin(g, KH_K_EMF);
-    if (g->p.emf == KH_EMF_UPWIND) {
+    if (g->p.emf != KH_EMF_ARITHMETIC) {
       if (g->flat) ecent_kernel<true><<<zone_grid(v.n1 + 2, v.n2 + 2, v.n3 + 2), 128, 0, g->stream>>>(v, Ps, g->ecent[0], g->ecent[1], g->ecent[2], g->ecent[3]);
       else ecent_kernel<false><<<zone_grid(v.n1 + 2, v.n2 + 2, v.n3 + 2), 128, 0, g->stream>>>(v, Ps, g->ecent[0], g->ecent[1], g->ecent[2], g->ecent[3]);
-      emf_upwind_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, g->F[0], g->F[1], g->F[2], g->ecent[0], g->ecent[1],
-                                                                                          g->ecent[2], g->ecent[3], g->emf[0], g->emf[1], g->emf[2]);
+      if (g->p.emf == KH_EMF_UPWIND)
+        emf_upwind_kernel<false><<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, g->F[0], g->F[1], g->F[2], g->ecent[0], g->ecent[1],
+                                                                                                 g->ecent[2], g->ecent[3], g->emf[0], g->emf[1], g->emf[2]);
+      else
+        emf_upwind_kernel<true><<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, g->F[0], g->F[1], g->F[2], g->ecent[0], g->ecent[1],
+                                                                                                g->ecent[2], g->ecent[3], g->emf[0], g->emf[1], g->emf[2]);
       g->launches++;
     } else {
       emf_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], g->emf[2]);
@@ -365,8 +394,11 @@ static int enter(kh_grid* g) {
 #define ENTER(g) do { int rc_ = enter(g); if (rc_) return rc_; } while (0)
 
 static void destroy_graphs(kh_grid* g) {
-  for (int c = 0; c < 3; c++)
+  for (int c = 0; c < 3; c++) {
     if (g->gexec[c]) { cudaGraphExecDestroy(g->gexec[c]); g->gexec[c] = nullptr; }
+    if (g->gexec_prof[c]) { cudaGraphExecDestroy(g->gexec_prof[c]); g->gexec_prof[c] = nullptr; }
+    g->gpn[c] = 0;
+  }
 }
 
 // The zone arrays start ONE DOUBLE past the (256 B aligned) allocation: with 3 ghost zones per side, interior zone i = 0 of every
@@ -414,7 +446,7 @@ int kh_grid_destroy(kh_grid* g) {
 int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   if (!p || !out) return KH_EINVAL;
   if (p->n1 < 1 || p->n2 < 1 || p->n3 < 1) return KH_EINVAL;
-  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1 || p->inverter < 0 || p->inverter > 1 || p->fofc < 0 || p->fofc > 1 || p->floor_frame < 0 || p->floor_frame > 2 || p->transport < 0 || p->transport > 1 || p->emf < 0 || p->emf > 1) return KH_EINVAL;
+  if (p->coords < 0 || p->coords > 2 || p->recon < 0 || p->recon > 1 || p->inverter < 0 || p->inverter > 1 || p->fofc < 0 || p->fofc > 1 || p->floor_frame < 0 || p->floor_frame > 2 || p->transport < 0 || p->transport > 1 || p->emf < 0 || p->emf > 2) return KH_EINVAL;
   if (!(p->gamma > 1.0) || !(p->cfl > 0.0) || !(p->dt_growth_max > 0.0)) return KH_EINVAL;
   const int N[3] = {p->n1, p->n2, p->n3};
   for (int d = 0; d < 3; d++) {
@@ -524,7 +556,7 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   ALLOC(g->fflag, v.ntot);
   if (p->fofc) ALLOC(g->mask, v.ntot);
   if (p->transport == KH_B_FACE_CT) for (int b = 0; b < 3; b++) for (int d = 0; d < 3; d++) ALLOC_SHIFTED(g->Bf[b][d], fb);
-  if (p->emf == KH_EMF_UPWIND) for (int d = 0; d < 4; d++) ALLOC(g->ecent[d], fb);
+  if (p->emf != KH_EMF_ARITHMETIC) for (int d = 0; d < 4; d++) ALLOC(g->ecent[d], fb);
   ALLOC(g->faillist, sizeof(unsigned) * (size_t)v.n1 * v.n2 * v.n3);
   ALLOC(g->sc, sizeof(StepScalars));
 #undef ALLOC_SHIFTED
@@ -692,8 +724,9 @@ int kh_step(kh_grid* g, double dt, double* dt_next) {
   CK(cudaGetLastError());
   int cur = g->cur;
   bool replayed = false;
-  if (g->use_graph && !g->profile) {
-    if (!g->gexec[cur]) {
+  if (g->use_graph) {
+    cudaGraphExec_t* slot = g->profile ? &g->gexec_prof[cur] : &g->gexec[cur];
+    if (!*slot) {
       // Capture one step.  Any failure (a stream that cannot be captured, a capture already active on it, ...) switches
       // this grid to direct launches for good: the same kernels, enqueued one by one.
       const long long before = g->launches;
@@ -701,23 +734,35 @@ int kh_step(kh_grid* g, double dt, double* dt_next) {
       cudaError_t e = cudaStreamBeginCapture(g->stream, cudaStreamCaptureModeThreadLocal);
       int rc = KH_OK;
       if (e == cudaSuccess) {
+        if (g->profile) { g->gp_capture = cur + 1; g->gpn[cur] = 0; }
         rc = enqueue_step(g, cur);
+        g->gp_capture = 0;
         e = cudaStreamEndCapture(g->stream, &graph);
         g->graph_launches = g->launches - before;
         g->launches = before;
-        if (e == cudaSuccess && rc == KH_OK) e = cudaGraphInstantiate(&g->gexec[cur], graph, 0);
+        if (e == cudaSuccess && rc == KH_OK) e = cudaGraphInstantiate(slot, graph, 0);
         if (graph) cudaGraphDestroy(graph);
       }
       if (e != cudaSuccess || rc != KH_OK) {
         cudaGetLastError();
-        if (g->gexec[cur]) { cudaGraphExecDestroy(g->gexec[cur]); g->gexec[cur] = nullptr; }
+        if (*slot) { cudaGraphExecDestroy(*slot); *slot = nullptr; }
         g->use_graph = false;
       }
     }
-    if (g->gexec[cur]) {
-      CK(cudaGraphLaunch(g->gexec[cur], g->stream));
+    if (*slot) {
+      CK(cudaGraphLaunch(*slot, g->stream));
       g->launches += g->graph_launches;
       replayed = true;
+      if (g->profile) {           // read the event nodes of this replay out before the next one overwrites them
+        CK(cudaStreamSynchronize(g->stream));
+        for (int r = 0; r < g->gpn[cur]; r++) {
+          float ms = 0.f;
+          if (cudaEventElapsedTime(&ms, g->gpev[cur][r][0], g->gpev[cur][r][1]) == cudaSuccess) {
+            g->prof_ms[g->gpkind[cur][r]] += ms;
+            g->prof_n[g->gpkind[cur][r]]++;
+          }
+        }
+      }
     }
   }
   if (!replayed) {

@@ -85,3 +85,21 @@ def l1_diff(p, got, ref):
             gii = np.sqrt(gcov[..., i + 1, i + 1])[None]
             out[base + i] = (np.abs(got[base + i] - ref[base + i]) * gii).sum() / max(norm, 1e-300)
     return out
+
+
+def bondi_errors(p, P1, P0, rmin=2.5):
+    """Config 2 ("error against the analytic steady state"): L1 difference between a state and the analytic initial
+    state over the zones with r > rmin (outside the horizon and its boundary layer), [rho, u, velocity, field] -- scalars
+    relative to sum |ref|, vectors as sum sqrt(g_ii) |d v^i| over i relative to the sum of the vector's norm (S23)."""
+    x1, _, _ = geometry.zone_coords(p)
+    keep = np.exp(x1) > rmin
+    gcov = zone_metric(p)
+    out = []
+    for v in (0, 1):
+        out.append(np.abs(P1[v] - P0[v])[..., keep].sum() / np.abs(P0[v])[..., keep].sum())
+    for base in (2, 5):
+        vec = np.moveaxis(P0[base:base + 3], 0, -1)
+        norm = np.sqrt(np.einsum("kjia,jiab,kjib->kji", vec, gcov[..., 1:, 1:], vec))[..., keep].sum()
+        num = sum((np.abs(P1[base + i] - P0[base + i]) * np.sqrt(gcov[..., i + 1, i + 1])[None])[..., keep].sum() for i in range(3))
+        out.append(num / norm)
+    return np.array(out)

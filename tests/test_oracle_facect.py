@@ -181,6 +181,71 @@ def test_upwinded_emf_keeps_second_order_convergence_of_a_rotated_mode(kho):
     assert 1.7 < slope < 2.4, (errs, slope)
 
 
+# ------------------------------------------------------------------------------------------ un-upwinded Gardiner-Stone EMF (S30)
+def test_centred_emf_design_condition_uniform_state_and_difference_from_the_other_two(kho):
+    """KH_EMF_CENTRED = 1/2 (faces) - 1/4 (centres): (1) plane-parallel flow along each grid direction sees the
+    one-dimensional face value at the edge (the design condition the arithmetic average fails); (2) a uniform state gives
+    the zone-centred value; (3) it does not depend on the direction of the flow the way the upwinded scheme does: for
+    grid-aligned 1-D flow all three agree with (1) except the arithmetic one, for a 3-D state all three differ."""
+    p0 = ki.config_params(5, n=(12, 10, 8), recon=kp.RECON_WENO5)
+    I = (slice(NG, -NG),) * 3
+    for d in (1, 2, 3):
+        g = kho.Grid(dict(p0, emf=kp.EMF_CENTRED))
+        g.set_prims(_one_d_state(p0, d, seed=d))
+        g.debug_emf()
+        F, _ = g.get_flux(d)
+        a, b = d % 3 + 1, (d + 1) % 3 + 1
+        assert np.abs(g.get_emf(b)[I] - F[4 + a][I]).max() <= 1e-14 * np.abs(F[4 + a][I]).max(), d
+        assert np.abs(g.get_emf(a)[I] + F[4 + b][I]).max() <= 1e-14 * np.abs(F[4 + b][I]).max(), d
+    P0 = np.zeros((8, 8, 10, 12)); P0[0] = 1.0; P0[1] = 0.7; P0[2] = 0.3; P0[3] = -0.2; P0[4] = 0.1; P0[5] = 0.4; P0[6] = -0.3; P0[7] = 0.2
+    g = kho.Grid(dict(p0, emf=kp.EMF_CENTRED)); g.set_prims(P0); g.debug_emf()
+    gamma = np.sqrt(1 + 0.3 ** 2 + 0.2 ** 2 + 0.1 ** 2)
+    v = np.array([0.3, -0.2, 0.1]) / gamma; B = np.array([0.4, -0.3, 0.2])
+    for c in range(3):
+        a, b = (c + 1) % 3, (c + 2) % 3
+        assert np.allclose(g.get_emf(c + 1)[I], B[b] * v[a] - B[a] * v[b], rtol=1e-13, atol=1e-15)
+    # a genuinely 3-D state: three different discretisations; the centred one is the mean of the upwinded scheme's two
+    # one-sided choices, so it lies between "upwinded with the flow" and "upwinded against it" (the flow reversed)
+    P3 = modes.config5(p0, seed=4, amp=5e-2)
+    e = {}
+    for kind in (kp.EMF_ARITHMETIC, kp.EMF_UPWIND, kp.EMF_CENTRED):
+        g = kho.Grid(dict(p0, emf=kind)); g.set_prims(P3); g.debug_emf()
+        e[kind] = np.stack([g.get_emf(c)[I] for c in (1, 2, 3)])
+    scale = np.abs(e[kp.EMF_ARITHMETIC]).max()
+    assert np.abs(e[kp.EMF_CENTRED] - e[kp.EMF_ARITHMETIC]).max() > 1e-6 * scale
+    assert np.abs(e[kp.EMF_CENTRED] - e[kp.EMF_UPWIND]).max() > 1e-6 * scale
+
+
+def test_centred_emf_keeps_divergence_and_second_order(kho):
+    from kharm_inputs import facefield
+    q = ki.config_params(5, n=(12, 10, 8), recon=kp.RECON_WENO5)
+    P0 = modes.config5(q, seed=2, amp=5e-2)
+    faces = facefield.face_from_potential(q, *facefield.periodic_potential(q, seed=3, amp=5e-2))
+    g = kho.Grid(dict(q, transport=kp.B_FACE_CT, emf=kp.EMF_CENTRED))
+    g.set_prims(P0); g.set_face_B(*faces)
+    dt = g.estimate_dt()
+    for _ in range(5):
+        dt = g.step(dt)
+    assert g.divB_face() < 1e-12
+    g = kho.Grid(dict(q, emf=kp.EMF_CENTRED)); g.set_prims(P0)                 # Flux-CT transport: corner divergence
+    d0 = g.divB(); dt = g.estimate_dt()
+    for _ in range(5):
+        dt = g.step(dt)
+    assert abs(g.divB() - d0) < 1e-12
+    errs = []
+    for n in (16, 32):
+        p = dict(ki.config_params(1, n=(n, n, 4)), emf=kp.EMF_CENTRED)
+        Pm, T = modes.config1(p, rotated=True)
+        g = kho.Grid(p, omp=True); g.set_prims(Pm)
+        dt, t = g.estimate_dt(), 0.0
+        while t < T * (1 - 1e-12):
+            dt = min(dt, T - t); t += dt
+            dt = g.step(dt)
+        errs.append(np.abs(g.get_prims() - Pm).mean(axis=(1, 2, 3)).max())
+    slope = np.log2(errs[0] / errs[1])
+    assert 1.7 < slope < 2.4, (errs, slope)
+
+
 def test_face_ct_equals_flux_ct_for_any_emf_and_option_mix(kho):
     """The zone-centred mean of the face field obeys the Flux-CT update for ANY edge EMFs (the identity is algebra on the
     EMF arrays), so the two transports must agree to round-off whatever the EMF kind, inverter, floor frame or FOFC."""
@@ -188,7 +253,7 @@ def test_face_ct_equals_flux_ct_for_any_emf_and_option_mix(kho):
     for trial in range(6):
         n = (int(rng.integers(8, 20)), int(rng.integers(6, 14)), int(rng.integers(1, 6)))
         opts = dict(recon=int(rng.integers(0, 2)), inverter=int(rng.integers(0, 2)), floor_frame=int(rng.integers(0, 3)),
-                    fofc=int(rng.integers(0, 2)), emf=int(rng.integers(0, 2)))
+                    fofc=int(rng.integers(0, 2)), emf=int(rng.integers(0, 3)))
         p = dict(ki.config_params(3, n=n), **opts)
         P0 = torus.torus_state(p, seed=trial)
         faces = facefield.face_from_potential(p, *facefield.axisymmetric_loop_potential(p, amp=2e-3, x1c=2.3))

@@ -155,6 +155,36 @@ def test_bondi_short_run_stays_near_analytic(kho):
     assert abs(g.divB() - d0) < 1e-11
 
 
+def test_config2_as_stated_stays_at_the_analytic_steady_state_to_t_50(kho):
+    """BASELINE config 2 as it is stated ("one Bondi accretion problem"): r in [1.8, 50], sonic radius 8, monopole field
+    with b^2 / rho = 1 at r_s, initialised from the analytic solution and run for 50 M; error against the analytic steady
+    state outside the horizon.  Here at 32^2 and 64^2 (the stated 128^2 runs on the GPU box: tests/test_gpu_parity.py,
+    where this oracle is run beside the CUDA path).  What holds, and is asserted: the run settles (t = 25 -> 50 changes
+    the error by < 15 %), the settled state is the analytic one to a few per cent, and the error falls with resolution --
+    by 1.8 to 4 per doubling, NOT by the 4 of a clean second-order steady state: the field is b^2 / rho ~ 30 at the inner
+    edge, the outflow copy there is first order, and fast waves carry that error outwards (config 2).
+    Measured 32 -> 64 -> 128: rho 0.026 / 0.014 / 0.006, u 0.16 / 0.040 / 0.022, field 0.030 / 0.011 / 0.003."""
+    from parity_util import bondi_errors
+    errs = {}
+    for n in (32, 64):
+        p = ki.config_params(2, n=(n, n, 1))
+        g = kho.Grid(p, omp=True)
+        g.set_prims(bondi.config2(p), with_ghosts=True)
+        P0 = g.get_prims()
+        d0 = g.divB()
+        _evolve(g, 25.0)
+        mid = bondi_errors(p, g.get_prims(), P0)
+        _evolve(g, 25.0)
+        errs[n] = bondi_errors(p, g.get_prims(), P0)
+        assert np.all(np.abs(errs[n] / mid - 1) < 0.15), (n, mid, errs[n])        # settled, no secular drift
+        assert abs(g.divB() - d0) < 1e-10
+        assert (g.get_flags()[0] != 0).sum() <= (16 if n == 32 else 8)             # a handful of failed inversions at the inner edge
+    e32, e64 = errs[32], errs[64]
+    assert e64[0] < 0.02 and e64[1] < 0.05 and e64[3] < 0.015, e64                # rho, u, field at 64^2
+    ratio = e32 / e64
+    assert np.all(ratio > 1.7) and ratio[1] > 3.0 and ratio[3] > 2.4, ratio
+
+
 def test_mirror_symmetry_of_a_full_step(kho):
     """x1 -> -x1 with ut1, B1 -> -ut1, -B1 maps solutions to solutions; the scheme (reconstruction L/R,
     LLF, Flux-CT signs, dt rule) must respect it to round-off."""
