@@ -843,7 +843,10 @@ __global__ void finalize_dt_kernel(StepScalars* sc, double cfl, double growth) {
   sc->dt_next = sc->nonfinite ? __longlong_as_double(0x7ff8000000000000LL) : (d < cap ? d : cap);     // kh_step reports KH_ENAN
   sc->rate_bits = 0ULL;
 }
-__global__ void set_dt_kernel(StepScalars* sc, double dt, int from_next) { sc->dt = from_next ? sc->dt_next : dt; sc->nonfinite = 0ULL; }
+__global__ void set_dt_kernel(StepScalars* sc, double dt, int from_next) {      // opens a step: dt, the sticky bit and the predictor's failure counters
+  sc->dt = from_next ? sc->dt_next : dt;
+  sc->nonfinite = 0ULL; sc->n_pflag = 0ULL; sc->n_fflag = 0ULL;
+}
 __global__ void reset_counters_kernel(StepScalars* sc, int also_rate) {
   sc->n_pflag = 0; sc->n_fflag = 0;
   if (also_rate) sc->rate_bits = 0ULL;      // FOFC: the speculative corrector update has written its CFL maximum
@@ -856,11 +859,10 @@ __global__ void reset_counters_kernel(StepScalars* sc, int also_rate) {
 // direction maps below, value transforms applied in pass order (outflow: B rescaled by the ratio of tabulated
 // sqrt(-g), S20b; polar: sign of ut^2, B^2).  One launch, bit-identical to the three passes.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128)
-fill_kernel(GV g, double* __restrict__ P, unsigned char* __restrict__ flag) {
+// ghost zone number t of the shell (t >= the shell size: nothing)
+__device__ __forceinline__ void fill_zone(const GV& g, double* __restrict__ P, unsigned char* __restrict__ flag, long t) {
   // ghost shell = slab A (k ghost, all i, j) + slab B (j ghost, k interior, all i) + slab C (i ghost, j, k interior)
   const long nA = (long)g.nt1 * g.nt2 * (2 * KH_NGH), nB = (long)g.nt1 * (2 * KH_NGH) * g.n3, nC = (long)(2 * KH_NGH) * g.n2 * g.n3;
-  long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
   int a, b, c;    // interior-based indices of the ghost zone
   if (t < nA) {
     a = (int)(t % g.nt1) - KH_NGH; long r = t / g.nt1;
@@ -902,6 +904,14 @@ fill_kernel(GV g, double* __restrict__ P, unsigned char* __restrict__ flag) {
   if (flag) flag[ng] = flag[ns];
 }
 
+__device__ __forceinline__ long shell_size(const GV& g) {
+  return (long)g.nt1 * g.nt2 * (2 * KH_NGH) + (long)g.nt1 * (2 * KH_NGH) * g.n3 + (long)(2 * KH_NGH) * g.n2 * g.n3;
+}
+__global__ void __launch_bounds__(128)
+fill_kernel(GV g, double* __restrict__ P, unsigned char* __restrict__ flag) {
+  fill_zone(g, P, flag, (long)blockIdx.x * blockDim.x + threadIdx.x);
+}
+
 // ---------------------------------------------------------------------------------------------
 // K5b: fix-up of failed inversions (S19): 26-neighbour weighted mean of good zones from the pre-fix-up
 // snapshot.  The update kernel appends every failed zone to a list, so both kernels run over the list only
@@ -917,9 +927,8 @@ __device__ __forceinline__ void zone_of(const GV& g, long n, int& i, int& j, int
 }
 
 // One warp per failed zone: lane l < 26 owns one neighbour (independent loads in flight), butterfly sums.
-__global__ void __launch_bounds__(128)
-fixup_gather_kernel(GV g, const double* __restrict__ Pf, const unsigned char* __restrict__ pflag, const unsigned* __restrict__ list,
-                    double* __restrict__ fix, const StepScalars* __restrict__ sc) {
+__device__ __forceinline__ void fixup_gather(const GV& g, const double* __restrict__ Pf, const unsigned char* __restrict__ pflag,
+                                             const unsigned* __restrict__ list, double* __restrict__ fix, const StepScalars* __restrict__ sc) {
   const long count = (long)sc->n_pflag, nt = g.ntot;
   const int lane = threadIdx.x & 31;
   const long warp = ((long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = ((long)gridDim.x * blockDim.x) >> 5;
@@ -951,11 +960,15 @@ fixup_gather_kernel(GV g, const double* __restrict__ Pf, const unsigned char* __
     }
   }
 }
+__global__ void __launch_bounds__(128)
+fixup_gather_kernel(GV g, const double* __restrict__ Pf, const unsigned char* __restrict__ pflag, const unsigned* __restrict__ list,
+                    double* __restrict__ fix, const StepScalars* __restrict__ sc) {
+  fixup_gather(g, Pf, pflag, list, fix, sc);
+}
 
 template <bool FLAT>
-__global__ void __launch_bounds__(128)
-fixup_apply_kernel(GV g, double* __restrict__ Pf, const unsigned* __restrict__ list, unsigned char* __restrict__ fflag,
-                   const double* __restrict__ fix, const StepScalars* __restrict__ sc) {
+__device__ __forceinline__ void fixup_apply(const GV& g, double* __restrict__ Pf, const unsigned* __restrict__ list,
+                                            unsigned char* __restrict__ fflag, const double* __restrict__ fix, const StepScalars* __restrict__ sc) {
   const long count = (long)sc->n_pflag, nt = g.ntot;
   for (long q = (long)blockIdx.x * blockDim.x + threadIdx.x; q < count; q += (long)gridDim.x * blockDim.x) {
     const long n = list[q];
@@ -1003,6 +1016,12 @@ fixup_apply_kernel(GV g, double* __restrict__ Pf, const unsigned* __restrict__ l
     for (int v = 0; v < 5; v++) Pf[v * nt + n] = P[v];
     store_ghost_images<5>(g, Pf, nullptr, i, j, k, P, 0);
   }
+}
+template <bool FLAT>
+__global__ void __launch_bounds__(128)
+fixup_apply_kernel(GV g, double* __restrict__ Pf, const unsigned* __restrict__ list, unsigned char* __restrict__ fflag,
+                   const double* __restrict__ fix, const StepScalars* __restrict__ sc) {
+  fixup_apply<FLAT>(g, Pf, list, fflag, fix, sc);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -9,6 +9,8 @@
 #include <cstring>
 #include <new>
 
+#include <nvtx3/nvToolsExt.h>      // header-only; ranges are no-ops unless a tool is attached
+
 #include "kh_geometry.cuh"
 #include "kh_kernels.cuh"
 
@@ -104,8 +106,12 @@ static void prof_flush(kh_grid* g) {
   }
   g->npev = 0;
 }
-// bracket one launch: PROF_BEGIN(kind); kernel<<<...>>>(...); PROF_END();
+struct NvtxRange { explicit NvtxRange(const char* n) { nvtxRangePushA(n); } ~NvtxRange() { nvtxRangePop(); } };
+static const char* const kKindName[KH_K_COUNT] = {"kh:flux", "kh:flux2", "kh:flux3", "kh:emf", "kh:update", "kh:fill", "kh:fixup", "kh:fofc"};
+// bracket one launch group: prof_begin(kind); kernel<<<...>>>(...); prof_end();  Always an NVTX range (host side: it marks the
+// enqueue, or the capture, of the group); with kh_set_profile also a pair of CUDA events.
 static inline void prof_begin(kh_grid* g, int kind) {
+  nvtxRangePushA(kKindName[kind]);
   if (!g->profile) return;
   if (g->gp_capture) {
     const int c = g->gp_capture - 1, r = g->gpn[c];
@@ -120,6 +126,7 @@ static inline void prof_begin(kh_grid* g, int kind) {
   cudaEventRecord(g->pev[2 * g->npev], g->stream);
 }
 static inline void prof_end(kh_grid* g) {
+  nvtxRangePop();
   if (!g->profile) return;
   if (g->gp_capture) {
     const int c = g->gp_capture - 1, r = g->gpn[c];
@@ -719,6 +726,7 @@ int kh_step(kh_grid* g, double dt, double* dt_next) {
   if (g->has_block) return KH_EINVAL;                                       // a block with KH_BC_BLOCK sides steps with its neighbours: kh_step_blocks
   if (!(dt > 0.0) && !g->have_dt_next) return KH_EINVAL;                    // no dt_next on the device yet
   ENTER(g);
+  NvtxRange range_("kh_step");
   set_dt_kernel<<<1, 1, 0, g->stream>>>(g->sc, dt, dt > 0.0 ? 0 : 1);
   g->launches++;
   CK(cudaGetLastError());

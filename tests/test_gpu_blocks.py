@@ -162,3 +162,45 @@ def test_link_validation(kh):
     c = kh.Grid(dict(parts[1], n1=10), stream=stream.cuda_stream)
     with pytest.raises(kh.KharmError):
         kh.link_blocks(a, c, 3)                              # transverse shapes differ
+
+
+# ------------------------------------------------------------------------------------------ boundary behaviour added in round 2
+def test_stream_device_and_error_paths(kh):
+    import torch
+    p = ki.config_params(5, n=(16, 12, 8))
+    P0 = modes.config5(p, seed=1, amp=1e-2)
+    s = torch.cuda.Stream()
+    g = kh.Grid(p, stream=s.cuda_stream)
+    assert g.get_stream() == s.cuda_stream                   # the caller's stream is the grid's stream
+    g0 = kh.Grid(p, stream=0)
+    assert g0.get_stream() not in (0, s.cuda_stream)         # NULL: a stream of the grid's own (kh_get_stream names it)
+    g.set_prims(P0)
+    with pytest.raises(kh.KharmError):
+        g.step(-1.0)                                         # no dt_next on the device before the first completed step
+    dt = g.estimate_dt()
+    g.step(dt, sync=False)
+    g.sync()                                                 # kh_sync: everything enqueued on the grid's stream has finished
+    g.step(-1.0)                                             # now legal
+    # non-finite input: the CFL reduction must not swallow it (fmax drops NaNs): KH_ENAN
+    bad = P0.copy()
+    bad[1, 3, 4, 5] = np.nan
+    gb = kh.Grid(p)
+    gb.set_prims(bad)
+    with pytest.raises(kh.KharmError, match="non-finite"):
+        gb.estimate_dt()
+
+
+def test_step_falls_back_to_direct_launches_when_the_stream_cannot_be_captured(kh):
+    """the legacy default stream (cudaStreamLegacy = 0x1) cannot be captured into a CUDA graph; kh_step must then
+    launch the same kernels directly instead of failing, and give the same result bit for bit."""
+    p = ki.config_params(5, n=(20, 12, 8), recon=kp.RECON_WENO5)
+    P0 = modes.config5(p, seed=2, amp=1e-2)
+    outs = []
+    for stream in (None, 1):
+        g = kh.Grid(p) if stream is None else kh.Grid(p, stream=stream)
+        g.set_prims(P0)
+        dt = g.estimate_dt()
+        for _ in range(3):
+            dt = g.step(dt)
+        outs.append(g.get_prims())
+    assert np.array_equal(outs[0], outs[1])
