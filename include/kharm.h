@@ -111,7 +111,7 @@ int kh_get_flags(kh_grid* g, int* pflag, int* fflag, int mem);
 
 /* CFL time step dt = cfl / max_zones sum_d c^d / dx_d from zone-centred fast-magnetosonic speeds c^d, for the
  * first step (the step is set by the signal crossing time of the smallest zones; S22).
- * *dt is a HOST double.  KH_ENAN if a zone's speed is not finite. */
+ * *dt is a HOST double.  KH_ENAN if a primitive or a zone's speed is not finite. */
 int kh_estimate_dt(kh_grid* g, double* dt);
 
 /* One full predictor-corrector step:

@@ -1216,8 +1216,9 @@ __global__ void estimate_dt_kernel(GV g, const double* __restrict__ P, StepScala
     const long n = zidx(g, i, j, k), nt = g.ntot;
     Geo G;
     load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, pidx(g, i, j));
-    double p[KH_NP];
-    for (int v = 0; v < KH_NP; v++) p[v] = P[v * nt + n];
+    double p[KH_NP], psum = 0.0;
+    for (int v = 0; v < KH_NP; v++) { p[v] = P[v * nt + n]; psum += fabs(p[v]); }
+    if (rate_nonfinite(psum)) sc->nonfinite = 1ULL;      // a non-finite primitive: the wave-speed clamps would hide it from the rate
     FourVec D;
     four_vectors<FLAT>(G, FLAT ? 1.0 : -G.n00 * G.alpha, p, D);
     double pg = (g.gam - 1.0) * p[UU], ee = fma(g.gam, p[UU], p[RHO]) + D.bsq, gg1u = g.gam * pg;
