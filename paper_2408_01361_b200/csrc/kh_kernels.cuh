@@ -31,6 +31,11 @@ struct GV {                 // grid view, passed by value
   int bc[6];
   int polar_lo, polar_hi;
   int ndim_mask;            // bit d set if N_d > 1 (enters the CFL sum)
+  // Transverse rows the flux kernels compute, [tlo, thi) in interior indices (j for x1 / x3 faces, k for x1 / x2 faces).  Flux-CT
+  // needs one ghost row each side, EXCEPT where that row is redundant: beyond a polar boundary (the edge EMFs on the axis are
+  // zero whatever it holds) and in a periodic direction whose ghost rows are exact images (alias: x3 always -- the metric does
+  // not depend on x3 -- and any direction in Minkowski), where emf_kernel reads the image's source row instead.
+  int tlo2, thi2, tlo3, thi3, alias2, alias3;
   const double* geom[4];    // CENT, FACE1, FACE2, FACE3 tables
   const double* conn;       // Gamma table (kh_get_conn only)
   const double* dg;         // source table, KH_NDG x n2d
@@ -112,8 +117,8 @@ __device__ __forceinline__ void face_flux(const GV& g, const double PL[KH_NP], c
 template <int RECON, bool FLAT>
 __global__ void __launch_bounds__(128, KH_MINB_X1)
 flux_x1_kernel(GV g, const double* __restrict__ P, double* __restrict__ F, double* __restrict__ ctop) {
-  const int c1 = g.n1 + 2, c2 = g.n2 + 2;                // zones -1 .. N per row; rows (j, k) in [-1, N]
-  const long Z = (long)c1 * c2 * (g.n3 + 2);
+  const int c1 = g.n1 + 2, c2 = g.thi2 - g.tlo2;         // zones -1 .. N per row; rows (j, k) in [tlo, thi) (GV)
+  const long Z = (long)c1 * c2 * (g.thi3 - g.tlo3);
   const int lane = threadIdx.x & 31;
   const long warp = ((long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const long z = warp * 31 + lane;                       // consecutive warps overlap by one zone
@@ -121,7 +126,7 @@ flux_x1_kernel(GV g, const double* __restrict__ P, double* __restrict__ F, doubl
   const long zc = valid ? z : Z - 1;
   const int i = (int)(zc % c1) - 1;
   const long row = zc / c1;
-  const int j = (int)(row % c2) - 1, k = (int)(row / c2) - 1;
+  const int j = (int)(row % c2) + g.tlo2, k = (int)(row / c2) + g.tlo3;
   const long n = zidx(g, i, j, k), nt = g.ntot;
   double PL[KH_NP], PR[KH_NP];
 #pragma unroll
@@ -178,10 +183,10 @@ flux_march_kernel(GV g, const double* __restrict__ P, double* __restrict__ F, do
   extern __shared__ double ring[];
   constexpr int H = MarchRing<RECON>::H, R = MarchRing<RECON>::R;
   const int c1 = g.n1 + 2;
-  const int cb = (DIR == 2 ? g.n3 : g.n2) + 2;
+  const int blo = DIR == 2 ? g.tlo3 : g.tlo2, cb = (DIR == 2 ? g.thi3 : g.thi2) - blo;     // transverse rows [tlo, thi) (GV)
   const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= (long)c1 * cb) return;                     // no barriers below: early exit is safe
-  const int i = (int)(t % c1) - 1, b = (int)(t / c1) - 1;
+  const int i = (int)(t % c1) - 1, b = (int)(t / c1) + blo;
   const int N = (DIR == 2) ? g.n2 : g.n3;
   const int f0 = blockIdx.y * J;
   const int f1 = (f0 + J < N + 1) ? f0 + J : N + 1;
@@ -253,16 +258,20 @@ emf_kernel(GV g, const double* __restrict__ F1, const double* __restrict__ F2, c
   if (i > g.n1) return;
   const long n = zidx(g, i, j, k), nt = g.ntot;
   bool axis = polar_face(g, j);
+  // offsets to the transverse rows j - 1, j and k - 1, k of the face fluxes; where a periodic direction's ghost rows are exact
+  // images and were not computed (GV.alias), row -1 is row N - 1 and row N is row 0
+  const long jm = (g.alias2 && j == 0) ? (long)(g.n2 - 1) * g.s2 : -g.s2, j0 = (g.alias2 && j == g.n2) ? -(long)g.n2 * g.s2 : 0;
+  const long km = (g.alias3 && k == 0) ? (long)(g.n3 - 1) * g.s3 : -g.s3, k0 = (g.alias3 && k == g.n3) ? -(long)g.n3 * g.s3 : 0;
   if (k < g.n3) {
-    double v = 0.25 * (F1[B2 * nt + n] + F1[B2 * nt + n - g.s2] - F2[B1 * nt + n] - F2[B1 * nt + n - 1]);
+    double v = 0.25 * (F1[B2 * nt + n + j0] + F1[B2 * nt + n + jm] - F2[B1 * nt + n] - F2[B1 * nt + n - 1]);
     e3[n] = axis ? 0.0 : v;
   }
   if (j < g.n2) {
-    double v = -0.25 * (F1[B3 * nt + n] + F1[B3 * nt + n - g.s3] - F3[B1 * nt + n] - F3[B1 * nt + n - 1]);
+    double v = -0.25 * (F1[B3 * nt + n + k0] + F1[B3 * nt + n + km] - F3[B1 * nt + n] - F3[B1 * nt + n - 1]);
     e2[n] = v;
   }
   if (i < g.n1) {
-    double v = 0.25 * (F2[B3 * nt + n] + F2[B3 * nt + n - g.s3] - F3[B2 * nt + n] - F3[B2 * nt + n - g.s2]);
+    double v = 0.25 * (F2[B3 * nt + n + k0] + F2[B3 * nt + n + km] - F3[B2 * nt + n + j0] - F3[B2 * nt + n + jm]);
     e1[n] = axis ? 0.0 : v;
   }
 }

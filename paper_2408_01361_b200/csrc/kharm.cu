@@ -212,7 +212,7 @@ static void launch_flux(kh_grid* g, const double* Ps, cudaStream_t stream, bool 
   const bool mc = g->p.recon == KH_RECON_MC;
   if (prof) prof_begin(g, KH_K_FLUX1 + DIR - 1);
   if (DIR == 1) {
-    const long zones = (long)(v.n1 + 2) * (v.n2 + 2) * (v.n3 + 2);
+    const long zones = (long)(v.n1 + 2) * (v.thi2 - v.tlo2) * (v.thi3 - v.tlo3);
     const long warps = (zones + 30) / 31;
     const unsigned blocks = (unsigned)((warps + 3) / 4);
     if (g->flat) {
@@ -224,7 +224,7 @@ static void launch_flux(kh_grid* g, const double* Ps, cudaStream_t stream, bool 
     }
   } else {
     const int N = (DIR == 2) ? v.n2 : v.n3;
-    const long cols = (long)(v.n1 + 2) * ((DIR == 2 ? v.n3 : v.n2) + 2);
+    const long cols = (long)(v.n1 + 2) * (DIR == 2 ? v.thi3 - v.tlo3 : v.thi2 - v.tlo2);
     // concurrent directions: whole columns (no redundant reconstruction at chunk starts; the x1 kernel's many small blocks fill
     // the SMs the few long-running marching blocks leave free); alone: chunks that fill the SMs in whole waves
     int J;
@@ -530,6 +530,17 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   for (int b = 0; b < 6; b++) v.bc[b] = p->bc[b];
   v.polar_lo = p->bc[2] == KH_BC_POLAR; v.polar_hi = p->bc[3] == KH_BC_POLAR;
   v.ndim_mask = (v.n1 > 1 ? 1 : 0) | (v.n2 > 1 ? 2 : 0) | (v.n3 > 1 ? 4 : 0);
+  {
+    // transverse ghost rows of the face fluxes that nothing reads (GV): only with the arithmetic EMFs and without FOFC (the other
+    // EMF kernels and the re-flux read the ghost rows directly)
+    const bool skip = p->emf == KH_EMF_ARITHMETIC && !p->fofc;
+    v.alias2 = skip && p->bc[2] == KH_BC_PERIODIC && g->flat;
+    v.alias3 = skip && p->bc[4] == KH_BC_PERIODIC;
+    v.tlo2 = (v.alias2 || (skip && v.polar_lo)) ? 0 : -1;
+    v.thi2 = (v.alias2 || (skip && v.polar_hi)) ? v.n2 : v.n2 + 1;
+    v.tlo3 = v.alias3 ? 0 : -1;
+    v.thi3 = v.alias3 ? v.n3 : v.n3 + 1;
+  }
   v.fp.inv_bsq_over_rho_max = 1.0 / p->bsq_over_rho_max; v.fp.inv_bsq_over_u_max = 1.0 / p->bsq_over_u_max;
   v.fp.u_over_rho_max = p->u_over_rho_max; v.fp.gamma_max = p->gamma_max;
   v.floor_frame = p->floor_frame; v.inverter = p->inverter;
