@@ -269,6 +269,10 @@ static int do_fixup(kh_grid* g, double* Pf) {
 static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, double dt_factor, bool corrector,
                    double* const* Bfi = nullptr, double* const* Bff = nullptr, bool with_fixup = true) {
   const GV& v = g->gv;
+  // One thread's worth of work, but also the SINGLE predecessor of the three flux kernels in the step's graph.  Measured (r02):
+  // with the reset folded into another kernel the predictor's flux kernels become root nodes of the graph, the executor
+  // launches x1 first, its short blocks take every slot before the marching blocks are placed, and the step costs 9 % more
+  // (1.66 -> 1.81 ms); a higher priority of the side streams does not change that.
   reset_counters_kernel<<<1, 1, 0, g->stream>>>(g->sc, 0);
   g->launches++;
   if (g->flux_concurrent) {
