@@ -6,6 +6,8 @@
 //   K7 fill_kernel<DIR>              ghost fills (periodic / outflow / polar / fixed)
 //   misc: cons, divB, estimate_dt, dt finalise
 #pragma once
+#include <cuda.h>          // CUtensorMap (type only: the maps are encoded by the host through the driver entry point)
+
 #include "kh_device.cuh"
 
 // Minimum resident blocks per SM of the hot kernels (register caps: 4 -> 128, 5 -> 102, 6 -> 85 registers).
@@ -465,32 +467,35 @@ struct GlobalAcc {
   __device__ __forceinline__ double c3(int d) const { return C3[n + d * s3]; }
 };
 
-// Layout of a warp's tile (32 zones of one x1 row) in shared memory, in doubles.  Rows whose x1 neighbour i+1 is read hold
-// 34 doubles (272 B: a multiple of 16 B for the bulk copy), the others 32.
+// Layout of a warp's tile (32 zones of one x1 row) in shared memory, in doubles.  One REGION per tensor copy (a box of one
+// array: dense [v][k][j][i] as the TMA unit writes it), each starting on a 128 B boundary.  Rows whose x1 neighbour i+1 is read
+// hold 34 doubles (272 B: the box's inner extent must be a multiple of 16 B), the others 32.  c_top is not staged (its six
+// values per zone are loaded before the wait): the tile of the corrector is then exactly what four blocks per SM can hold.
+__host__ __device__ constexpr int tile_pad(int doubles) { return (doubles + 15) / 16 * 16; }
 template <bool FLAT, bool CORR, int MODE>
 struct TileLayout {
   static constexpr bool FACE = (MODE & 8) != 0;
   static constexpr bool PS = CORR && !FLAT;            // a separate P_s (predictor: P_s = P_i; Minkowski: no source term)
   static constexpr int WL = 34, WS = 32;
-  static constexpr int F1 = 0;                                   // 5 long rows
-  static constexpr int E3 = F1 + 5 * WL;                         // 2 long rows (j, j+1)          | face CT: BF1, 1 long row
-  static constexpr int E2 = E3 + (FACE ? 1 : 2) * WL;            // 2 long rows (k, k+1)          | face CT: none
-  static constexpr int C1 = E2 + (FACE ? 0 : 2) * WL;            // 1 long row (corrector)
-  static constexpr int F2 = C1 + (CORR ? 1 : 0) * WL;            // 5 x 2 rows
-  static constexpr int F3 = F2 + 10 * WS;                        // 5 x 2 rows
-  static constexpr int E1 = F3 + 10 * WS;                        // 4 rows (j, k), (j+1, k), (j, k+1), (j+1, k+1) | face CT: BF2 x 2, BF3 x 2
-  static constexpr int PI = E1 + 4 * WS;                         // 8 rows
-  static constexpr int PSO = PI + 8 * WS;                        // 8 rows if PS
-  static constexpr int C2 = PSO + (PS ? 8 : 0) * WS;             // 2 rows (corrector)
-  static constexpr int C3 = C2 + (CORR ? 2 : 0) * WS;            // 2 rows (corrector)
-  static constexpr int DOUBLES = C3 + (CORR ? 2 : 0) * WS;
-  static constexpr int BYTES = DOUBLES * 8;                      // per warp; a multiple of 16
+  static constexpr int F1 = 0;                                   // box (34, 1, 1, 5)
+  static constexpr int E3 = F1 + tile_pad(5 * WL);               // box (34, 2, 1): rows j, j+1       | face CT: BF1, box (34, 1, 1)
+  static constexpr int E2 = E3 + tile_pad((FACE ? 1 : 2) * WL);  // box (34, 1, 2): planes k, k+1     | face CT: none
+  static constexpr int F2 = E2 + tile_pad((FACE ? 0 : 2) * WL);  // box (32, 2, 1, 5)
+  static constexpr int F3 = F2 + 10 * WS;                        // box (32, 1, 2, 5)
+  static constexpr int E1 = F3 + 10 * WS;                        // box (32, 2, 2): (j, k), (j+1, k), (j, k+1), (j+1, k+1) | face CT: BF2 (32, 2, 1), BF3 (32, 1, 2)
+  static constexpr int PI = E1 + 4 * WS;                         // box (32, 1, 1, 8)
+  static constexpr int PSO = PI + 8 * WS;                        // box (32, 1, 1, 8) if PS
+  static constexpr int DOUBLES = PSO + (PS ? 8 : 0) * WS;
+  static constexpr int BYTES = DOUBLES * 8;                      // per warp; a multiple of 128
+  // bytes the copies of one tile deliver (the boxes, unpadded)
+  static constexpr int TX = 8 * (5 * WL + (FACE ? WL : 4 * WL) + 20 * WS + 4 * WS + 8 * WS + (PS ? 8 * WS : 0));
 };
 
 template <bool FLAT, bool CORR, int MODE>
 struct TileAcc {
   using L = TileLayout<FLAT, CORR, MODE>;
   const double* t;      // the warp's tile + lane
+  const double* ct;     // c_top at the zone's six faces: (x1 lo, hi, x2 lo, hi, x3 lo, hi), loaded by the thread itself
   __device__ __forceinline__ double pi(int v) const { return t[L::PI + v * L::WS]; }
   __device__ __forceinline__ double ps(int v) const { return t[(L::PS ? L::PSO : L::PI) + v * L::WS]; }
   __device__ __forceinline__ double f1(int v, int d) const { return t[L::F1 + v * L::WL + d]; }
@@ -502,9 +507,9 @@ struct TileAcc {
   __device__ __forceinline__ double bf1(int d) const { return t[L::E3 + d]; }
   __device__ __forceinline__ double bf2(int d) const { return t[L::E1 + d * L::WS]; }
   __device__ __forceinline__ double bf3(int d) const { return t[L::E1 + (2 + d) * L::WS]; }
-  __device__ __forceinline__ double c1(int d) const { return t[L::C1 + d]; }
-  __device__ __forceinline__ double c2(int d) const { return t[L::C2 + d * L::WS]; }
-  __device__ __forceinline__ double c3(int d) const { return t[L::C3 + d * L::WS]; }
+  __device__ __forceinline__ double c1(int d) const { return ct[d]; }
+  __device__ __forceinline__ double c2(int d) const { return ct[2 + d]; }
+  __device__ __forceinline__ double c3(int d) const { return ct[4 + d]; }
 };
 
 // Phase A: everything that consumes the streamed inputs -- the advanced conserved state Uh = U_f / sqrt(-g), the guess W0 and
@@ -701,6 +706,24 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
       "KH_MBAR_DONE:\n"
       "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
+// one box of a tensor (cp.async.bulk.tensor, tile mode): c0 = innermost coordinate; completion counted on the mbarrier
+__device__ __forceinline__ void tensor_g2s(double* dst, const CUtensorMap* map, int c0, int c1, int c2, int c3, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(smem_u32(dst)),
+               "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tensor_g2s(double* dst, const CUtensorMap* map, int c0, int c1, int c2, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(smem_u32(dst)),
+               "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
+// The tensor maps of one update launch (built once per grid by the host; kernel parameter, __grid_constant__).  Every array
+// starts one double past its 256 B aligned allocation (kharm.cu), so the maps describe the allocation and the innermost
+// coordinate carries that one double: element (i, j, k) of an array is (i + 4, j + 3, k + 3) of its map.
+struct alignas(64) TileMaps {
+  CUtensorMap f1, f2, f3;      // hydro fluxes, boxes (34,1,1,5), (32,2,1,5), (32,1,2,5)
+  CUtensorMap a, b, c;         // e3 (34,2,1), e2 (34,1,2), e1 (32,2,2)   | face CT: Bf1 (34,1,1), Bf2 (32,2,1), Bf3 (32,1,2)
+  CUtensorMap pi, ps;          // primitives, box (32,1,1,8)
+};
+
 __device__ __forceinline__ void bulk_g2s(double* dst, const double* src, unsigned bytes, unsigned long long* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src),
                "r"(bytes), "r"(smem_u32(bar)) : "memory");
@@ -712,53 +735,25 @@ __device__ __forceinline__ bool elect_one() {     // one lane of the (converged)
   return p != 0;
 }
 
+// the copies of one tile: 8 (predictor) or 9 (corrector) tensor boxes; (c0, c1, c2) = map coordinates of zone (i0, j, k)
 template <bool FLAT, bool CORR, int MODE>
-__device__ __forceinline__ void issue_tile(const GV& g, double* tile, unsigned long long* bar, long n0, const double* __restrict__ Pi,
-                                           const double* __restrict__ Ps, const double* __restrict__ F1, const double* __restrict__ F2,
-                                           const double* __restrict__ F3, const double* __restrict__ e1, const double* __restrict__ e2,
-                                           const double* __restrict__ e3, const double* __restrict__ ct1, const double* __restrict__ ct2,
-                                           const double* __restrict__ ct3, const double* __restrict__ Bface1, const double* __restrict__ Bface2,
-                                           const double* __restrict__ Bface3) {
+__device__ __forceinline__ void issue_tile(const TileMaps& M, double* tile, unsigned long long* bar, int c0, int c1, int c2) {
   using L = TileLayout<FLAT, CORR, MODE>;
-  const long nt = g.ntot, s2 = g.s2, s3 = g.s3;
-  constexpr unsigned BL = L::WL * 8, BS = L::WS * 8;
-  mbar_expect_tx(bar, (unsigned)L::BYTES);
-#pragma unroll
-  for (int v = 0; v < 5; v++) {
-    bulk_g2s(tile + L::F1 + v * L::WL, F1 + v * nt + n0, BL, bar);
-    bulk_g2s(tile + L::F2 + (2 * v) * L::WS, F2 + v * nt + n0, BS, bar);
-    bulk_g2s(tile + L::F2 + (2 * v + 1) * L::WS, F2 + v * nt + n0 + s2, BS, bar);
-    bulk_g2s(tile + L::F3 + (2 * v) * L::WS, F3 + v * nt + n0, BS, bar);
-    bulk_g2s(tile + L::F3 + (2 * v + 1) * L::WS, F3 + v * nt + n0 + s3, BS, bar);
-  }
+  mbar_expect_tx(bar, (unsigned)L::TX);
+  tensor_g2s(tile + L::F1, &M.f1, c0, c1, c2, 0, bar);
+  tensor_g2s(tile + L::F2, &M.f2, c0, c1, c2, 0, bar);
+  tensor_g2s(tile + L::F3, &M.f3, c0, c1, c2, 0, bar);
   if (MODE & 8) {
-    bulk_g2s(tile + L::E3, Bface1 + n0, BL, bar);
-    bulk_g2s(tile + L::E1, Bface2 + n0, BS, bar);
-    bulk_g2s(tile + L::E1 + L::WS, Bface2 + n0 + s2, BS, bar);
-    bulk_g2s(tile + L::E1 + 2 * L::WS, Bface3 + n0, BS, bar);
-    bulk_g2s(tile + L::E1 + 3 * L::WS, Bface3 + n0 + s3, BS, bar);
+    tensor_g2s(tile + L::E3, &M.a, c0, c1, c2, bar);
+    tensor_g2s(tile + L::E1, &M.b, c0, c1, c2, bar);
+    tensor_g2s(tile + L::E1 + 2 * L::WS, &M.c, c0, c1, c2, bar);
   } else {
-    bulk_g2s(tile + L::E3, e3 + n0, BL, bar);
-    bulk_g2s(tile + L::E3 + L::WL, e3 + n0 + s2, BL, bar);
-    bulk_g2s(tile + L::E2, e2 + n0, BL, bar);
-    bulk_g2s(tile + L::E2 + L::WL, e2 + n0 + s3, BL, bar);
-    bulk_g2s(tile + L::E1, e1 + n0, BS, bar);
-    bulk_g2s(tile + L::E1 + L::WS, e1 + n0 + s2, BS, bar);
-    bulk_g2s(tile + L::E1 + 2 * L::WS, e1 + n0 + s3, BS, bar);
-    bulk_g2s(tile + L::E1 + 3 * L::WS, e1 + n0 + s2 + s3, BS, bar);
+    tensor_g2s(tile + L::E3, &M.a, c0, c1, c2, bar);
+    tensor_g2s(tile + L::E2, &M.b, c0, c1, c2, bar);
+    tensor_g2s(tile + L::E1, &M.c, c0, c1, c2, bar);
   }
-#pragma unroll
-  for (int v = 0; v < KH_NP; v++) {
-    bulk_g2s(tile + L::PI + v * L::WS, Pi + v * nt + n0, BS, bar);
-    if (L::PS) bulk_g2s(tile + L::PSO + v * L::WS, Ps + v * nt + n0, BS, bar);
-  }
-  if (CORR) {
-    bulk_g2s(tile + L::C1, ct1 + n0, BL, bar);
-    bulk_g2s(tile + L::C2, ct2 + n0, BS, bar);
-    bulk_g2s(tile + L::C2 + L::WS, ct2 + n0 + s2, BS, bar);
-    bulk_g2s(tile + L::C3, ct3 + n0, BS, bar);
-    bulk_g2s(tile + L::C3 + L::WS, ct3 + n0 + s3, BS, bar);
-  }
+  tensor_g2s(tile + L::PI, &M.pi, c0, c1, c2, 0, bar);
+  if (L::PS) tensor_g2s(tile + L::PSO, &M.ps, c0, c1, c2, 0, bar);
 }
 
 // Persistent: the grid is sized to the resident blocks; every warp walks over the tiles T = warp, warp + #warps, ...  The
@@ -767,15 +762,13 @@ __device__ __forceinline__ void issue_tile(const GV& g, double* tile, unsigned l
 // tile t without a second buffer (16 warps x 14 KB already fill the SM's shared memory).
 template <bool FLAT, bool CORR, int MODE>
 __global__ void __launch_bounds__(128, KH_MINB_UPDATE)
-update_tma_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps, double* __restrict__ Pf,
-                  const double* __restrict__ F1, const double* __restrict__ F2, const double* __restrict__ F3,
-                  const double* __restrict__ e1, const double* __restrict__ e2, const double* __restrict__ e3,
+update_tma_kernel(GV g, const __grid_constant__ TileMaps M, const double* __restrict__ Pi, double* __restrict__ Pf,
                   const double* __restrict__ ct1, const double* __restrict__ ct2, const double* __restrict__ ct3,
                   unsigned char* __restrict__ pflag, unsigned char* __restrict__ fflag, unsigned* __restrict__ faillist,
-                  StepScalars* __restrict__ sc, double dt_factor, const double* __restrict__ Bface1, const double* __restrict__ Bface2,
-                  const double* __restrict__ Bface3) {
+                  StepScalars* __restrict__ sc, double dt_factor) {
   using L = TileLayout<FLAT, CORR, MODE>;
-  extern __shared__ __align__(16) double tiles[];
+  extern __shared__ __align__(16) unsigned char tile_raw[];
+  double* const tiles = reinterpret_cast<double*>(tile_raw + ((128u - (smem_u32(tile_raw) & 127u)) & 127u));   // tensor copies land on 128 B boundaries
   // warp-uniform by construction (the shuffle tells the compiler so: tile addresses then live in uniform registers)
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
   double* const tile = tiles + warp * L::DOUBLES;
@@ -797,7 +790,7 @@ update_tma_kernel(GV g, const double* __restrict__ Pi, const double* __restrict_
     tile_origin(T, i0, j, k);
     if (elect_one()) {
       mbar_init(bar, 1);
-      issue_tile<FLAT, CORR, MODE>(g, tile, bar, zidx(g, i0, j, k), Pi, Ps, F1, F2, F3, e1, e2, e3, ct1, ct2, ct3, Bface1, Bface2, Bface3);
+      issue_tile<FLAT, CORR, MODE>(M, tile, bar, i0 + KH_NGH + 1, j + KH_NGH, k + KH_NGH);
     }
     __syncwarp();
   }
@@ -809,11 +802,16 @@ update_tma_kernel(GV g, const double* __restrict__ Pi, const double* __restrict_
     const long p2 = pidx(g, active ? i : g.n1 - 1, j);
     Geo G;                                              // geometry of the zone (L2 resident tables): in flight during the wait
     load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, p2);
+    double ct[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};      // c_top at the zone's faces (corrector): likewise
+    if (CORR) {
+      const long nz = active ? n0 + lane : n0;
+      ct[0] = ct1[nz]; ct[1] = ct1[nz + 1]; ct[2] = ct2[nz]; ct[3] = ct2[nz + g.s2]; ct[4] = ct3[nz]; ct[5] = ct3[nz + g.s3];
+    }
     mbar_wait(bar, parity);
     parity ^= 1u;
     double Uh[KH_NP], W0, r = 0.0;
     {
-      TileAcc<FLAT, CORR, MODE> A{tile + lane};
+      TileAcc<FLAT, CORR, MODE> A{tile + lane, ct};
       update_zone_a<FLAT, CORR, MODE>(g, A, G, p2, Dt, Uh, W0, r);
     }
     __syncwarp();                                       // every lane has read its part of the tile
@@ -823,7 +821,7 @@ update_tma_kernel(GV g, const double* __restrict__ Pi, const double* __restrict_
       tile_origin(T, i0, j, k);
       if (elect_one()) {
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic-proxy reads before the async-proxy overwrite
-        issue_tile<FLAT, CORR, MODE>(g, tile, bar, zidx(g, i0, j, k), Pi, Ps, F1, F2, F3, e1, e2, e3, ct1, ct2, ct3, Bface1, Bface2, Bface3);
+        issue_tile<FLAT, CORR, MODE>(M, tile, bar, i0 + KH_NGH + 1, j + KH_NGH, k + KH_NGH);
       }
     }
     if (active) {
