@@ -680,13 +680,14 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
   update_block_tail<CORR>(sc, rate, ff);
 }
 
-// Variant 2 (even n1; the library's arrays start 8 B past a 16 B boundary so that interior zone i = 0 of every row is
-// 16 B aligned): a warp owns a tile of 32 zones of one x1 row.  One lane issues a TMA bulk copy (cp.async.bulk, completion
-// on the warp's mbarrier) per input row -- 41 (predictor) to 54 (corrector) rows of 256 / 272 B, ~14 KB per warp -- so that
-// ALL streamed inputs of the tile are in flight at once and cost neither registers nor issue slots of the other lanes; the
-// geometry loads go out meanwhile.  After the wait the zone arithmetic reads shared memory only.  (The per-thread variant
-// keeps ~5 loads in flight per warp and spends 58 % of its cycles with every warp waiting on one of five dependent load
-// phases: profiles/r02_*.)
+// Variant 2 (even n1: the padded row length must be a multiple of 16 B for the tensor maps): a warp owns a tile of 32 zones of one
+// x1 row.  One elected lane issues 8 (predictor) or 9 (corrector) TMA tensor copies (cp.async.bulk.tensor, completion on the
+// warp's mbarrier) -- one box per input array: 5 flux components x 2 faces, 4 edge EMFs, 8 primitives ... -- 10 - 12 KB per warp,
+// so that ALL streamed inputs of the tile are in flight at once and cost neither registers nor issue slots of the other lanes;
+// the geometry and c_top loads go out meanwhile.  After the wait the zone arithmetic reads shared memory only.  (The per-thread
+// variant keeps ~5 loads in flight per warp and spends 58 % of its cycles with every warp waiting on one of five dependent load
+// phases; 41 - 54 row-wise bulk copies instead of the boxes cost 13 % of the kernel's instructions in address arithmetic:
+// profiles/r02_*.)
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
@@ -724,10 +725,6 @@ struct alignas(64) TileMaps {
   CUtensorMap pi, ps;          // primitives, box (32,1,1,8)
 };
 
-__device__ __forceinline__ void bulk_g2s(double* dst, const double* src, unsigned bytes, unsigned long long* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)), "l"(src),
-               "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
 
 __device__ __forceinline__ bool elect_one() {     // one lane of the (converged) warp, chosen by the hardware
   unsigned p;

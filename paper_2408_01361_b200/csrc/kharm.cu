@@ -79,6 +79,8 @@ struct kh_grid {
   cudaEvent_t ev_fork, ev_join[2];
   bool flux_concurrent;
   bool update_tma;            // update_tma_kernel (needs an even padded row length) instead of update_kernel
+  // tensor maps of the update kernel's tile copies (cuTensorMapEncodeTiled, once per grid): one per array and box shape
+  CUtensorMap mapF[3], mapE[3], mapP[3], mapBf[3][3];
   int march_J;                // 0 = chosen by march_chunk()
   double prof_ms[KH_K_COUNT];
   long long prof_n[KH_K_COUNT];
@@ -164,8 +166,50 @@ static void setup_march_kernels() {
   setup_march_one<3, 0, true>(); setup_march_one<3, 1, true>(); setup_march_one<3, 0, false>(); setup_march_one<3, 1, false>();
 }
 
+// A tensor map over one zone array as ALLOCATED (the array proper starts one double later: TileMaps): rank 3 (nt1, nt2, nt3) or,
+// with nvar > 1, rank 4 (nt1, nt2, nt3, nvar); box = the tile's box.  false if the driver entry point or the encoding fails.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess) fn = (EncodeTiledFn)p;
+    cudaGetLastError();
+  }
+  return fn;
+}
+static bool make_tile_map(CUtensorMap* map, const double* array, const GV& v, int nvar, int b0, int b1, int b2) {
+  EncodeTiledFn fn = encode_tiled_fn();
+  if (!fn) return false;
+  const cuuint32_t rank = nvar > 1 ? 4 : 3;
+  cuuint64_t dims[4] = {(cuuint64_t)v.nt1, (cuuint64_t)v.nt2, (cuuint64_t)v.nt3, (cuuint64_t)nvar};
+  cuuint64_t strides[3] = {(cuuint64_t)v.nt1 * 8, (cuuint64_t)v.s3 * 8, (cuuint64_t)v.ntot * 8};      // bytes, dimensions 1 .. rank - 1
+  cuuint32_t box[4] = {(cuuint32_t)b0, (cuuint32_t)b1, (cuuint32_t)b2, (cuuint32_t)nvar};
+  cuuint32_t es[4] = {1, 1, 1, 1};
+  return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, rank, (void*)(array - 1), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+static bool make_tile_maps(kh_grid* g) {
+  const GV& v = g->gv;
+  bool ok = make_tile_map(&g->mapF[0], g->F[0], v, 5, 34, 1, 1) && make_tile_map(&g->mapF[1], g->F[1], v, 5, 32, 2, 1) &&
+            make_tile_map(&g->mapF[2], g->F[2], v, 5, 32, 1, 2);
+  // e3 at (i, i+1) x (j, j+1); e2 at (i, i+1) x (k, k+1); e1 at (j, j+1) x (k, k+1)
+  ok = ok && make_tile_map(&g->mapE[2], g->emf[2], v, 1, 34, 2, 1) && make_tile_map(&g->mapE[1], g->emf[1], v, 1, 34, 1, 2) &&
+       make_tile_map(&g->mapE[0], g->emf[0], v, 1, 32, 2, 2);
+  for (int b = 0; b < 3 && ok; b++) ok = make_tile_map(&g->mapP[b], g->P[b], v, KH_NP, 32, 1, 1);
+  if (g->p.transport == KH_B_FACE_CT)
+    for (int b = 0; b < 3 && ok; b++)
+      ok = make_tile_map(&g->mapBf[b][0], g->Bf[b][0], v, 1, 34, 1, 1) && make_tile_map(&g->mapBf[b][1], g->Bf[b][1], v, 1, 32, 2, 1) &&
+           make_tile_map(&g->mapBf[b][2], g->Bf[b][2], v, 1, 32, 1, 2);
+  return ok;
+}
+
 template <bool FL, bool CO, int MODE>
-static constexpr size_t tile_smem_bytes() { return 4 * (size_t)TileLayout<FL, CO, MODE>::BYTES + 64; }     // 4 warp tiles + 4 mbarriers
+static constexpr size_t tile_smem_bytes() { return 4 * (size_t)TileLayout<FL, CO, MODE>::BYTES + 64 + 128; }     // 4 warp tiles + 4 mbarriers + alignment to 128 B
 template <bool FL, bool CO, int MODE>
 static cudaError_t setup_update_tma_one() {
   cudaError_t e = cudaFuncSetAttribute(update_tma_kernel<FL, CO, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_smem_bytes<FL, CO, MODE>());
@@ -329,9 +373,24 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
     const unsigned tgrid = (unsigned)(tgroups < 4L * g->sm_count ? tgroups : 4L * g->sm_count);
 #define UPD_ARGS v, Pi, Ps, Pf, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, \
                  g->fflag, g->faillist, g->sc, dt_factor, fb1, fb2, fb3
+    TileMaps M;
+    if (g->update_tma) {
+      auto pbuf = [&](const double* q) { for (int b = 0; b < 3; b++) if (g->P[b] == q) return b; return 0; };
+      M.f1 = g->mapF[0]; M.f2 = g->mapF[1]; M.f3 = g->mapF[2];
+      M.pi = g->mapP[pbuf(Pi)]; M.ps = g->mapP[pbuf(Ps)];
+      if (fb1) {
+        int st = 0;
+        for (int b = 0; b < 3; b++) if (g->Bf[b][0] == fb1) st = b;
+        M.a = g->mapBf[st][0]; M.b = g->mapBf[st][1]; M.c = g->mapBf[st][2];
+      } else {
+        M.a = g->mapE[2]; M.b = g->mapE[1]; M.c = g->mapE[0];
+      }
+    }
 #define UPD(FL, CO, IN)                                                                                       \
   do {                                                                                                        \
-    if (g->update_tma) update_tma_kernel<FL, CO, IN><<<tgrid, 128, tile_smem_bytes<FL, CO, IN>(), g->stream>>>(UPD_ARGS); \
+    if (g->update_tma)                                                                                        \
+      update_tma_kernel<FL, CO, IN><<<tgrid, 128, tile_smem_bytes<FL, CO, IN>(), g->stream>>>(v, M, Pi, Pf, g->ctop[0], g->ctop[1], g->ctop[2], \
+                                                                                               g->pflag, g->fflag, g->faillist, g->sc, dt_factor); \
     else update_kernel<FL, CO, IN><<<grid, 128, 0, g->stream>>>(UPD_ARGS);                                   \
   } while (0)
     prof_begin(g, KH_K_UPDATE);
@@ -514,6 +573,7 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   g->update_tma = (p->n1 % 2 == 0);
   if (const char* e = getenv("KH_UPDATE_TMA")) g->update_tma = g->update_tma && atoi(e) != 0;
   if (g->update_tma) {
+    // (the maps themselves are encoded after the allocations below)
     // the FOFC pass and the face-CT flag select the MODE at launch: set up every instantiation this grid can launch
     for (int face = 0; face < 2; face++) {
       if (face && p->transport != KH_B_FACE_CT) continue;
@@ -588,6 +648,7 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   if (cudaMemcpyAsync(g->sc, g->sc_host, sizeof(StepScalars), cudaMemcpyHostToDevice, g->stream) != cudaSuccess) { kh_grid_destroy(g); return KH_ECUDA; }
   for (int l = 0; l < 4; l++) v.geom[l] = g->geom[l];
   v.conn = g->conn; v.dg = g->dg; v.floorp = g->floorp;
+  if (g->update_tma && !make_tile_maps(g)) g->update_tma = false;      // no tensor maps: the per-thread update kernel
 
   GeomPar gp;
   gp.coords = p->coords; gp.a = p->a; gp.hslope = p->hslope; gp.poly_xt = p->poly_xt; gp.poly_alpha = p->poly_alpha;
