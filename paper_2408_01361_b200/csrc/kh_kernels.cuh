@@ -515,8 +515,8 @@ struct TileAcc {
 // Phase A: everything that consumes the streamed inputs -- the advanced conserved state Uh = U_f / sqrt(-g), the guess W0 and
 // (corrector) the zone's CFL rate.
 template <bool FLAT, bool CORR, int MODE, class ACC>
-__device__ __forceinline__ void update_zone_a(const GV& g, const ACC& A, const Geo& G, long p2, double Dt, double Uh[KH_NP], double& W0,
-                                              double& rate) {
+__device__ __forceinline__ void update_zone_a(const GV& g, const ACC& A, const Geo& G, const double* __restrict__ dg, long dgm, double Dt,
+                                              double Uh[KH_NP], double& W0, double& rate) {
   const double ialpha = FLAT ? 1.0 : -G.n00 * G.alpha;
   const double gm1 = g.gam - 1.0;
   double S1 = 0.0, S2 = 0.0;
@@ -542,11 +542,10 @@ __device__ __forceinline__ void update_zone_a(const GV& g, const ACC& A, const G
         ptot = fma(0.5, D.bsq, pg);
       }
       // T^{kap lam} = (w + b^2) u^kap u^lam + (p + b^2/2) g^{kap lam} - b^kap b^lam on the packed pairs with d g != 0
-      const double* __restrict__ dg = g.dg + p2;
-      const long m = g.n2d;
+      // dg: this zone's column of the source table, component stride dgm (the global table, or its row staged in shared memory)
       double eu0 = ee * D.ucon[0], eu1 = ee * D.ucon[1], eu2 = ee * D.ucon[2], eu3 = ee * D.ucon[3];
 #define KH_T(a, b, gc) fma(eu##a, D.ucon[b], fma(ptot, gc, -D.bcon[a] * D.bcon[b]))
-#define KH_ACC(c, T) { double T_ = (T); S1 = fma(T_, __ldg(dg + (long)(c) * m), S1); S2 = fma(T_, __ldg(dg + (long)(10 + (c)) * m), S2); }
+#define KH_ACC(c, T) { double T_ = (T); S1 = fma(T_, dg[(long)(c) * dgm], S1); S2 = fma(T_, dg[(long)(10 + (c)) * dgm], S2); }
       KH_ACC(G00, KH_T(0, 0, G.n00));
       KH_ACC(G01, KH_T(0, 1, G.n01));
       KH_ACC(G03, fma(eu0, D.ucon[3], -D.bcon[0] * D.bcon[3]));            // g^03 = 0
@@ -596,17 +595,13 @@ __device__ __forceinline__ bool rate_nonfinite(double r) { return ((unsigned)__d
 
 // Phase B: inversion + floors of the advanced state, stores.  Pi: the guess (global memory; read only by the rare failed zone).
 template <bool FLAT, int MODE>
-__device__ __forceinline__ void update_zone_b(const GV& g, const Geo& G, const double Uh[KH_NP], double W0, int i, int j, int k, long n,
-                                              long p2, const double* __restrict__ Pi, double* __restrict__ Pf, unsigned char* __restrict__ pflag,
+__device__ __forceinline__ void update_zone_b(const GV& g, const Geo& G, const double Uh[KH_NP], double W0, double rho_g, double u_g, long n,
+                                              const double* __restrict__ Pi, double* __restrict__ Pf, unsigned char* __restrict__ pflag,
                                               unsigned char* __restrict__ fflag, unsigned* __restrict__ faillist,
                                               StepScalars* __restrict__ sc, int& pf_flag, int& ff) {
   const long nt = g.ntot;
   double pf[KH_NP];
-  {
-    const double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2);
-    const double u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
-    pf_flag = invert_with_floors<FLAT, MODE & 1>(G, Uh, W0, g.gam, g.fp, (MODE & 7) >> 1, rho_g, u_g, pf, ff);
-  }
+  pf_flag = invert_with_floors<FLAT, MODE & 1>(G, Uh, W0, g.gam, g.fp, (MODE & 7) >> 1, rho_g, u_g, pf, ff);
   if (pf_flag != 0) {          // rare: the hydro primitives keep the guess (S16); queue the zone for the fix-up
 #pragma unroll
     for (int v = 0; v < 5; v++) pf[v] = Pi[v * nt + n];
@@ -673,9 +668,10 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
     load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, p2);
     GlobalAcc A{Pi, Ps, F1, F2, F3, e1, e2, e3, ct1, ct2, ct3, Bface1, Bface2, Bface3, n, nt, g.s2, g.s3};
     double Uh[KH_NP], W0;
-    update_zone_a<FLAT, CORR, MODE>(g, A, G, p2, Dt, Uh, W0, rate);
+    update_zone_a<FLAT, CORR, MODE>(g, A, G, g.dg + p2, g.n2d, Dt, Uh, W0, rate);
     if (CORR && rate_nonfinite(rate)) { sc->nonfinite = 1ULL; rate = 0.0; }
-    update_zone_b<FLAT, MODE>(g, G, Uh, W0, i, j, k, n, p2, Pi, Pf, pflag, fflag, faillist, sc, pf_flag, ff);
+    const double rho_g = FLAT ? __ldg(g.floorp) : __ldg(g.floorp + p2), u_g = FLAT ? __ldg(g.floorp + g.n2d) : __ldg(g.floorp + g.n2d + p2);
+    update_zone_b<FLAT, MODE>(g, G, Uh, W0, rho_g, u_g, n, Pi, Pf, pflag, fflag, faillist, sc, pf_flag, ff);
   }
   update_block_tail<CORR>(sc, rate, ff);
 }
@@ -723,6 +719,7 @@ struct alignas(64) TileMaps {
   CUtensorMap f1, f2, f3;      // hydro fluxes, boxes (34,1,1,5), (32,2,1,5), (32,1,2,5)
   CUtensorMap a, b, c;         // e3 (34,2,1), e2 (34,1,2), e1 (32,2,2)   | face CT: Bf1 (34,1,1), Bf2 (32,2,1), Bf3 (32,1,2)
   CUtensorMap pi, ps;          // primitives, box (32,1,1,8)
+  CUtensorMap geo, dgt, flo;   // centre geometry (KH_NGEO), source (KH_NDG) and floor (2) tables as (nt1, nt2, components): boxes (32,1,components)
 };
 
 
@@ -753,81 +750,170 @@ __device__ __forceinline__ void issue_tile(const TileMaps& M, double* tile, unsi
   if (L::PS) tensor_g2s(tile + L::PSO, &M.ps, c0, c1, c2, 0, bar);
 }
 
-// Persistent: the grid is sized to the resident blocks; every warp walks over the tiles T = warp, warp + #warps, ...  The
-// tile buffer is dead once phase A has formed the advanced conserved state, so the NEXT tile's copies are issued before the
-// inversion (phase B, ~60 % of a zone's instructions) and land while it runs: the loads of tile t+1 overlap the arithmetic of
-// tile t without a second buffer (16 warps x 14 KB already fill the SM's shared memory).
+// Persistent: one block of 16 warps per SM.  The tile buffer is dead once phase A has formed the advanced conserved state, so
+// the NEXT tile's copies are issued before the inversion (phase B, ~60 % of a zone's instructions) and land while it runs: the
+// loads of tile t+1 overlap the arithmetic of tile t without a second buffer (16 warps x 13 KB nearly fill the SM's shared memory).
+//
+// Work unit: the tiles (i0, j, k) of KU = 16 TPW consecutive planes k at one (i0, j); warp w takes planes w, w + 16, ... of the
+// unit.  Units are ordered (i0, j, k-block), i0 fastest, and dealt out to the blocks round robin, so that at any moment the grid
+// streams a compact slab of the arrays (an order in which each SM walks a region of its own costs 20 - 40 % in DRAM efficiency).
+// The geometry of a unit -- the rows of the 44 table components at (i0 .. i0 + 31, j), a function of (i, j) only -- is staged in
+// shared memory ONCE per unit by three tensor copies, two units ahead (two buffers): with per-thread loads every warp waited
+// ~5 times per tile for an L2 round trip (36 % of the kernel's stall samples, profiles/r02_ncu_full.md), and the 28 KB of L1 that
+// the tiles leave cannot hold the tables of 16 tiles at different (i0, j).  Protocol: full[b] (mbarrier, tx count) says buffer
+// b holds the unit's rows; done[b] counts the warps that have finished the unit, and the LAST one re-arms full[b] and issues the
+// copies of the unit two ahead -- nobody blocks.  Every warp visits every unit of its block, also one in which it owns no plane.
+#ifndef KH_UPD_TPW
+#define KH_UPD_TPW 4
+#endif
+#define KH_UPD_WARPS 16
+#define KH_GEO_ROWS (KH_NGEO + KH_NDG + 2)
+__device__ __forceinline__ double ld_stream(const double* p) {       // read once: no L1 allocation
+  double v;
+  asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
+  return v;
+}
+// the staged rows: [component][32 zones]; components 0 .. KH_NGEO-1 as in the geometry table, then the source table, then the floors
+__device__ __forceinline__ void load_geo_rows(Geo& G, const double* __restrict__ r) {
+#define KH_LD(c) r[(c) * 32]
+  G.c00 = KH_LD(G00); G.c01 = KH_LD(G01); G.c03 = KH_LD(G03); G.c11 = KH_LD(G11); G.c12 = KH_LD(G12);
+  G.c13 = KH_LD(G13); G.c22 = KH_LD(G22); G.c33 = KH_LD(G33);
+  G.n00 = KH_LD(10 + G00); G.n01 = KH_LD(10 + G01); G.n02 = KH_LD(10 + G02); G.n11 = KH_LD(10 + G11); G.n22 = KH_LD(10 + G22);
+  G.n33 = KH_LD(10 + G33); G.n12 = KH_LD(10 + G12); G.n13 = KH_LD(10 + G13); G.n23 = KH_LD(10 + G23);
+  G.gdet = KH_LD(20); G.alpha = KH_LD(21);
+#undef KH_LD
+}
+__device__ __forceinline__ void issue_geo(const TileMaps& M, double* rows, unsigned long long* bar, int c0, int c1) {
+  mbar_expect_tx(bar, (unsigned)(KH_GEO_ROWS * 32 * 8));
+  tensor_g2s(rows, &M.geo, c0, c1, 0, bar);
+  tensor_g2s(rows + KH_NGEO * 32, &M.dgt, c0, c1, 0, bar);
+  tensor_g2s(rows + (KH_NGEO + KH_NDG) * 32, &M.flo, c0, c1, 0, bar);
+}
+
 template <bool FLAT, bool CORR, int MODE>
-__global__ void __launch_bounds__(128, KH_MINB_UPDATE)
+__global__ void __launch_bounds__(32 * KH_UPD_WARPS, 1)
 update_tma_kernel(GV g, const __grid_constant__ TileMaps M, const double* __restrict__ Pi, double* __restrict__ Pf,
                   const double* __restrict__ ct1, const double* __restrict__ ct2, const double* __restrict__ ct3,
                   unsigned char* __restrict__ pflag, unsigned char* __restrict__ fflag, unsigned* __restrict__ faillist,
                   StepScalars* __restrict__ sc, double dt_factor) {
   using L = TileLayout<FLAT, CORR, MODE>;
+  constexpr unsigned WARPS = KH_UPD_WARPS, TPW = KH_UPD_TPW, KU = WARPS * TPW;
+  constexpr int GEO = FLAT ? 0 : KH_GEO_ROWS * 32;          // doubles per geometry buffer
   extern __shared__ __align__(16) unsigned char tile_raw[];
   double* const tiles = reinterpret_cast<double*>(tile_raw + ((128u - (smem_u32(tile_raw) & 127u)) & 127u));   // tensor copies land on 128 B boundaries
   // warp-uniform by construction (the shuffle tells the compiler so: tile addresses then live in uniform registers)
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
   double* const tile = tiles + warp * L::DOUBLES;
-  unsigned long long* const bar = reinterpret_cast<unsigned long long*>(tiles + 4 * L::DOUBLES) + warp;
+  double* const geo = tiles + WARPS * L::DOUBLES;           // two buffers of GEO doubles
+  unsigned long long* const bars = reinterpret_cast<unsigned long long*>(geo + 2 * GEO);
+  unsigned long long* const bar = bars + warp;              // this warp's tile
+  unsigned long long* const full = bars + WARPS;            // [2]
+  unsigned* const done = reinterpret_cast<unsigned*>(bars + WARPS + 2);      // [2]
   const unsigned tpr = ((unsigned)g.n1 + 31u) >> 5;                      // tiles per row
-  const unsigned ntiles = tpr * (unsigned)g.n2 * (unsigned)g.n3, stride = gridDim.x * 4u;
-  unsigned T = blockIdx.x * 4u + (unsigned)warp;
+  const unsigned upp = tpr * (unsigned)g.n2, nunits = upp * (((unsigned)g.n3 + KU - 1u) / KU);
+  const unsigned groups = gridDim.x;
+  auto unit_origin = [&](unsigned u, int& i0, int& j, int& k0) {
+    const unsigned kb = u / upp, r = u - kb * upp;
+    k0 = (int)(kb * KU);
+    j = (int)(r / tpr);
+    i0 = (int)(r - (unsigned)j * tpr) << 5;
+  };
+  if (!FLAT) {
+    if (warp == 0 && elect_one()) {
+      mbar_init(full, 1); mbar_init(full + 1, 1);
+      done[0] = done[1] = 0u;
+      for (unsigned q = 0; q < 2; q++) {
+        const unsigned u = blockIdx.x + q * groups;
+        if (u < nunits) {
+          int i0, j, k0;
+          unit_origin(u, i0, j, k0);
+          issue_geo(M, geo + q * GEO, full + q, i0 + KH_NGH + 1, j + KH_NGH);
+        }
+      }
+    }
+    __syncthreads();
+  }
   double rate = 0.0;
   int nff = 0;
   const double Dt = dt_factor * sc->dt;
-  auto tile_origin = [&](unsigned t, int& i0, int& j, int& k) {
-    const unsigned row = t / tpr;
-    i0 = (int)(t - row * tpr) << 5;
-    k = (int)(row / (unsigned)g.n2);
-    j = (int)(row - (unsigned)k * (unsigned)g.n2);
+  // the warp's next tile: plane tm of unit tu, at or after the given position
+  unsigned tu = blockIdx.x, tm = 0;
+  int i0 = 0, j = 0, k = 0;
+  auto find_tile = [&]() -> bool {
+    while (tu < nunits) {
+      int k0;
+      unit_origin(tu, i0, j, k0);
+      k = k0 + warp + (int)(WARPS * tm);
+      if (tm < TPW && k < g.n3) return true;
+      tm = 0;
+      tu += groups;
+    }
+    return false;
   };
-  int i0, j, k;
-  if (T < ntiles) {
-    tile_origin(T, i0, j, k);
-    if (elect_one()) {
-      mbar_init(bar, 1);
-      issue_tile<FLAT, CORR, MODE>(M, tile, bar, i0 + KH_NGH + 1, j + KH_NGH, k + KH_NGH);
-    }
-    __syncwarp();
+  bool have = find_tile();
+  if (elect_one()) {
+    mbar_init(bar, 1);
+    if (have) issue_tile<FLAT, CORR, MODE>(M, tile, bar, i0 + KH_NGH + 1, j + KH_NGH, k + KH_NGH);
   }
-  unsigned parity = 0;
-  while (T < ntiles) {
-    const long n0 = zidx(g, i0, j, k);
-    const int i = i0 + lane;
-    const bool active = i < g.n1;
-    const long p2 = pidx(g, active ? i : g.n1 - 1, j);
-    Geo G;                                              // geometry of the zone (L2 resident tables): in flight during the wait
-    load_geo<FLAT, 0, 1>(G, g.geom[0], g.n2d, p2);
-    double ct[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};      // c_top at the zone's faces (corrector): likewise
-    if (CORR) {
-      const long nz = active ? n0 + lane : n0;
-      ct[0] = ct1[nz]; ct[1] = ct1[nz + 1]; ct[2] = ct2[nz]; ct[3] = ct2[nz + g.s2]; ct[4] = ct3[nz]; ct[5] = ct3[nz + g.s3];
-    }
-    mbar_wait(bar, parity);
-    parity ^= 1u;
-    double Uh[KH_NP], W0, r = 0.0;
-    {
-      TileAcc<FLAT, CORR, MODE> A{tile + lane, ct};
-      update_zone_a<FLAT, CORR, MODE>(g, A, G, p2, Dt, Uh, W0, r);
-    }
-    __syncwarp();                                       // every lane has read its part of the tile
-    const int jz = j, kz = k;
-    T += stride;
-    if (T < ntiles) {
-      tile_origin(T, i0, j, k);
-      if (elect_one()) {
+  __syncwarp();
+  unsigned parity = 0, q = 0;
+  for (unsigned u = blockIdx.x; u < nunits; u += groups, q++) {
+    const unsigned b = q & 1u;
+    const double* const rows = geo + b * GEO;
+    if (!FLAT) mbar_wait(full + b, (q >> 1) & 1u);
+    while (have && tu == u) {
+      const long n0 = zidx(g, i0, j, k);
+      const int i = i0 + lane;
+      const bool active = i < g.n1;
+      const int gl = active ? lane : g.n1 - 1 - i0;     // a lane beyond the row computes on the last zone's geometry
+      Geo G;
+      if (FLAT) load_geo<true, 0, 1>(G, nullptr, 0, 0);
+      else load_geo_rows(G, rows + gl);
+      double ct[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};      // c_top at the zone's faces (corrector): in flight during the wait
+      if (CORR) {
+        const long nz = active ? n0 + lane : n0;
+        ct[0] = ld_stream(ct1 + nz); ct[1] = ld_stream(ct1 + nz + 1); ct[2] = ld_stream(ct2 + nz); ct[3] = ld_stream(ct2 + nz + g.s2);
+        ct[4] = ld_stream(ct3 + nz); ct[5] = ld_stream(ct3 + nz + g.s3);
+      }
+      mbar_wait(bar, parity);
+      parity ^= 1u;
+      double Uh[KH_NP], W0, r = 0.0;
+      {
+        TileAcc<FLAT, CORR, MODE> A{tile + lane, ct};
+        update_zone_a<FLAT, CORR, MODE>(g, A, G, rows + KH_NGEO * 32 + gl, 32, Dt, Uh, W0, r);
+      }
+      __syncwarp();                                       // every lane has read its part of the tile
+      const long nz = n0 + lane;
+      tm++;
+      have = find_tile();
+      if (have && elect_one()) {
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic-proxy reads before the async-proxy overwrite
         issue_tile<FLAT, CORR, MODE>(M, tile, bar, i0 + KH_NGH + 1, j + KH_NGH, k + KH_NGH);
       }
+      if (active) {
+        const double rho_g = FLAT ? __ldg(g.floorp) : rows[(KH_NGEO + KH_NDG) * 32 + gl];
+        const double u_g = FLAT ? __ldg(g.floorp + g.n2d) : rows[(KH_NGEO + KH_NDG + 1) * 32 + gl];
+        int pf_flag, ff;
+        update_zone_b<FLAT, MODE>(g, G, Uh, W0, rho_g, u_g, nz, Pi, Pf, pflag, fflag, faillist, sc, pf_flag, ff);
+        nff += (ff != 0);
+        if (CORR) { if (rate_nonfinite(r)) sc->nonfinite = 1ULL; else rate = fmax(rate, r); }
+      }
+      __syncwarp();
     }
-    if (active) {
-      int pf_flag, ff;
-      update_zone_b<FLAT, MODE>(g, G, Uh, W0, i, jz, kz, n0 + lane, p2, Pi, Pf, pflag, fflag, faillist, sc, pf_flag, ff);
-      nff += (ff != 0);
-      if (CORR) { if (rate_nonfinite(r)) sc->nonfinite = 1ULL; else rate = fmax(rate, r); }
+    if (!FLAT) {      // this warp is through with the unit's rows; the last of the 16 refills the buffer for the unit two ahead
+      __syncwarp();
+      if (elect_one() && atomicAdd(done + b, 1u) == WARPS - 1u) {
+        done[b] = 0u;
+        const unsigned un = u + 2u * groups;
+        if (un < nunits) {
+          int ui, uj, uk;
+          unit_origin(un, ui, uj, uk);
+          __threadfence_block();
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          issue_geo(M, geo + b * GEO, full + b, ui + KH_NGH + 1, uj + KH_NGH);
+        }
+      }
     }
-    __syncwarp();
   }
   // block-level bookkeeping, once per block: floor-hit counter and the CFL rate maximum
 #pragma unroll

@@ -80,7 +80,7 @@ struct kh_grid {
   bool flux_concurrent;
   bool update_tma;            // update_tma_kernel (needs an even padded row length) instead of update_kernel
   // tensor maps of the update kernel's tile copies (cuTensorMapEncodeTiled, once per grid): one per array and box shape
-  CUtensorMap mapF[3], mapE[3], mapP[3], mapBf[3][3];
+  CUtensorMap mapF[3], mapE[3], mapP[3], mapBf[3][3], mapT[3];     // mapT: centre geometry, source and floor tables
   int march_J;                // 0 = chosen by march_chunk()
   double prof_ms[KH_K_COUNT];
   long long prof_n[KH_K_COUNT];
@@ -193,8 +193,24 @@ static bool make_tile_map(CUtensorMap* map, const double* array, const GV& v, in
   return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, rank, (void*)(array - 1), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
+// a table of `comps` components over the padded (x1, x2) plane: box = 32 zones of one row, all components.  Like the zone arrays
+// the table starts one double past its allocation, which is what the map describes: every box then starts on a 16 B boundary
+// (a box starting 8 B off one raises an illegal-instruction fault on sm_100a)
+static bool make_table_map(CUtensorMap* map, const double* table, const GV& v, int comps) {
+  EncodeTiledFn fn = encode_tiled_fn();
+  if (!fn) return false;
+  cuuint64_t dims[3] = {(cuuint64_t)v.nt1, (cuuint64_t)v.nt2, (cuuint64_t)comps};
+  cuuint64_t strides[2] = {(cuuint64_t)v.nt1 * 8, (cuuint64_t)v.n2d * 8};
+  cuuint32_t box[3] = {32, 1, (cuuint32_t)comps};
+  cuuint32_t es[3] = {1, 1, 1};
+  return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)(table - 1), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 static bool make_tile_maps(kh_grid* g) {
   const GV& v = g->gv;
+  if (!g->flat && !(make_table_map(&g->mapT[0], g->geom[0], v, KH_NGEO) && make_table_map(&g->mapT[1], g->dg, v, KH_NDG) &&
+                    make_table_map(&g->mapT[2], g->floorp, v, 2)))
+    return false;
   bool ok = make_tile_map(&g->mapF[0], g->F[0], v, 5, 34, 1, 1) && make_tile_map(&g->mapF[1], g->F[1], v, 5, 32, 2, 1) &&
             make_tile_map(&g->mapF[2], g->F[2], v, 5, 32, 1, 2);
   // e3 at (i, i+1) x (j, j+1); e2 at (i, i+1) x (k, k+1); e1 at (j, j+1) x (k, k+1)
@@ -209,7 +225,9 @@ static bool make_tile_maps(kh_grid* g) {
 }
 
 template <bool FL, bool CO, int MODE>
-static constexpr size_t tile_smem_bytes() { return 4 * (size_t)TileLayout<FL, CO, MODE>::BYTES + 64 + 128; }     // 4 warp tiles + 4 mbarriers + alignment to 128 B
+static constexpr size_t tile_smem_bytes() {     // one tile and one mbarrier per warp, two geometry buffers with their barriers and counters, alignment to 128 B
+  return KH_UPD_WARPS * ((size_t)TileLayout<FL, CO, MODE>::BYTES + 8) + (FL ? 0 : 2 * (size_t)KH_GEO_ROWS * 32 * 8) + 32 + 128;
+}
 template <bool FL, bool CO, int MODE>
 static cudaError_t setup_update_tma_one() {
   cudaError_t e = cudaFuncSetAttribute(update_tma_kernel<FL, CO, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_smem_bytes<FL, CO, MODE>());
@@ -369,14 +387,15 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
     }
     const unsigned grid = (unsigned)(((long)v.n1 * v.n2 * v.n3 + 127) / 128);
     // persistent: as many blocks as stay resident (4 per SM), never more than there are groups of 4 warp tiles
-    const long tgroups = ((long)((v.n1 + 31) / 32) * v.n2 * v.n3 + 3) / 4;
-    const unsigned tgrid = (unsigned)(tgroups < 4L * g->sm_count ? tgroups : 4L * g->sm_count);
+    const long tgroups = (long)((v.n1 + 31) / 32) * v.n2 * ((v.n3 + 16 * KH_UPD_TPW - 1) / (16 * KH_UPD_TPW));      // work units of update_tma_kernel
+    const unsigned tgrid = (unsigned)(tgroups < (long)g->sm_count ? tgroups : (long)g->sm_count) * (16 / KH_UPD_WARPS);
 #define UPD_ARGS v, Pi, Ps, Pf, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, \
                  g->fflag, g->faillist, g->sc, dt_factor, fb1, fb2, fb3
     TileMaps M;
     if (g->update_tma) {
       auto pbuf = [&](const double* q) { for (int b = 0; b < 3; b++) if (g->P[b] == q) return b; return 0; };
       M.f1 = g->mapF[0]; M.f2 = g->mapF[1]; M.f3 = g->mapF[2];
+      M.geo = g->mapT[0]; M.dgt = g->mapT[1]; M.flo = g->mapT[2];
       M.pi = g->mapP[pbuf(Pi)]; M.ps = g->mapP[pbuf(Ps)];
       if (fb1) {
         int st = 0;
@@ -389,7 +408,7 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
 #define UPD(FL, CO, IN)                                                                                       \
   do {                                                                                                        \
     if (g->update_tma)                                                                                        \
-      update_tma_kernel<FL, CO, IN><<<tgrid, 128, tile_smem_bytes<FL, CO, IN>(), g->stream>>>(v, M, Pi, Pf, g->ctop[0], g->ctop[1], g->ctop[2], \
+      update_tma_kernel<FL, CO, IN><<<tgrid, 32 * KH_UPD_WARPS, tile_smem_bytes<FL, CO, IN>(), g->stream>>>(v, M, Pi, Pf, g->ctop[0], g->ctop[1], g->ctop[2], \
                                                                                                g->pflag, g->fflag, g->faillist, g->sc, dt_factor); \
     else update_kernel<FL, CO, IN><<<grid, 128, 0, g->stream>>>(UPD_ARGS);                                   \
   } while (0)
@@ -493,8 +512,9 @@ const char* kh_last_cuda_error(void) { return g_cuda_err; }
 int kh_grid_destroy(kh_grid* g) {
   if (!g) return KH_OK;
   destroy_graphs(g);
-  for (int l = 0; l < 4; l++) cudaFree(g->geom[l]);
-  cudaFree(g->conn); cudaFree(g->dg); cudaFree(g->floorp);
+  free_shifted(g->geom[0]);
+  for (int l = 1; l < 4; l++) cudaFree(g->geom[l]);
+  cudaFree(g->conn); free_shifted(g->dg); free_shifted(g->floorp);
   for (int b = 0; b < 3; b++) { free_shifted(g->P[b]); free_shifted(g->F[b]); free_shifted(g->ctop[b]); free_shifted(g->emf[b]); }
   cudaFree(g->pflag); cudaFree(g->fflag); cudaFree(g->mask);
   for (int b = 0; b < 3; b++) for (int d = 0; d < 3; d++) free_shifted(g->Bf[b][d]);
@@ -623,10 +643,12 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
     (ptr) = raw_ + 1;                                                           \
   } while (0)
   const size_t fb = sizeof(double) * v.ntot;
-  for (int l = 0; l < 4; l++) ALLOC(g->geom[l], sizeof(double) * KH_NGEO * v.n2d);
+  // the tables the update kernel stages by tensor copies are shifted like the zone arrays (the copy of a row starts at zone i0)
+  ALLOC_SHIFTED(g->geom[0], sizeof(double) * KH_NGEO * v.n2d);
+  for (int l = 1; l < 4; l++) ALLOC(g->geom[l], sizeof(double) * KH_NGEO * v.n2d);
   ALLOC(g->conn, sizeof(double) * KH_NCONN * v.n2d);
-  ALLOC(g->dg, sizeof(double) * KH_NDG * v.n2d);
-  ALLOC(g->floorp, sizeof(double) * 2 * v.n2d);
+  ALLOC_SHIFTED(g->dg, sizeof(double) * KH_NDG * v.n2d);
+  ALLOC_SHIFTED(g->floorp, sizeof(double) * 2 * v.n2d);
   for (int b = 0; b < 3; b++) {
     ALLOC_SHIFTED(g->P[b], KH_NP * fb);
     ALLOC_SHIFTED(g->F[b], KH_NP * fb);
