@@ -38,7 +38,8 @@ extern "C" {
 #define KH_NG 3
 #define KH_NPRIM 8
 
-enum { KH_OK = 0, KH_EINVAL = -1, KH_ENOMEM = -2, KH_ECUDA = -3, KH_ENAN = -4 };
+enum { KH_OK = 0, KH_EINVAL = -1, KH_ENOMEM = -2, KH_ECUDA = -3, KH_ENAN = -4,
+       KH_ESIZE = -5 /* kh_divB_noalloc: more corners than its static scratch covers (KH_NOALLOC_MAX_CORNERS) */ };
 enum { KH_MINKOWSKI = 0, KH_KS = 1, KH_FMKS = 2 };                            /* coords          */
 enum { KH_BC_PERIODIC = 0, KH_BC_OUTFLOW = 1, KH_BC_POLAR = 2, KH_BC_FIXED = 3,
        KH_BC_BLOCK = 4 /* ghost layers owned by a neighbouring block: kh_link_blocks, kh_step_blocks */ };
@@ -130,6 +131,25 @@ int kh_step(kh_grid* g, double dt, double* dt_next);
 
 /* max |div B| of the corner-centred divergence that Flux-CT preserves.  HOST double. */
 int kh_divB(kh_grid* g, double* max_abs);
+
+/* The same divergence for callers that cannot allocate (code under CUDA-graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): no grid handle, no cudaMalloc / cudaFree / allocating library call, no synchronisation -- a memset node and one
+ * kernel on `cuda_stream` (NULL: the legacy default stream).  The reduction's scratch is a static device array of
+ * KH_NOALLOC_SCRATCH_BYTES that every GPU loading the library holds until exit; its address is looked up once per device on
+ * the first call made with that device current (make one call before starting a capture).
+ *   B        DEVICE, the field B^1..B^3 in the padded layout of kh_get_prims(with_ghosts = 1): [3][n3+6][n2+6][n1+6]
+ *            (the last three components of that array); read only, owned by the caller;
+ *   gdet     DEVICE, sqrt(-g) at zone centres as kh_get_geom(loc = 0) returns it, [n2+6][n1+6]; NULL = 1 (Minkowski);
+ *   dx1..3   zone sizes (> 0);  lower_mask  bit d-1 set: the corners on the lower boundary plane of direction d count
+ *            (their ghost zones hold data: periodic images or a neighbouring block's zones) -- kh_divB's own rule;
+ *   max_abs  DEVICE, one double, written by the kernel: valid once the stream has reached it (+inf if a corner is NaN).
+ * Errors: KH_EINVAL (NULL B / max_abs, sizes < 1, dx <= 0), KH_ESIZE when the corner count exceeds KH_NOALLOC_MAX_CORNERS
+ * (nothing is enqueued), KH_ECUDA.  Every call shares the one scratch array per device: calls that overlap on the GPU (two
+ * streams, two threads) race; calls ordered on one stream do not. */
+#define KH_NOALLOC_MAX_CORNERS 16777216LL                       /* 65536 blocks of 256 corners: a 256^3 block fits */
+#define KH_NOALLOC_SCRATCH_BYTES (8 * (32 + KH_NOALLOC_MAX_CORNERS / 256))
+int kh_divB_noalloc(const double* B, const double* gdet, int n1, int n2, int n3, double dx1, double dx2, double dx3, int lower_mask,
+                    double* max_abs, void* cuda_stream);
 
 /* Number of zones with pflag != 0 and with fflag != 0 in the last sub-step (HOST ints; may be NULL). */
 int kh_count_flags(kh_grid* g, long long* n_pflag, long long* n_fflag);

@@ -6,6 +6,6 @@ This package is the thin Python binding (argument marshalling only).  There is n
 importing works anywhere, but creating a Grid needs libkharm.so and a CUDA device.
 """
 from .binding import (Grid, KharmError, Params, lib, make_params, measure_fp64_peak,  # noqa: F401
-                      link_blocks, exchange_halos, step_blocks,
+                      link_blocks, exchange_halos, step_blocks, divB_noalloc, NOALLOC_MAX_CORNERS,
                       MINKOWSKI, KS, FMKS, BC_PERIODIC, BC_OUTFLOW, BC_POLAR, BC_FIXED, BC_BLOCK, RECON_MC, RECON_WENO5,
                       LOC_CENT, LOC_FACE1, LOC_FACE2, LOC_FACE3, NG, EXPORTED_SYMBOLS, KERNEL_KINDS)

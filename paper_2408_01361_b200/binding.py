@@ -22,6 +22,7 @@ EXPORTED_SYMBOLS = (
     "kh_estimate_dt", "kh_step", "kh_divB", "kh_set_face_B", "kh_get_face_B", "kh_divB_face", "kh_count_flags", "kh_get_geom", "kh_get_conn", "kh_get_flux",
     "kh_get_emf", "kh_debug_fixup", "kh_debug_predictor", "kh_launch_count", "kh_set_graph", "kh_set_profile", "kh_get_profile", "kh_measure_fp64_peak", "kh_strerror",
     "kh_last_cuda_error", "kh_get_stream", "kh_sync", "kh_link_blocks", "kh_exchange_halos", "kh_step_blocks",
+    "kh_divB_noalloc",
 )
 
 
@@ -100,6 +101,8 @@ def lib():
         L.kh_link_blocks.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.kh_exchange_halos.argtypes = [C.POINTER(C.c_void_p), C.c_int]
         L.kh_step_blocks.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_double, C.POINTER(C.c_double)]
+        L.kh_divB_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int,
+                                      C.c_void_p, C.c_void_p]
         _LIB = L
     return _LIB
 
@@ -119,6 +122,16 @@ def measure_fp64_peak():
     tf, mhz = C.c_double(), C.c_double()
     _chk(lib().kh_measure_fp64_peak(C.byref(tf), C.byref(mhz)))
     return tf.value, mhz.value
+
+
+NOALLOC_MAX_CORNERS = 16777216      # KH_NOALLOC_MAX_CORNERS
+
+
+def divB_noalloc(B_ptr, gdet_ptr, n, dx, lower_mask, out_ptr, stream=0):
+    """kh_divB_noalloc: B_ptr, gdet_ptr (0 = Minkowski) and out_ptr are DEVICE addresses (ints); n = (n1, n2, n3), dx likewise.
+    Enqueues on `stream` and returns; the caller synchronises before reading the double at out_ptr."""
+    _chk(lib().kh_divB_noalloc(C.c_void_p(B_ptr), C.c_void_p(gdet_ptr or None), int(n[0]), int(n[1]), int(n[2]), float(dx[0]),
+                               float(dx[1]), float(dx[2]), int(lower_mask), C.c_void_p(out_ptr), C.c_void_p(stream or None)))
 
 
 def _handles(blocks):

@@ -11,7 +11,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 SRC = os.path.join(HERE, "csrc", "kharm.cu")
-DEPS = [SRC] + [os.path.join(HERE, "csrc", f) for f in ("kh_device.cuh", "kh_geometry.cuh", "kh_kernels.cuh")] + \
+SRC_NOALLOC = os.path.join(HERE, "csrc", "kh_noalloc.cu")      # kh_divB_noalloc: a translation unit of its own (static scratch)
+DEPS = [SRC, SRC_NOALLOC] + [os.path.join(HERE, "csrc", f) for f in ("kh_device.cuh", "kh_geometry.cuh", "kh_kernels.cuh")] + \
        [os.path.join(ROOT, "include", "kharm.h")]
 OUT = os.path.join(HERE, "libkharm.so")
 
@@ -23,7 +24,7 @@ def build(force=False, verbose=False):
     if not force and os.path.exists(OUT) and all(os.path.getmtime(d) <= os.path.getmtime(OUT) for d in DEPS):
         return OUT
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", OUT, SRC]
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", OUT, SRC, SRC_NOALLOC]
     if verbose:
         print(" ".join(cmd))
     subprocess.check_call(cmd)

@@ -504,6 +504,7 @@ const char* kh_strerror(int code) {
     case KH_ENOMEM: return "out of memory";
     case KH_ECUDA: return "CUDA error (see kh_last_cuda_error)";
     case KH_ENAN: return "non-finite value";
+    case KH_ESIZE: return "problem larger than the static scratch of the allocation-free entry point (KH_NOALLOC_MAX_CORNERS)";
     default: return "unknown error";
   }
 }
