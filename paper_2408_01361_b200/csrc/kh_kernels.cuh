@@ -951,25 +951,33 @@ __global__ void reset_counters_kernel(StepScalars* sc, int also_rate) {
 // ---------------------------------------------------------------------------------------------
 // ghost zone number t of the shell (t >= the shell size: nothing)
 __device__ __forceinline__ void fill_zone(const GV& g, double* __restrict__ P, unsigned char* __restrict__ flag, long t) {
-  // ghost shell = slab A (k ghost, all i, j) + slab B (j ghost, k interior, all i) + slab C (i ghost, j, k interior)
-  const long nA = (long)g.nt1 * g.nt2 * (2 * KH_NGH), nB = (long)g.nt1 * (2 * KH_NGH) * g.n3, nC = (long)(2 * KH_NGH) * g.n2 * g.n3;
+  // ghost shell = slab A (k ghost, all i, j) + slab B (j ghost, k interior, all i) + slab C (i ghost, j, k interior).
+  // 32-bit index arithmetic: the shell has fewer than 2^32 zones on any block that fits a GPU (kh_grid_create checks), and a
+  // 64-bit division costs ~100 instructions where this kernel has little else to do.
+  const unsigned nt1 = (unsigned)g.nt1, nt2 = (unsigned)g.nt2;
+  const unsigned nA = nt1 * nt2 * (2u * KH_NGH), nB = nt1 * (2u * KH_NGH) * (unsigned)g.n3, nC = (2u * KH_NGH) * (unsigned)g.n2 * (unsigned)g.n3;
+  if (t >= (long)nA + (long)nB + (long)nC) return;
+  unsigned u = (unsigned)t;
   int a, b, c;    // interior-based indices of the ghost zone
-  if (t < nA) {
-    a = (int)(t % g.nt1) - KH_NGH; long r = t / g.nt1;
-    b = (int)(r % g.nt2) - KH_NGH; int m = (int)(r / g.nt2);
-    c = m < KH_NGH ? m - KH_NGH : g.n3 + m - KH_NGH;
-  } else if (t < nA + nB) {
-    t -= nA;
-    a = (int)(t % g.nt1) - KH_NGH; long r = t / g.nt1;
-    int m = (int)(r % (2 * KH_NGH)); c = (int)(r / (2 * KH_NGH));
+  if (u < nA) {
+    const unsigned r = u / nt1, q = r / nt2;
+    a = (int)(u - r * nt1) - KH_NGH;
+    b = (int)(r - q * nt2) - KH_NGH;
+    c = (int)q < KH_NGH ? (int)q - KH_NGH : g.n3 + (int)q - KH_NGH;
+  } else if (u < nA + nB) {
+    u -= nA;
+    const unsigned r = u / nt1, q = r / (2u * KH_NGH);
+    const int m = (int)(r - q * (2u * KH_NGH));
+    a = (int)(u - r * nt1) - KH_NGH;
+    c = (int)q;
     b = m < KH_NGH ? m - KH_NGH : g.n2 + m - KH_NGH;
-  } else if (t < nA + nB + nC) {
-    t -= nA + nB;
-    int m = (int)(t % (2 * KH_NGH)); long r = t / (2 * KH_NGH);
-    b = (int)(r % g.n2); c = (int)(r / g.n2);
-    a = m < KH_NGH ? m - KH_NGH : g.n1 + m - KH_NGH;
   } else {
-    return;
+    u -= nA + nB;
+    const unsigned r = u / (2u * KH_NGH), q = r / (unsigned)g.n2;
+    const int m = (int)(u - r * (2u * KH_NGH));
+    b = (int)(r - q * (unsigned)g.n2);
+    c = (int)q;
+    a = m < KH_NGH ? m - KH_NGH : g.n1 + m - KH_NGH;
   }
   int k1, k2, k3;
   const int s1 = ghost_map(a, g.n1, g.bc[0], g.bc[1], k1);
@@ -978,18 +986,25 @@ __device__ __forceinline__ void fill_zone(const GV& g, double* __restrict__ P, u
   if (k1 == KH_MAP_ID && k2 == KH_MAP_ID && k3 == KH_MAP_ID) return;      // fixed ghost (or nothing to do)
   const long ng = zidx(g, a, b, c), ns = zidx(g, s1, s2, s3), nt = g.ntot;
   if (P) {
+    // all loads first: source and ghost zone are in the same array, so a load written after a store would have to wait for it
+    // (one DRAM round trip per variable instead of one per zone); the sqrt(-g) ratios of the outflow ghosts come after them
+    double val[KH_NP];
+#pragma unroll
+    for (int v = 0; v < KH_NP; v++) val[v] = P[v * nt + ns];
+    const unsigned char fl = flag ? flag[ns] : (unsigned char)0;
     const double* gd = g.geom[0] + 20 * g.n2d;
     double r1 = 1.0, r2 = 1.0;
     if (k1 == KH_MAP_OUTFLOW) r1 = __ldg(gd + pidx(g, s1, s2)) / __ldg(gd + pidx(g, a, s2));     // pass 1 acts on row s2
     if (k2 == KH_MAP_OUTFLOW) r2 = __ldg(gd + pidx(g, a, s2)) / __ldg(gd + pidx(g, a, b));       // pass 2 acts on column a
 #pragma unroll
     for (int v = 0; v < KH_NP; v++) {
-      double val = P[v * nt + ns];
-      if (v >= B1) { if (k1 == KH_MAP_OUTFLOW) val *= r1; }
-      if (k2 == KH_MAP_POLAR && (v == U2 || v == B2)) val = -val;
-      if (v >= B1) { if (k2 == KH_MAP_OUTFLOW) val *= r2; }
-      P[v * nt + ng] = val;
+      if (v >= B1) { if (k1 == KH_MAP_OUTFLOW) val[v] *= r1; }
+      if (k2 == KH_MAP_POLAR && (v == U2 || v == B2)) val[v] = -val[v];
+      if (v >= B1) { if (k2 == KH_MAP_OUTFLOW) val[v] *= r2; }
+      P[v * nt + ng] = val[v];
     }
+    if (flag) flag[ng] = fl;
+    return;
   }
   if (flag) flag[ng] = flag[ns];
 }
@@ -1017,11 +1032,16 @@ __device__ __forceinline__ void zone_of(const GV& g, long n, int& i, int& j, int
 }
 
 // One warp per failed zone: lane l < 26 owns one neighbour (independent loads in flight), butterfly sums.
+// MAPPED: a neighbour in a ghost layer is read from the zone the ghost fill copies it from (with the polar sign flip of ut^2;
+// outflow scales the field only) instead of from the ghost zone itself -- the same values, but the gather then does not
+// depend on the fill and runs in the same launch (fill_gather_kernel).  `bid`, `nb`: the block's number among the gather blocks.
+template <bool MAPPED>
 __device__ __forceinline__ void fixup_gather(const GV& g, const double* __restrict__ Pf, const unsigned char* __restrict__ pflag,
-                                             const unsigned* __restrict__ list, double* __restrict__ fix, const StepScalars* __restrict__ sc) {
+                                             const unsigned* __restrict__ list, double* __restrict__ fix, const StepScalars* __restrict__ sc,
+                                             unsigned bid, unsigned nblk) {
   const long count = (long)sc->n_pflag, nt = g.ntot;
   const int lane = threadIdx.x & 31;
-  const long warp = ((long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = ((long)gridDim.x * blockDim.x) >> 5;
+  const long warp = ((long)bid * blockDim.x + threadIdx.x) >> 5, nwarp = ((long)nblk * blockDim.x) >> 5;
   // lane -> neighbour offset (skipping the centre, index 13 of the 3x3x3 box)
   const int c = lane < 13 ? lane : lane + 1;
   const int di = c % 3 - 1, dj = (c / 3) % 3 - 1, dk = c / 9 - 1;
@@ -1029,11 +1049,25 @@ __device__ __forceinline__ void fixup_gather(const GV& g, const double* __restri
   const double w = nb ? 1.0 / (double)(abs(di) + abs(dj) + abs(dk) + 1) : 0.0;
   for (long q = warp; q < count; q += nwarp) {
     const long n = list[q];
-    const long m = nb ? n + dk * g.s3 + dj * g.s2 + di : n;
+    long m = nb ? n + dk * g.s3 + dj * g.s2 + di : n;
+    bool flip = false;
+    if (MAPPED && nb) {
+      int i, j, k, k1, k2, k3;
+      zone_of(g, n, i, j, k);
+      const int s1 = ghost_map(i + di, g.n1, g.bc[0], g.bc[1], k1);
+      const int s2 = ghost_map(j + dj, g.n2, g.bc[2], g.bc[3], k2);
+      const int s3 = ghost_map(k + dk, g.n3, g.bc[4], g.bc[5], k3);
+      m = zidx(g, s1, s2, s3);
+      flip = k2 == KH_MAP_POLAR;
+    }
     const double wg = (nb && pflag[m] == 0) ? w : 0.0;
     double sum[5], sall[5], wsum = wg, wall = w;
 #pragma unroll
-    for (int v = 0; v < 5; v++) { double val = Pf[v * nt + m]; sall[v] = w * val; sum[v] = wg * val; }
+    for (int v = 0; v < 5; v++) {
+      double val = Pf[v * nt + m];
+      if (MAPPED && v == U2 && flip) val = -val;
+      sall[v] = w * val; sum[v] = wg * val;
+    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
       wsum += __shfl_xor_sync(0xffffffffu, wsum, o);
@@ -1053,7 +1087,19 @@ __device__ __forceinline__ void fixup_gather(const GV& g, const double* __restri
 __global__ void __launch_bounds__(128)
 fixup_gather_kernel(GV g, const double* __restrict__ Pf, const unsigned char* __restrict__ pflag, const unsigned* __restrict__ list,
                     double* __restrict__ fix, const StepScalars* __restrict__ sc) {
-  fixup_gather(g, Pf, pflag, list, fix, sc);
+  fixup_gather<false>(g, Pf, pflag, list, fix, sc, blockIdx.x, gridDim.x);
+}
+// Ghost fill and the fix-up's gather in ONE launch (two launches of a few microseconds each are mostly launch latency): the
+// first `gather_blocks` blocks gather with mapped neighbours (they read interior zones only, the fill writes ghost zones
+// only), the others fill.  The gather blocks come first so that their chain of dependent loads starts at once.
+#ifndef KH_MINB_FILL
+#define KH_MINB_FILL 1
+#endif
+__global__ void __launch_bounds__(128, KH_MINB_FILL)
+fill_gather_kernel(GV g, double* P, unsigned char* flag, const unsigned* __restrict__ list, double* __restrict__ fix,
+                   const StepScalars* __restrict__ sc, unsigned gather_blocks) {
+  if (blockIdx.x < gather_blocks) fixup_gather<true>(g, P, flag, list, fix, sc, blockIdx.x, gather_blocks);
+  else fill_zone(g, P, flag, (long)(blockIdx.x - gather_blocks) * blockDim.x + threadIdx.x);
 }
 
 template <bool FLAT>

@@ -315,14 +315,26 @@ static void launch_flux(kh_grid* g, const double* Ps, cudaStream_t stream, bool 
 }
 
 // Fix-up of the zones on the failure list (+ floors, + their ghost images).
-static int do_fixup(kh_grid* g, double* Pf) {
+static int do_fixup(kh_grid* g, double* Pf, bool gathered = false) {
   const GV& v = g->gv;
   prof_begin(g, KH_K_FIXUP);
-  fixup_gather_kernel<<<64, 128, 0, g->stream>>>(v, Pf, g->pflag, g->faillist, g->fix, g->sc);
+  if (!gathered) fixup_gather_kernel<<<64, 128, 0, g->stream>>>(v, Pf, g->pflag, g->faillist, g->fix, g->sc);
   if (g->flat) fixup_apply_kernel<true><<<64, 128, 0, g->stream>>>(v, Pf, g->faillist, g->fflag, g->fix, g->sc);
   else fixup_apply_kernel<false><<<64, 128, 0, g->stream>>>(v, Pf, g->faillist, g->fflag, g->fix, g->sc);
   prof_end(g);
-  g->launches += 2;
+  g->launches += gathered ? 1 : 2;
+  CK(cudaGetLastError());
+  return KH_OK;
+}
+
+// Ghost fill of the sub-step's result together with the fix-up's gather (fill_gather_kernel)
+static int fill_ghosts_and_gather(kh_grid* g, double* Pf) {
+  const GV& v = g->gv;
+  const long shell = (long)v.nt1 * v.nt2 * (2 * KH_NGH) + (long)v.nt1 * (2 * KH_NGH) * v.n3 + (long)(2 * KH_NGH) * v.n2 * v.n3;
+  prof_begin(g, KH_K_FILL);
+  fill_gather_kernel<<<(unsigned)((shell + 127) / 128) + 64u, 128, 0, g->stream>>>(v, Pf, g->pflag, g->faillist, g->fix, g->sc, 64u);
+  prof_end(g);
+  g->launches += 1;
   CK(cudaGetLastError());
   return KH_OK;
 }
@@ -448,9 +460,9 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
     }
   }
   if (!with_fixup) return fill_ghosts(g, Pf, g->pflag);          // linked blocks: halo exchange, fix-up, halo exchange follow (kh_step_blocks)
-  int rc = fill_ghosts(g, Pf, g->pflag);
+  int rc = fill_ghosts_and_gather(g, Pf);
   if (rc) return rc;
-  return do_fixup(g, Pf);      // also refreshes the ghost images of the fixed zones (the second fill of S22)
+  return do_fixup(g, Pf, true);      // also refreshes the ghost images of the fixed zones (the second fill of S22)
 }
 
 static int enqueue_step(kh_grid* g, int cur) {
@@ -610,6 +622,9 @@ int kh_grid_create(const kh_params* p, void* cuda_stream, kh_grid** out) {
   v.nt1 = v.n1 + 2 * KH_NGH; v.nt2 = v.n2 + 2 * KH_NGH; v.nt3 = v.n3 + 2 * KH_NGH;
   v.s2 = v.nt1; v.s3 = (long)v.nt1 * v.nt2; v.ntot = v.s3 * v.nt3;
   v.n2d = (long)v.nt1 * v.nt2;
+  // zone numbers are held in 32 bits in several kernels (failure list, fill and update tile indices); 8 x ntot doubles of one
+  // state array beyond that would not fit the device anyway
+  if (v.ntot >= (1L << 31)) { kh_grid_destroy(g); return KH_EINVAL; }
   v.idx1 = v.n1 / (p->xmax[0] - p->xmin[0]); v.idx2 = v.n2 / (p->xmax[1] - p->xmin[1]); v.idx3 = v.n3 / (p->xmax[2] - p->xmin[2]);
   v.gam = p->gamma;
   for (int b = 0; b < 6; b++) v.bc[b] = p->bc[b];
