@@ -382,7 +382,7 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
                                                                                                 g->ecent[2], g->ecent[3], g->emf[0], g->emf[1], g->emf[2]);
       g->launches++;
     } else {
-      emf_kernel<<<zone_grid(v.n1 + 1, v.n2 + 1, v.n3 + 1), 128, 0, g->stream>>>(v, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], g->emf[2]);
+      emf_kernel<<<dim3((unsigned)(((long)(v.n1 + 1) * (v.n2 + 1) + 127) / 128), (unsigned)(v.n3 + 1)), 128, 0, g->stream>>>(v, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], g->emf[2]);
     }
     prof_end(g);
     g->launches++;
