@@ -84,7 +84,9 @@ typedef struct kh_grid kh_grid;   /* opaque */
 /* Create a grid on the current CUDA device and run the one-time geometry precompute (kernel K1:
  * gcov, gcon, sqrt(-g), lapse at zone centres and the three face centres, connection coefficients
  * and floor profiles at centres; the "caches of expensive-to-calculate quantities" of P:285).
- * cuda_stream: a cudaStream_t (as void*), or NULL: the grid then creates its own blocking stream. */
+ * cuda_stream: a cudaStream_t (as void*), or NULL: the grid then creates its own blocking stream.
+ * Errors: KH_EINVAL for parameters out of range, also for a block of 2^31 or more zones with ghosts (zone numbers are held
+ * in 32 bits; one state array of such a block would not fit a device); KH_ENOMEM; KH_ECUDA. */
 int kh_grid_create(const kh_params* params, void* cuda_stream, kh_grid** out);
 int kh_grid_destroy(kh_grid* g);
 /* The stream every call on this grid enqueues on (a cudaStream_t as void*), and a wait for all of it. */
