@@ -188,6 +188,9 @@ def test_stream_device_and_error_paths(kh):
     gb.set_prims(bad)
     with pytest.raises(kh.KharmError, match="non-finite"):
         gb.estimate_dt()
+    # a block of 2^31 or more zones (with ghosts) is refused before anything is allocated: zone numbers are held in 32 bits
+    with pytest.raises(kh.KharmError, match="invalid argument"):
+        kh.Grid(dict(p, n1=2000, n2=1100, n3=1000))
 
 
 def test_step_falls_back_to_direct_launches_when_the_stream_cannot_be_captured(kh):
