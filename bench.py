@@ -78,8 +78,8 @@ ALG_FLOPS = {
 # DRAM traffic per launch (bytes) of the default workload's kernels: dram__bytes_read.sum + dram__bytes_write.sum of one
 # `ncu --set full` capture (update = mean of the predictor and the corrector launch).  Source file in profiles/.
 NCU_DRAM_SOURCE = "profiles/r02_ncu_full.md"
-NCU_DRAM_BYTES_PER_LAUNCH = {"flux1": 215.7e6 + 165.2e6, "flux2": 229.0e6 + 166.6e6, "flux3": 227.6e6 + 165.0e6, "emf": 159.6e6 + 53.0e6,
-                             "update": 0.5 * (1069.3e6 + 192.1e6 + 728.2e6 + 188.0e6)}
+NCU_DRAM_BYTES_PER_LAUNCH = {"flux1": 215.7e6 + 165.4e6, "flux2": 229.0e6 + 166.9e6, "flux3": 227.5e6 + 165.8e6, "emf": 159.6e6 + 53.5e6,
+                             "update": 0.5 * (1068.7e6 + 192.4e6 + 728.5e6 + 190.5e6)}
 
 
 def load_peaks():

