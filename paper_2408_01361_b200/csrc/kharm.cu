@@ -398,9 +398,9 @@ static int substep(kh_grid* g, const double* Pi, const double* Ps, double* Pf, d
       fb1 = Bff[0]; fb2 = Bff[1]; fb3 = Bff[2];
     }
     const unsigned grid = (unsigned)(((long)v.n1 * v.n2 * v.n3 + 127) / 128);
-    // persistent: as many blocks as stay resident (4 per SM), never more than there are groups of 4 warp tiles
-    const long tgroups = (long)((v.n1 + 31) / 32) * v.n2 * ((v.n3 + 16 * KH_UPD_TPW - 1) / (16 * KH_UPD_TPW));      // work units of update_tma_kernel
-    const unsigned tgrid = (unsigned)(tgroups < (long)g->sm_count ? tgroups : (long)g->sm_count) * (16 / KH_UPD_WARPS);
+    // persistent: one block of 16 warps per SM, never more blocks than there are work units (update_tma_kernel)
+    const long tunits = (long)((v.n1 + 31) / 32) * v.n2 * ((v.n3 + 16 * KH_UPD_TPW - 1) / (16 * KH_UPD_TPW));
+    const unsigned tgrid = (unsigned)(tunits < (long)g->sm_count ? tunits : (long)g->sm_count);
 #define UPD_ARGS v, Pi, Ps, Pf, g->F[0], g->F[1], g->F[2], g->emf[0], g->emf[1], g->emf[2], g->ctop[0], g->ctop[1], g->ctop[2], g->pflag, \
                  g->fflag, g->faillist, g->sc, dt_factor, fb1, fb2, fb3
     TileMaps M;
