@@ -472,7 +472,8 @@ struct GlobalAcc {
 // Layout of a warp's tile (32 zones of one x1 row) in shared memory, in doubles.  One REGION per tensor copy (a box of one
 // array: dense [v][k][j][i] as the TMA unit writes it), each starting on a 128 B boundary.  Rows whose x1 neighbour i+1 is read
 // hold 34 doubles (272 B: the box's inner extent must be a multiple of 16 B), the others 32.  c_top is not staged (its six
-// values per zone are loaded before the wait): the tile of the corrector is then exactly what four blocks per SM can hold.
+// values per zone are loaded before the wait): 16 corrector tiles and the two geometry buffers of update_tma_kernel then just fit
+// the 227 KB of shared memory of an SM.
 __host__ __device__ constexpr int tile_pad(int doubles) { return (doubles + 15) / 16 * 16; }
 template <bool FLAT, bool CORR, int MODE>
 struct TileLayout {
@@ -682,7 +683,8 @@ update_kernel(GV g, const double* __restrict__ Pi, const double* __restrict__ Ps
 // x1 row.  One elected lane issues 8 (predictor) or 9 (corrector) TMA tensor copies (cp.async.bulk.tensor, completion on the
 // warp's mbarrier) -- one box per input array: 5 flux components x 2 faces, 4 edge EMFs, 8 primitives ... -- 10 - 12 KB per warp,
 // so that ALL streamed inputs of the tile are in flight at once and cost neither registers nor issue slots of the other lanes;
-// the geometry and c_top loads go out meanwhile.  After the wait the zone arithmetic reads shared memory only.  (The per-thread
+// the c_top loads go out meanwhile (the geometry is staged per work unit, below).  After the wait the zone arithmetic reads
+// shared memory only.  (The per-thread
 // variant keeps ~5 loads in flight per warp and spends 58 % of its cycles with every warp waiting on one of five dependent load
 // phases; 41 - 54 row-wise bulk copies instead of the boxes cost 13 % of the kernel's instructions in address arithmetic:
 // profiles/r02_*.)
